@@ -1,0 +1,240 @@
+"""Pins for the oracle's Magnus steps (SURVEY.md 8(c) pins c-P6..c-P11).
+
+References are independent of the oracle: numpy.linalg.eigh exponentials, a
+brute-force fine-step propagator, closed forms for commuting operators, and the
+convergence order the paper states (PAPER.md lines 97-101 Method 2 "order
+four", lines 130-134 Method 4 "order 4", line 156 Figure 1).
+"""
+import math
+
+import numpy as np
+import pytest
+
+import workloads as W
+from workloads import xxz
+
+
+def rand_herm(n, seed, scale=1.0):
+    r = np.random.default_rng(seed)
+    G = r.normal(size=(n, n)) + 1j * r.normal(size=(n, n))
+    return scale * (G + G.conj().T) / 2
+
+
+def rand_vec(n, seed):
+    r = np.random.default_rng(seed)
+    v = r.normal(size=n) + 1j * r.normal(size=n)
+    return v / np.linalg.norm(v)
+
+
+def expm_h(M, h):
+    lam, U = np.linalg.eigh(M)
+    return (U * np.exp(-1j * h * lam)) @ U.conj().T
+
+
+def brute_force(H0, H1, f, t0, t1, psi, nfine=4000):
+    """psi(t1) by the exponential midpoint rule with exact small exponentials on a very
+    fine grid (error O(dt^2) ~ 1e-8 * const): an integrator that shares nothing with
+    the Gauss-node schemes under test."""
+    dt = (t1 - t0) / nfine
+    for k in range(nfine):
+        psi = expm_h(H0 + f(t0 + (k + 0.5) * dt) * H1, dt) @ psi
+    return psi
+
+
+def csr_pair(oracle, N):
+    return oracle.CsrHost.of(xxz.xxz_h0(N)), oracle.CsrHost.of(xxz.xxz_h1(N))
+
+
+# ------------------------------------------------------------------ c-P6
+@pytest.mark.parametrize("scheme", ["cf4", "m4"])
+@pytest.mark.parametrize("nsteps", [1, 3, 8])
+def test_time_independent_hamiltonian_is_exact(oracle, scheme, nsteps):
+    n = 24
+    H0, H1 = rand_herm(n, 1, 0.5), rand_herm(n, 2, 0.5)
+    psi0 = rand_vec(n, 3)
+    fc = 0.37
+    psi, iters = oracle.magnus_integrate(H0, H1, lambda t: fc, scheme, 0.0, 0.9, nsteps, psi0)
+    ref = expm_h(H0 + fc * H1, 0.9) @ psi0
+    assert np.linalg.norm(psi - ref) < 2e-11
+    assert len(iters) == nsteps * (2 if scheme == "cf4" else 1) and np.all(iters > 0)
+
+
+# ------------------------------------------------------------------ c-P7
+def test_commuting_operators(oracle):
+    n = 20
+    U = np.linalg.qr(rand_herm(n, 4))[0]
+    r = np.random.default_rng(5)
+    H0 = (U * r.normal(size=n)) @ U.conj().T
+    H1 = (U * r.normal(size=n)) @ U.conj().T
+    H0, H1 = (H0 + H0.conj().T) / 2, (H1 + H1.conj().T) / 2
+    K = oracle.commutator(H0, H1)
+    assert np.abs(K).max() < 1e-14
+    f = lambda t: math.cos(2 * t)
+    psi0 = rand_vec(n, 6)
+    T, ns = 0.8, 4
+    tau = T / ns
+    c1, c2 = 0.5 - math.sqrt(3) / 6, 0.5 + math.sqrt(3) / 6
+    Q = sum(tau / 2 * (f(s * tau + c1 * tau) + f(s * tau + c2 * tau)) for s in range(ns))
+    ref = expm_h(H0 * T + H1 * Q, 1.0) @ psi0
+    a, _ = oracle.magnus_integrate(H0, H1, f, "cf4", 0.0, T, ns, psi0)
+    b, _ = oracle.magnus_integrate(H0, H1, f, "m4", 0.0, T, ns, psi0)
+    assert np.linalg.norm(a - ref) < 1e-11 and np.linalg.norm(b - ref) < 1e-11
+    assert np.linalg.norm(a - b) < 1e-11
+
+
+# ------------------------------------------------------------------ c-P8
+def observed_order(oracle, H0, H1, f, scheme, psi0, T, ref, steps=(4, 8, 16)):
+    errs = []
+    for ns in steps:
+        psi, _ = oracle.magnus_integrate(H0, H1, f, scheme, 0.0, T, ns, psi0, tol=1e-14)
+        errs.append(np.linalg.norm(psi - ref))
+    slopes = [math.log2(errs[i] / errs[i + 1]) for i in range(len(errs) - 1)]
+    return errs, slopes
+
+
+def test_fourth_order_dense_and_negative_control(oracle):
+    n = 12
+    H0, H1 = rand_herm(n, 7, 0.6), rand_herm(n, 8, 0.6)
+    f = lambda t: math.sin(3 * t)
+    psi0 = rand_vec(n, 9)
+    T = 1.0
+    ref = brute_force(H0, H1, f, 0.0, T, psi0, nfine=20000)   # error ~1e-9, below the errors measured
+    for scheme in ("cf4", "m4"):
+        errs, slopes = observed_order(oracle, H0, H1, f, scheme, psi0, T, ref, steps=(8, 16, 32))
+        assert all(3.7 < s < 4.4 for s in slopes), (scheme, errs, slopes)
+    errs, slopes = observed_order(oracle, H0, H1, f, "m4_wrong_sign", psi0, T, ref, steps=(8, 16, 32))
+    assert all(1.7 < s < 2.3 for s in slopes), ("flipped commutator must drop to order 2", errs, slopes)
+
+
+def test_fourth_order_xxz_csr_self_convergence(oracle):
+    """Order on the sparse path; reference = same scheme at a 16x finer step (pin c-P8)."""
+    N = 6
+    H0, H1 = csr_pair(oracle, N)
+    psi0 = xxz.neel_state(N).numpy()
+    f = xxz.f_cos2t
+    T = 0.5
+    for scheme in ("cf4", "m4"):
+        ref, _ = oracle.magnus_integrate(H0, H1, f, scheme, 0.0, T, 256, psi0, tol=1e-14)
+        errs, slopes = observed_order(oracle, H0, H1, f, scheme, psi0, T, ref, steps=(4, 8, 16))
+        assert all(3.8 < s < 4.2 for s in slopes), (scheme, errs, slopes)
+    # and both schemes converge to the SAME solution (brute force, dense copy of the chain)
+    D0, D1 = xxz.xxz_h0(N).to_scipy().toarray(), xxz.xxz_h1(N).to_scipy().toarray()
+    bf = brute_force(D0, D1, f, 0.0, T, psi0, nfine=8000)
+    for scheme in ("cf4", "m4"):
+        psi, _ = oracle.magnus_integrate(H0, H1, f, scheme, 0.0, T, 64, psi0)
+        assert np.linalg.norm(psi - bf) < 5e-8
+
+
+# ------------------------------------------------------------------ c-P9
+def test_cf4_vs_m4_and_error_constant(oracle):
+    n = 16
+    H0, H1 = rand_herm(n, 11, 0.5), rand_herm(n, 12, 0.5)
+    f = lambda t: math.sin(3 * t)
+    psi0 = rand_vec(n, 13)
+    ref = brute_force(H0, H1, f, 0.0, 1.0, psi0, nfine=20000)
+    d = []
+    for ns in (4, 8):
+        a, _ = oracle.magnus_integrate(H0, H1, f, "cf4", 0.0, 1.0, ns, psi0)
+        b, _ = oracle.magnus_integrate(H0, H1, f, "m4", 0.0, 1.0, ns, psi0)
+        d.append(np.linalg.norm(a - b))
+        # "Cf4 ... is somewhat more accurate compared to the M4 method"
+        assert np.linalg.norm(a - ref) < np.linalg.norm(b - ref)
+    assert 3.5 < math.log2(d[0] / d[1]) < 4.5          # the two differ by O(tau^4)
+
+
+# ------------------------------------------------------------------ c-P10
+@pytest.mark.parametrize("scheme", ["cf4", "m4"])
+def test_time_reversal_symmetry(oracle, scheme):
+    n = 16
+    H0, H1 = rand_herm(n, 14, 0.5), rand_herm(n, 15, 0.5)
+    f = lambda t: math.sin(3 * t)
+    psi0 = rand_vec(n, 16)
+    psi1, _ = oracle.magnus_step(H0, H1, f, scheme, 0.2, 0.1, psi0)
+    back, _ = oracle.magnus_step(H0, H1, f, scheme, 0.3, -0.1, psi1)
+    assert np.linalg.norm(back - psi0) < 1e-11
+    assert abs(np.linalg.norm(psi1) - 1) < 1e-10
+
+
+# ------------------------------------------------------------------ c-P11
+def test_commutator_identities(oracle):
+    n = 18
+    A, B = rand_herm(n, 17), rand_herm(n, 18)
+    K = oracle.commutator(A, B)
+    assert np.allclose(K, A @ B - B @ A, atol=1e-13)
+    P = A @ B
+    assert np.allclose(K, P - P.conj().T, atol=1e-13)          # Hermitian operands
+    assert np.allclose(K, -K.conj().T, atol=1e-13) and abs(np.trace(K)) < 1e-12
+    # [H(t2), H(t1)] = (f1 - f2) [H0, H1]
+    f1, f2 = 0.3, -0.8
+    K21 = oracle.commutator(A + f2 * B, A + f1 * B)
+    assert np.allclose(K21, (f1 - f2) * oracle.commutator(A, B), atol=1e-12)
+
+
+def test_sparse_commutator_matches_dense(oracle):
+    N = 5
+    H0, H1 = csr_pair(oracle, N)
+    K = oracle.commutator(H0, H1)
+    import scipy.sparse as sp
+    Ks = sp.csr_matrix((K.values, K.col_idx, K.row_ptr), shape=(K.n, K.n)).toarray()
+    D0, D1 = xxz.xxz_h0(N).to_scipy().toarray(), xxz.xxz_h1(N).to_scipy().toarray()
+    assert np.array_equal(Ks, D0 @ D1 - D1 @ D0)
+    assert np.all(Ks.imag == 0) and np.array_equal(Ks, -Ks.T)   # real antisymmetric
+    nz = Ks != 0
+    assert np.all(D1[nz] != 0)                                   # pattern inside H1's
+    assert nz.sum() == N * 2 ** (N - 1)
+
+
+def test_sparse_and_dense_steps_agree(oracle):
+    N = 5
+    H0, H1 = csr_pair(oracle, N)
+    D0, D1 = xxz.xxz_h0(N).to_scipy().toarray(), xxz.xxz_h1(N).to_scipy().toarray()
+    psi0 = rand_vec(32, 19)
+    for scheme in ("cf4", "m4"):
+        a, ia = oracle.magnus_step(H0, H1, xxz.f_cos2t, scheme, 0.1, 0.05, psi0)
+        b, ib = oracle.magnus_step(D0, D1, xxz.f_cos2t, scheme, 0.1, 0.05, psi0)
+        assert np.linalg.norm(a - b) < 1e-13
+        assert [i["iters"] for i in ia] == [i["iters"] for i in ib]
+        assert [i["a"] for i in ia] == [i["a"] for i in ib]
+
+
+def test_single_step_matches_scheme_formula_with_exact_exponentials(oracle):
+    """One step against the printed formulas evaluated with
+    eigendecomposition exponentials of A = -iH."""
+    n = 10
+    H0, H1 = rand_herm(n, 20, 0.5), rand_herm(n, 21, 0.5)
+    f = lambda t: math.sin(3 * t)
+    psi0 = rand_vec(n, 22)
+    t, tau = 0.4, 0.2
+    c1, c2 = 0.5 - math.sqrt(3) / 6, 0.5 + math.sqrt(3) / 6
+    Ha, Hb = H0 + f(t + c1 * tau) * H1, H0 + f(t + c2 * tau) * H1    # H(t1), H(t2)
+    A1, A2 = -1j * Ha, -1j * Hb
+    a1, a2 = (3 - 2 * math.sqrt(3)) / 12, (3 + 2 * math.sqrt(3)) / 12
+
+    def expm_general(X):            # X = -i * Hermitian
+        return expm_h(1j * X, 1.0)
+
+    ref_cf4 = expm_general(tau * (a1 * A1 + a2 * A2)) @ (expm_general(tau * (a2 * A1 + a1 * A2)) @ psi0)
+    Om = tau / 2 * (A1 + A2) + math.sqrt(3) * tau ** 2 / 12 * (A2 @ A1 - A1 @ A2)
+    ref_m4 = expm_general(Om) @ psi0
+    got_cf4, _ = oracle.magnus_step(H0, H1, f, "cf4", t, tau, psi0)
+    got_m4, _ = oracle.magnus_step(H0, H1, f, "m4", t, tau, psi0)
+    assert np.linalg.norm(got_cf4 - ref_cf4) < 1e-11
+    assert np.linalg.norm(got_m4 - ref_m4) < 1e-11
+
+
+def test_cfg1_totals_are_stable(oracle):
+    """CFG1 end to end on the oracle: norm conserved to 1e-10 (north_star), CF4 and M4
+    agree to O(tau^4); the iteration totals are recorded in tests/golden by
+    tests/golden/make_golden.py (oracle-only) and must not drift silently."""
+    import json, os
+    cfg = W.CONFIGS["cfg1"]
+    H0, H1, psi0, f = W.build(cfg)
+    H0, H1 = oracle.CsrHost.of(H0), oracle.CsrHost.of(H1)
+    out = {}
+    for scheme in cfg.schemes:
+        psi, iters = oracle.magnus_integrate(H0, H1, f, scheme, cfg.t0, cfg.t_end, cfg.nsteps, psi0.numpy(), cfg.tol)
+        assert abs(np.linalg.norm(psi) - 1) < 1e-10
+        out[scheme] = (psi, int(iters.sum()))
+    assert 1e-10 < np.linalg.norm(out["cf4"][0] - out["m4"][0]) < 1e-8
+    gold = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "cfg1_oracle.json")))
+    assert out["cf4"][1] == gold["cf4"]["total_matvecs"] and out["m4"][1] == gold["m4"]["total_matvecs"]
