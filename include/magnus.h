@@ -1,0 +1,231 @@
+/* magnus.h -- C-ABI of the B200-native Magnus/Leja library (libmagnus_b200.so).
+ *
+ * Hot path of arXiv 1709.06483 ("Magnus integrators on multicore CPUs and
+ * GPUs"): one time step of the 4th-order Magnus integrators Cf4 and M4 for
+ *     i dpsi/dt = H(t) psi,   H(t) = H0 + f(t) H1            (eq. (1), l.17; l.237)
+ * with exp(-i h M) v computed by Newton interpolation at Leja points
+ * (section 3, l.169-190) on a Gershgorin spectral interval.
+ *
+ * "P:n" below = /root/reference/PAPER.md line n.  "c1..c7" = the readings of
+ * the paper listed in DESIGN.md section 3.
+ *
+ * Conventions common to every call
+ *   - complex128 everywhere: interleaved (re, im) doubles == cuDoubleComplex ==
+ *     torch.complex128.  Indices are int32, 0-based.
+ *   - "device" pointers are CUDA device pointers of the current device (e.g. a
+ *     torch tensor's data_ptr()); "host" pointers are ordinary host memory.
+ *     Unless a call says otherwise, matrix and vector pointers are DEVICE.
+ *   - Every call returns an int: MAGNUS_OK (0) or a negative MAGNUS_E* code.
+ *     No exception or abort crosses the ABI.  magnus_last_error() returns a
+ *     thread-local human-readable detail for the last failure.
+ *   - Ownership: the caller owns H0, H1, psi, v; the library never frees,
+ *     reallocates or writes H0/H1.  A handle owns only its own workspace.
+ *   - Work is enqueued on the options' stream (0 = the legacy default stream;
+ *     pass torch.cuda.current_stream().cuda_stream).  Calls synchronise that
+ *     stream where a scalar must reach the host (spectral interval, stop test).
+ *   - Calls on one handle are not thread-safe.  There is no CPU fallback: with
+ *     no usable CUDA device every compute call returns MAGNUS_ECUDA.
+ */
+#ifndef MAGNUS_B200_H
+#define MAGNUS_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MAGNUS_OK             0
+#define MAGNUS_EINVAL        -1   /* bad argument (null pointer, n <= 0, format mismatch, ...) */
+#define MAGNUS_ENOMEM        -2   /* device or host allocation failed */
+#define MAGNUS_ECUDA         -3   /* a CUDA runtime call or kernel launch failed */
+#define MAGNUS_ENOCONV       -4   /* m_max reached without meeting tol; psi / v_out unspecified */
+#define MAGNUS_ENOTHERMITIAN -5   /* magnus_create's sampled Hermitian check failed */
+
+#define MAGNUS_DENSE 0            /* row-major n x n, leading dimension ld >= n (in elements) */
+#define MAGNUS_CSR   1            /* row_ptr[n+1], col_idx[nnz] ascending within a row, values[nnz] */
+
+#define MAGNUS_CF4   0            /* commutator-free, two exponentials  (Method 4) */
+#define MAGNUS_M4    1            /* classical, one commutator          (Method 2) */
+#define MAGNUS_M2    2            /* exponential midpoint rule          (Method 1) */
+#define MAGNUS_CF4_3 3            /* optimised commutator-free, three exponentials (Method 5) */
+
+#define MAGNUS_MAX_EXP_PER_STEP 3
+
+/* Matrix descriptor.  The matrix must be Hermitian: the dense storage is read
+ * ROW-major (reading the same buffer column-major would give conj(H)).
+ * CSR: row_ptr[0] == 0, row_ptr[n] == nnz < 2^31, columns sorted ascending and
+ * unique within a row.  An absent diagonal entry counts as 0. */
+typedef struct magnus_matrix {
+  int32_t format;          /* MAGNUS_DENSE or MAGNUS_CSR */
+  int32_t reserved;
+  int64_t n;               /* dimension */
+  int64_t nnz;             /* CSR: stored entries; dense: ignored */
+  const void* values;      /* complex128: dense n*ld, CSR nnz */
+  const int32_t* col_idx;  /* CSR only */
+  const int32_t* row_ptr;  /* CSR only */
+  int64_t ld;              /* dense only: row stride in elements (0 means n) */
+} magnus_matrix;
+
+/* f(t) of H(t) = H0 + f(t) H1.  Called on the calling host thread, once per
+ * quadrature node per step ("computed sequentially (on the CPU)"). */
+typedef double (*magnus_drive_fn)(double t, void* user);
+
+/* Options; a NULL pointer or a zero field selects the default. */
+typedef struct magnus_options {
+  double tol;          /* Leja stopping tolerance, relative 2-norm (c6); default 1e-12 */
+  double theta_max;    /* |h gamma| per sub-step (c6); default 16 */
+  int32_t m_max;       /* maximal interpolation degree per sub-step (c6); default and maximum 128 */
+  int32_t check_hermitian; /* 1: sampled check in magnus_create (costs a device pass); default 0 */
+  void* stream;        /* cudaStream_t; NULL = legacy default stream */
+  int32_t csr_kernel;  /* 0 auto, 1 force the generic row-per-subwarp kernel, 2 force the row-block kernel */
+  int32_t reserved;
+} magnus_options;
+
+/* What one exponential did (reading c4-c7). */
+typedef struct magnus_expmv_info {
+  int32_t iters;       /* mat-vecs used, summed over sub-steps */
+  int32_t substeps;    /* s = max(1, ceil(|h gamma| / theta_max)) */
+  int32_t status;      /* MAGNUS_OK or MAGNUS_ENOCONV */
+  int32_t reserved;
+  double a, b;         /* snapped Gershgorin interval used */
+  double theta;        /* (h/s) * gamma */
+  double err_est;      /* e_k + e_{k-1} at the stop */
+} magnus_expmv_info;
+
+typedef struct magnus_step_info {
+  int32_t n_exp;       /* exponentials in this step: CF4 2, M4 1, M2 1, CF4:3 3 */
+  int32_t reserved;
+  magnus_expmv_info exp[MAGNUS_MAX_EXP_PER_STEP];
+} magnus_step_info;
+
+typedef struct magnus_stats {
+  int64_t total_matvecs;   /* Leja iterations over the whole call */
+  int64_t n_exp;           /* exponentials computed */
+  int32_t* iters;          /* caller-provided HOST array (nullable): iterations per exponential, call order */
+  int64_t iters_cap;       /* capacity of iters */
+  double seconds_device;   /* CUDA-event time of the whole call on the stream */
+  double seconds_leja;     /* CUDA-event time spent inside fused Leja-iteration kernels (init..stop) */
+  double seconds_commutator; /* CUDA-event time inside the dense commutator GEMM (M4 dense), else 0 */
+  int64_t kernel_launches; /* kernels this call enqueued */
+} magnus_stats;
+
+typedef struct magnus_context* magnus_handle;
+
+/* magnus_create -- set up an integrator for H(t) = H0 + f(t) H1.
+ *   H0, H1  device matrices of the same format and n; BORROWED until magnus_destroy
+ *           (kept alive and unmodified by the caller).
+ *   f,user  the scalar drive; called on the host.
+ *   scheme  MAGNUS_CF4 / MAGNUS_M4 / MAGNUS_M2 / MAGNUS_CF4_3.
+ * Allocates every workspace once (w ping-pong, p, partial-norm buffers; dense: the
+ * assembled matrix, and for M4 the node matrices A1, A2 and the product P; CSR
+ * M4: computes and owns the sparse commutator C = [H0, H1] -- row S0 of the
+ * scope table -- so that a step only rescales it, since
+ * [H(t2), H(t1)] = (f1 - f2) [H0, H1]).
+ * Errors: EINVAL, ENOMEM, ECUDA, ENOTHERMITIAN (only with check_hermitian). */
+int magnus_create(magnus_handle* out, const magnus_matrix* H0, const magnus_matrix* H1,
+                  magnus_drive_fn f, void* user, int scheme, const magnus_options* opt);
+
+/* magnus_destroy -- frees handle-owned memory only.  NULL is allowed. */
+int magnus_destroy(magnus_handle h);
+
+/* leja_expmv -- v_out = exp(-i h H) v_in by Newton interpolation at Leja points
+ * (w = Aw - xi w; p = p + d_i w), on the Gershgorin interval of H
+ * (c4), with the two-term relative stopping test (c6) and
+ * sub-stepping (c6).  H: device matrix (dense or CSR); v_in, v_out: device,
+ * n complex128; v_in == v_out allowed; h may be negative or zero.  Standalone:
+ * allocates and frees a transient workspace.  stream: cudaStream_t or NULL.
+ * info nullable.  Errors: EINVAL, ENOMEM, ECUDA, ENOCONV. */
+int leja_expmv(const magnus_matrix* H, const void* v_in, void* v_out, double h, double tol,
+               void* stream, magnus_expmv_info* info);
+
+/* magnus_step -- one step t -> t + tau of the handle's scheme, psi (device,
+ * n complex128) updated in place.  CF4 (c1): exp(-i tau/2 (H0+g_a H1))
+ * then exp(-i tau/2 (H0+g_b H1)).  M4 (c1): one exponential of
+ * Omega_H = (H(t1)+H(t2))/2 - i (sqrt(3) tau/12) [H(t2),H(t1)] with h = tau; on dense
+ * H the commutator is one FP64 tensor-core complex GEMM per step.  info nullable. */
+int magnus_step(magnus_handle h, double t, double tau, void* psi, magnus_step_info* info);
+
+/* magnus_integrate -- nsteps steps of size tau = (t_end - t0)/nsteps from
+ * t_n = t0 + n tau (a product, not an accumulated sum).  psi device, in place.
+ * Synchronises the stream before returning so that stats (nullable) is valid. */
+int magnus_integrate(magnus_handle h, double t0, double t_end, int64_t nsteps, void* psi,
+                     magnus_stats* stats);
+
+/* magnus_integrate_host -- the same end to end with HOST buffers: H0, H1 (their
+ * values / col_idx / row_ptr pointers are HOST memory, ideally pinned) and
+ * psi_host (n complex128, in place) are copied to the device, a handle is
+ * created, the integration runs, psi is copied back, everything is freed.
+ * This is the call bench.py times for its "e2e" number. */
+int magnus_integrate_host(const magnus_matrix* H0_host, const magnus_matrix* H1_host,
+                          magnus_drive_fn f, void* user, int scheme, const magnus_options* opt,
+                          double t0, double t_end, int64_t nsteps, void* psi_host,
+                          magnus_stats* stats);
+
+/* ---- single kernels of the path, exposed for parity tests and roofline timing ---- */
+
+/* Gershgorin interval of M = H0 + g*H1 (H1 may be NULL: M = H0), raw (unsnapped):
+ * ab_host[0] = min_i(Re M_ii - R_i), ab_host[1] = max_i(Re M_ii + R_i),
+ * R_i = sum_{j != i} |M_ij| over the SUMMED entries (c4).  Device matrices. */
+int magnus_gershgorin(const magnus_matrix* H0, const magnus_matrix* H1, double g, void* stream,
+                      double* ab_host);
+
+/* One fused Leja iteration (row S6 of the scope table) on device vectors:
+ *   w_out = inv_gamma * (H0 + g*H1) w_in - shift * w_in;   p += d * w_out;
+ *   sums_host[0] = sum |w_out|^2, sums_host[1] = sum |p|^2   (after the update).
+ * H1 may be NULL.  w_in and w_out must not alias.  reps >= 1 repeats the launch
+ * (ping-ponging nothing: same inputs) and returns the mean kernel time in
+ * ms_per_launch (nullable), measured with CUDA events on the stream. */
+int magnus_leja_iteration(const magnus_matrix* H0, const magnus_matrix* H1, double g,
+                          const void* w_in, void* w_out, void* p, double inv_gamma, double shift,
+                          double d_re, double d_im, void* stream, int csr_kernel, int reps,
+                          double* sums_host, float* ms_per_launch);
+
+/* C = A * B, dense row-major complex128 n x n (device), by the FP64 tensor-core
+ * (DMMA m8n8k4) kernel used for the M4 commutator (P:262 l.6-7).  C must not
+ * alias A or B.  ms (nullable): CUDA-event time of the launch. */
+int magnus_zgemm(int64_t n, const void* A, int64_t lda, const void* B, int64_t ldb, void* C,
+                 int64_t ldc, void* stream, float* ms);
+
+/* K = A B - B A for Hermitian dense A, B (device): one GEMM P = A B and
+ * K = P - P^H (P:262 l.6-8; exact identity for Hermitian operands).
+ * work: device scratch of n*n complex128. */
+int magnus_commutator_dense(int64_t n, const void* A, const void* B, void* K, void* work,
+                            void* stream);
+
+/* C = A B - B A for CSR A, B (device), exact zeros dropped.  Two-call protocol:
+ * with cap_nnz == 0 only *nnz_out is written; otherwise row_ptr_out[n+1],
+ * col_idx_out, values_out (device, capacity cap_nnz) are filled. */
+int magnus_commutator_csr(const magnus_matrix* A, const magnus_matrix* B, int64_t cap_nnz,
+                          int64_t* nnz_out, int32_t* row_ptr_out, int32_t* col_idx_out,
+                          void* values_out, void* stream);
+
+/* Register-resident micro-benchmarks that fix the ALU-side roofline denominators
+ * (no FP64 peak is in MEASURED_PEAKS.json): DMMA m8n8k4 and plain DFMA, TFLOP/s. */
+int magnus_fp64_peaks(double* dmma_tflops, double* dfma_tflops, void* stream);
+
+/* ---- host-side pieces of the path (no GPU needed; used by the CPU tests) ---- */
+
+/* The first m Leja points of [-2, 2] (c2).  out_host: m doubles, m <= 129. */
+int magnus_host_leja_points(int m, double* out_host);
+
+/* d_k = exp(-i theta x)[l_0..l_k], k < m (c3), out_host: m complex128. */
+int magnus_host_divided_differences(double theta, int m, double* out_host);
+
+/* Widen [a,b] outward to the grid of spacing 2^(ceil(log2(b-a)) - 12) (c4). */
+int magnus_host_snap_interval(double* a, double* b);
+
+/* Per-exponential scalars of one step (c1).  coef_h1[e] multiplies H1 in the e-th
+ * exponential's matrix, h_scale[e]*tau is its h; for M4 kappa_out receives
+ * (sqrt(3) tau / 12) (f1 - f2), the factor of -i [H0, H1].  Returns n_exp. */
+int magnus_host_step_coefficients(int scheme, magnus_drive_fn f, void* user, double t, double tau,
+                                  double* coef_h1, double* h_scale, double* kappa_out);
+
+const char* magnus_strerror(int code);
+const char* magnus_last_error(void);
+const char* magnus_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MAGNUS_B200_H */

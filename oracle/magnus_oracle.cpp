@@ -493,6 +493,11 @@ int oracle_leja_expmv_csr(int64_t n, const int32_t* rp, const int32_t* ci, const
                     reinterpret_cast<cplx*>(v_out), h, tol, info);
 }
 
+// C = A B by the definition (P:262 line 6 "A_4 = A_2 A_1"): the product the commutator is made of.
+void oracle_matmul_dense(int64_t n, const double* A, const double* B, double* Cout) {
+  dense_mul(n, reinterpret_cast<const cplx*>(A), reinterpret_cast<const cplx*>(B), reinterpret_cast<cplx*>(Cout));
+}
+
 // K = A B - B A by the plain definition (P:262 lines 6-8 with A = A2, B = A1).
 void oracle_commutator_dense(int64_t n, const double* A, const double* B, double* K) {
   const cplx* a = reinterpret_cast<const cplx*>(A);

@@ -133,6 +133,14 @@ def leja_expmv(M, v, h: float, tol: float = 1e-12):
     return out, info.as_dict()
 
 
+def matmul(A, B) -> np.ndarray:
+    """Dense A @ B by the i-k-j definition loop (the product inside the commutator)."""
+    A = _c(A, np.complex128); B = _c(B, np.complex128)
+    out = np.empty_like(A)
+    lib().oracle_matmul_dense(C.c_int64(A.shape[0]), _p(A), _p(B), _p(out))
+    return out
+
+
 def commutator(A, B):
     """A B - B A by the plain definition; dense ndarray or CsrHost (returns the same kind)."""
     if isinstance(A, CsrHost):

@@ -1,0 +1,753 @@
+// C-ABI entry points (include/magnus.h) and the host-side step driver:
+// rows S1, S4 and the control flow of S5-S8 ("The control structures are
+// executed in sequence (on the CPU), while the vector and matrix operations ...
+// are parallelized").  Every arithmetic step on vectors and matrices runs in the
+// CUDA kernels of this library; there is no CPU fallback.
+#include "magnus_internal.h"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <vector>
+
+namespace magnus {
+
+static thread_local char g_err[512] = "";
+
+void set_error(const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof g_err, fmt, ap);
+  va_end(ap);
+}
+
+#define CU_TRY(expr)                                                                        \
+  do {                                                                                      \
+    cudaError_t _e = (expr);                                                                \
+    if (_e != cudaSuccess) {                                                                \
+      set_error("%s failed: %s (%s:%d)", #expr, cudaGetErrorString(_e), __FILE__, __LINE__); \
+      return MAGNUS_ECUDA;                                                                  \
+    }                                                                                       \
+  } while (0)
+
+static int require_device() {
+  int count = 0;
+  const cudaError_t e = cudaGetDeviceCount(&count);
+  if (e != cudaSuccess || count <= 0) {
+    set_error("no usable CUDA device (%s); this library has no CPU fallback",
+              e == cudaSuccess ? "device count 0" : cudaGetErrorString(e));
+    cudaGetLastError();
+    return MAGNUS_ECUDA;
+  }
+  return MAGNUS_OK;
+}
+
+static int check_matrix(const magnus_matrix* M, const char* name) {
+  if (!M) { set_error("%s is NULL", name); return MAGNUS_EINVAL; }
+  if (M->n <= 0) { set_error("%s: n must be positive", name); return MAGNUS_EINVAL; }
+  if (!M->values) { set_error("%s: values is NULL", name); return MAGNUS_EINVAL; }
+  if (M->format == MAGNUS_CSR) {
+    if (!M->col_idx || !M->row_ptr) { set_error("%s: CSR needs col_idx and row_ptr", name); return MAGNUS_EINVAL; }
+    if (M->nnz < 0 || M->nnz >= (int64_t)1 << 31) { set_error("%s: nnz must be in [0, 2^31)", name); return MAGNUS_EINVAL; }
+    if (M->n >= (int64_t)1 << 31) { set_error("%s: n must be < 2^31", name); return MAGNUS_EINVAL; }
+  } else if (M->format == MAGNUS_DENSE) {
+    if (M->ld != 0 && M->ld < M->n) { set_error("%s: ld < n", name); return MAGNUS_EINVAL; }
+  } else {
+    set_error("%s: unknown format %d", name, M->format);
+    return MAGNUS_EINVAL;
+  }
+  return MAGNUS_OK;
+}
+
+static int64_t dense_ld(const magnus_matrix* M) { return M->ld ? M->ld : M->n; }
+
+static CsrTerm csr_term(const magnus_matrix* M, double re, double im) {
+  CsrTerm t;
+  t.rp = M->row_ptr;
+  t.ci = M->col_idx;
+  t.v = (const cplx*)M->values;
+  t.coef = make_double2(re, im);
+  t.nnz = M->nnz;
+  return t;
+}
+
+// Either a CSR operator formed on the fly or a dense (assembled) matrix.
+struct OpRef {
+  bool dense;
+  CsrOp csr;
+  DenseOp dns;
+};
+
+static int read_interval(int nblk, Workspace* ws, cudaStream_t st, double* a, double* b) {
+  launch_minmax_finalize(nblk, ws, st);
+  CU_TRY(cudaMemcpyAsync(ws->ab_host, ws->gersh + 2 * kMaxPartials, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+  CU_TRY(cudaStreamSynchronize(st));
+  *a = ws->ab_host[0];
+  *b = ws->ab_host[1];
+  return MAGNUS_OK;
+}
+
+static int op_interval(const OpRef& op, Workspace* ws, cudaStream_t st, double* a, double* b) {
+  const int nblk = op.dense ? launch_dense_gershgorin(op.dns, ws, st) : launch_csr_gershgorin(op.csr, ws, st);
+  return read_interval(nblk, ws, st, a, b);
+}
+
+static int launch_iter(const OpRef& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma, double shift,
+                       cplx dk, Workspace* ws, cudaStream_t st) {
+  return op.dense ? launch_dense_leja_iter(op.dns, w_in, w_out, p, inv_gamma, shift, dk, ws, st)
+                  : launch_csr_leja_iter(op.csr, w_in, w_out, p, inv_gamma, shift, dk, ws, st);
+}
+
+// ---------------------------------------------------------------------------
+// exp(-i h M) v on the RAW Gershgorin interval [a_raw, b_raw] of M (S4-S8).
+//   B = (M - cI)/gamma, theta = (h/s) gamma, d_k = exp(-i theta x)[l_0..l_k]        (c3)
+//   w_0 = v, p_0 = d_0 v;  w_k = (1/gamma) M w_{k-1} - (c/gamma + l_{k-1}) w_{k-1};
+//   p_k = p_{k-1} + d_k w_k                                                          (c5)
+//   stop at the first k >= 1 with e_k + e_{k-1} <= tol ||p_k||, e_k = |d_k| ||w_k||    (c6)
+// The stop test is evaluated on the device after every iteration; iteration
+// kernels launched after it fired return immediately.  The host launches a
+// first chunk sized from the table alone (|d_k| + |d_{k-1}| <= tol) plus two,
+// then polls the device status every four iterations.
+// ---------------------------------------------------------------------------
+static int expmv_on_interval(const OpRef& op, double a_raw, double b_raw, const cplx* v_in, cplx* v_out, double h,
+                             const LejaParams& prm, Workspace* ws, cudaStream_t st, magnus_expmv_info* info) {
+  const int64_t n = op.dense ? op.dns.n : op.csr.n;
+  double a = a_raw, b = b_raw;
+  if (!std::isfinite(a) || !std::isfinite(b)) {
+    set_error("Gershgorin interval is not finite (NaN/Inf in the matrix?)");
+    return MAGNUS_EINVAL;
+  }
+  snap_interval(&a, &b);
+  const double c = 0.5 * (a + b), gamma = 0.25 * (b - a);
+  magnus_expmv_info loc;
+  std::memset(&loc, 0, sizeof loc);
+  loc.a = a;
+  loc.b = b;
+  if (!(gamma > 0.0)) {   // M = c I: exact, no iterations (c4)
+    launch_scale_copy(v_in, v_out, n, make_double2(std::cos(h * c), -std::sin(h * c)), st, ws);
+    loc.substeps = 1;
+    if (info) *info = loc;
+    return MAGNUS_OK;
+  }
+  const int s = std::max(1, (int)std::ceil(std::fabs(h * gamma) / prm.theta_max));
+  const double hs = h / s, theta = hs * gamma;
+  loc.substeps = s;
+  loc.theta = theta;
+
+  const double* l = leja_points();
+  const int full = prm.m_max + 1;
+  int have = std::min(full, std::max(24, (int)std::ceil(2.5 * std::fabs(theta)) + 32));
+  std::vector<std::complex<double>> d(full);
+  divided_differences(theta, have, d.data());
+  auto need = [&](int k) {
+    if (k >= have) {
+      have = full;
+      divided_differences(theta, have, d.data());
+    }
+  };
+  // a-priori length of the first chunk: first k with |d_k| + |d_{k-1}| <= tol, plus 2
+  int first_chunk = prm.m_max;
+  for (int k = 1; k <= prm.m_max; ++k) {
+    need(k);
+    if (std::abs(d[k]) + std::abs(d[k - 1]) <= prm.tol) {
+      first_chunk = std::min(prm.m_max, k + 2);
+      break;
+    }
+  }
+
+  const double inv_gamma = 1.0 / gamma, c_over_gamma = c / gamma;
+  const cplx phase = make_double2(std::cos(hs * c), -std::sin(hs * c));
+  CU_TRY(cudaMemsetAsync(ws->status, 0, sizeof(LejaStatus), st));
+  float ms = 0.f;
+  for (int sub = 0; sub < s; ++sub) {
+    const cplx* src = sub == 0 ? v_in : v_out;
+    if (ws->time_leja) CU_TRY(cudaEventRecord(ws->ev[0], st));
+    launch_leja_init(src, ws->w[0], ws->p, n, make_double2(d[0].real(), d[0].imag()), std::abs(d[0]), ws, st);
+    int k = 0;
+    bool done = false;
+    int chunk_end = first_chunk;
+    while (!done && k < prm.m_max) {
+      for (; k < chunk_end;) {
+        ++k;
+        need(k);
+        const double shift = c_over_gamma + l[k - 1];
+        const int nblk = launch_iter(op, ws->w[(k - 1) & 1], ws->w[k & 1], ws->p, inv_gamma, shift,
+                                     make_double2(d[k].real(), d[k].imag()), ws, st);
+        launch_leja_finalize(nblk, std::abs(d[k]), prm.tol, ws, st);
+      }
+      if (ws->time_leja) CU_TRY(cudaEventRecord(ws->ev[1], st));
+      CU_TRY(cudaMemcpyAsync(ws->status_host, ws->status, sizeof(LejaStatus), cudaMemcpyDeviceToHost, st));
+      CU_TRY(cudaStreamSynchronize(st));
+      if (ws->time_leja) {
+        CU_TRY(cudaEventElapsedTime(&ms, ws->ev[0], ws->ev[1]));
+        ws->leja_ms += ms;
+        CU_TRY(cudaEventRecord(ws->ev[0], st));
+      }
+      done = ws->status_host->done != 0;
+      chunk_end = std::min(prm.m_max, k + 4);
+    }
+    loc.iters = ws->status_host->iters;
+    loc.err_est = ws->status_host->err_est;
+    if (!done) {
+      loc.status = MAGNUS_ENOCONV;
+      if (info) *info = loc;
+      set_error("Leja interpolation did not reach tol=%g within m_max=%d (theta=%g)", prm.tol, prm.m_max, theta);
+      return MAGNUS_ENOCONV;
+    }
+    launch_leja_finish(ws->p, v_out, n, phase, st, ws);   // c7
+  }
+  CU_TRY(cudaGetLastError());
+  if (info) *info = loc;
+  return MAGNUS_OK;
+}
+
+static void default_params(const magnus_options* opt, LejaParams* prm, cudaStream_t* st, int* csr_kernel) {
+  prm->tol = (opt && opt->tol > 0.0) ? opt->tol : 1e-12;
+  prm->theta_max = (opt && opt->theta_max > 0.0) ? opt->theta_max : 16.0;
+  prm->m_max = (opt && opt->m_max > 0 && opt->m_max <= kMaxDegree) ? opt->m_max : kMaxDegree;
+  *st = opt ? (cudaStream_t)opt->stream : (cudaStream_t)0;
+  *csr_kernel = opt ? opt->csr_kernel : 0;
+}
+
+}  // namespace magnus
+
+using namespace magnus;
+
+struct magnus_context {
+  int scheme = 0;
+  int format = 0;
+  int64_t n = 0;
+  magnus_matrix H0, H1;
+  magnus_drive_fn f = nullptr;
+  void* user = nullptr;
+  LejaParams prm;
+  cudaStream_t stream = 0;
+  Workspace ws;
+  // dense: assembled matrix (commutator-free schemes) or A1 (M4; Omega_H overwrites it), A2, P
+  cplx* M = nullptr;
+  cplx* A2 = nullptr;
+  cplx* P = nullptr;
+  // CSR M4: cached C = [H0, H1] (row S0)
+  int32_t* c_rp = nullptr;
+  int32_t* c_ci = nullptr;
+  cplx* c_v = nullptr;
+  int64_t c_nnz = 0;
+  cudaEvent_t ev_comm[2] = {nullptr, nullptr};
+  double comm_ms = 0.0;
+  bool time_comm = false;
+};
+
+extern "C" {
+
+const char* magnus_strerror(int code) {
+  switch (code) {
+    case MAGNUS_OK: return "ok";
+    case MAGNUS_EINVAL: return "invalid argument";
+    case MAGNUS_ENOMEM: return "out of memory";
+    case MAGNUS_ECUDA: return "CUDA error";
+    case MAGNUS_ENOCONV: return "Leja interpolation did not converge within m_max";
+    case MAGNUS_ENOTHERMITIAN: return "matrix is not Hermitian";
+    default: return "unknown error";
+  }
+}
+
+const char* magnus_last_error(void) { return g_err; }
+
+const char* magnus_version(void) { return "magnus-b200 0.1 (sm_100a)"; }
+
+int magnus_host_leja_points(int m, double* out_host) {
+  if (!out_host || m < 0 || m > kMaxDegree + 1) { set_error("magnus_host_leja_points: bad m"); return MAGNUS_EINVAL; }
+  std::memcpy(out_host, leja_points(), sizeof(double) * (size_t)m);
+  return MAGNUS_OK;
+}
+
+int magnus_host_divided_differences(double theta, int m, double* out_host) {
+  if (!out_host || m < 1 || m > kMaxDegree + 1) { set_error("magnus_host_divided_differences: bad m"); return MAGNUS_EINVAL; }
+  divided_differences(theta, m, reinterpret_cast<std::complex<double>*>(out_host));
+  return MAGNUS_OK;
+}
+
+int magnus_host_snap_interval(double* a, double* b) {
+  if (!a || !b) return MAGNUS_EINVAL;
+  snap_interval(a, b);
+  return MAGNUS_OK;
+}
+
+int magnus_host_step_coefficients(int scheme, magnus_drive_fn f, void* user, double t, double tau, double* coef_h1,
+                                  double* h_scale, double* kappa_out) {
+  if (!f || !coef_h1 || !h_scale) return MAGNUS_EINVAL;
+  const int n = step_coefficients(scheme, f, user, t, tau, coef_h1, h_scale, kappa_out);
+  if (n < 0) { set_error("unknown scheme %d", scheme); return MAGNUS_EINVAL; }
+  return n;
+}
+
+int magnus_destroy(magnus_handle h) {
+  if (!h) return MAGNUS_OK;
+  workspace_free(&h->ws);
+  cudaFree(h->M);
+  cudaFree(h->A2);
+  cudaFree(h->P);
+  cudaFree(h->c_rp);
+  cudaFree(h->c_ci);
+  cudaFree(h->c_v);
+  for (int i = 0; i < 2; ++i)
+    if (h->ev_comm[i]) cudaEventDestroy(h->ev_comm[i]);
+  delete h;
+  return MAGNUS_OK;
+}
+
+int magnus_create(magnus_handle* out, const magnus_matrix* H0, const magnus_matrix* H1, magnus_drive_fn f, void* user,
+                  int scheme, const magnus_options* opt) {
+  if (!out) { set_error("out is NULL"); return MAGNUS_EINVAL; }
+  *out = nullptr;
+  int rc = check_matrix(H0, "H0");
+  if (rc) return rc;
+  rc = check_matrix(H1, "H1");
+  if (rc) return rc;
+  if (H0->format != H1->format || H0->n != H1->n) { set_error("H0 and H1 differ in format or n"); return MAGNUS_EINVAL; }
+  if (!f) { set_error("f is NULL"); return MAGNUS_EINVAL; }
+  if (scheme < MAGNUS_CF4 || scheme > MAGNUS_CF4_3) { set_error("unknown scheme %d", scheme); return MAGNUS_EINVAL; }
+  rc = require_device();
+  if (rc) return rc;
+
+  magnus_context* h = new (std::nothrow) magnus_context();
+  if (!h) return MAGNUS_ENOMEM;
+  h->scheme = scheme;
+  h->format = H0->format;
+  h->n = H0->n;
+  h->H0 = *H0;
+  h->H1 = *H1;
+  h->f = f;
+  h->user = user;
+  default_params(opt, &h->prm, &h->stream, &h->ws.csr_kernel);
+  const int csr_kernel = h->ws.csr_kernel;
+  rc = workspace_alloc(&h->ws, h->n);
+  h->ws.csr_kernel = csr_kernel;
+  h->ws.time_leja = true;
+  if (rc) { set_error("workspace allocation failed (n=%lld)", (long long)h->n); magnus_destroy(h); return rc; }
+
+  if (opt && opt->check_hermitian) {
+    double bad0 = 0.0, bad1 = 0.0;
+    if (h->format == MAGNUS_CSR) {
+      rc = csr_hermitian_check(H0, h->stream, &bad0);
+      if (!rc) rc = csr_hermitian_check(H1, h->stream, &bad1);
+    } else {
+      DenseOp d0{H0->n, dense_ld(H0), (const cplx*)H0->values}, d1{H1->n, dense_ld(H1), (const cplx*)H1->values};
+      rc = dense_hermitian_check(d0, h->stream, &bad0);
+      if (!rc) rc = dense_hermitian_check(d1, h->stream, &bad1);
+    }
+    if (rc) { magnus_destroy(h); return rc; }
+    if (bad0 > 1e-12 || bad1 > 1e-12) {
+      set_error("sampled Hermitian check failed: max |M_ij - conj(M_ji)| = %g (H0), %g (H1)", bad0, bad1);
+      magnus_destroy(h);
+      return MAGNUS_ENOTHERMITIAN;
+    }
+  }
+
+  if (h->format == MAGNUS_DENSE) {
+    const size_t bytes = sizeof(cplx) * (size_t)h->n * (size_t)h->n;
+    bool ok = cudaMalloc(&h->M, bytes) == cudaSuccess;
+    if (ok && scheme == MAGNUS_M4)
+      ok = cudaMalloc(&h->A2, bytes) == cudaSuccess && cudaMalloc(&h->P, bytes) == cudaSuccess;
+    if (!ok) {
+      cudaGetLastError();
+      set_error("dense workspace allocation failed (%zu bytes per matrix)", bytes);
+      magnus_destroy(h);
+      return MAGNUS_ENOMEM;
+    }
+    if (scheme == MAGNUS_M4) {
+      cudaEventCreate(&h->ev_comm[0]);
+      cudaEventCreate(&h->ev_comm[1]);
+      h->time_comm = true;
+    }
+  } else if (scheme == MAGNUS_M4) {
+    int64_t nnz = 0;
+    rc = csr_commutator_owned(H0, H1, &h->c_rp, &h->c_ci, &h->c_v, &nnz, h->stream);   // S0
+    if (rc) { magnus_destroy(h); return rc; }
+    h->c_nnz = nnz;
+  }
+  if (cudaStreamSynchronize(h->stream) != cudaSuccess) { magnus_destroy(h); return MAGNUS_ECUDA; }
+  *out = h;
+  return MAGNUS_OK;
+}
+
+int magnus_step(magnus_handle h, double t, double tau, void* psi_, magnus_step_info* info) {
+  if (!h || !psi_) { set_error("magnus_step: NULL handle or psi"); return MAGNUS_EINVAL; }
+  cplx* psi = (cplx*)psi_;
+  double coef[MAGNUS_MAX_EXP_PER_STEP], hscale[MAGNUS_MAX_EXP_PER_STEP], kappa = 0.0;
+  const int n_exp = step_coefficients(h->scheme, h->f, h->user, t, tau, coef, hscale, &kappa);   // S1
+  if (info) {
+    std::memset(info, 0, sizeof *info);
+    info->n_exp = n_exp;
+  }
+  cudaStream_t st = h->stream;
+  Workspace* ws = &h->ws;
+  int rc = MAGNUS_OK;
+  for (int e = 0; e < n_exp && rc == MAGNUS_OK; ++e) {
+    OpRef op;
+    double a = 0.0, b = 0.0;
+    if (h->format == MAGNUS_CSR) {
+      op.dense = false;
+      op.csr.n = h->n;
+      if (h->scheme == MAGNUS_M4) {
+        // Omega_H = H0 + fbar H1 - i kappa [H0, H1]   (c1; [H(t2),H(t1)] = (f1 - f2)[H0,H1])
+        op.csr.nterms = (h->c_nnz > 0 && kappa != 0.0) ? 3 : 2;
+        op.csr.t[0] = csr_term(&h->H0, 1.0, 0.0);
+        op.csr.t[1] = csr_term(&h->H1, 0.5 * (coef[0] + coef[1]), 0.0);
+        CsrTerm c;
+        c.rp = h->c_rp;
+        c.ci = h->c_ci;
+        c.v = h->c_v;
+        c.coef = make_double2(0.0, -kappa);
+        c.nnz = h->c_nnz;
+        op.csr.t[2] = c;
+      } else {
+        op.csr.nterms = 2;
+        op.csr.t[0] = csr_term(&h->H0, 1.0, 0.0);
+        op.csr.t[1] = csr_term(&h->H1, coef[e], 0.0);
+        op.csr.t[2] = op.csr.t[1];
+      }
+      rc = op_interval(op, ws, st, &a, &b);                                                        // S3
+    } else {
+      op.dense = true;
+      const cplx* H0v = (const cplx*)h->H0.values;
+      const cplx* H1v = (const cplx*)h->H1.values;
+      int nblk = 0;
+      if (h->scheme == MAGNUS_M4) {
+        launch_dense_assemble2(h->n, H0v, dense_ld(&h->H0), H1v, dense_ld(&h->H1), coef[0], coef[1], h->M, h->A2, ws,
+                               st);                                                                // S2: A1, A2
+        if (h->time_comm) cudaEventRecord(h->ev_comm[0], st);
+        rc = launch_zgemm(h->n, h->A2, h->n, h->M, h->n, h->P, h->n, st);                          // D3: P = A2 A1
+        ws->launches += 1;
+        if (h->time_comm) cudaEventRecord(h->ev_comm[1], st);
+        if (rc) { set_error("zgemm launch failed: %s", cudaGetErrorString(cudaGetLastError())); break; }
+        nblk = launch_dense_omega(h->n, h->M, h->A2, h->P, std::sqrt(3.0) * tau / 12.0, ws, st);    // D4 (+S3)
+      } else {
+        nblk = launch_dense_assemble(h->n, H0v, dense_ld(&h->H0), H1v, dense_ld(&h->H1), coef[e], h->M, ws, st);
+      }
+      op.dns.n = h->n;
+      op.dns.ld = h->n;
+      op.dns.M = h->M;
+      rc = read_interval(nblk, ws, st, &a, &b);
+      if (rc == MAGNUS_OK && h->time_comm) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, h->ev_comm[0], h->ev_comm[1]) == cudaSuccess) h->comm_ms += ms;
+      }
+    }
+    if (rc) break;
+    rc = expmv_on_interval(op, a, b, psi, psi, hscale[e] * tau, h->prm, ws, st, info ? &info->exp[e] : nullptr);
+  }
+  return rc;
+}
+
+int magnus_integrate(magnus_handle h, double t0, double t_end, int64_t nsteps, void* psi, magnus_stats* stats) {
+  if (!h || !psi || nsteps <= 0) { set_error("magnus_integrate: bad arguments"); return MAGNUS_EINVAL; }
+  const double tau = (t_end - t0) / (double)nsteps;
+  cudaStream_t st = h->stream;
+  Workspace* ws = &h->ws;
+  const int64_t launches0 = ws->launches;
+  ws->leja_ms = 0.0;
+  h->comm_ms = 0.0;
+  CU_TRY(cudaEventRecord(ws->ev[2], st));
+  int64_t total = 0, nexp = 0;
+  int rc = MAGNUS_OK;
+  for (int64_t s = 0; s < nsteps; ++s) {
+    magnus_step_info si;
+    rc = magnus_step(h, t0 + (double)s * tau, tau, psi, &si);
+    for (int e = 0; e < si.n_exp; ++e) {
+      if (rc != MAGNUS_OK && si.exp[e].iters == 0 && si.exp[e].substeps == 0) break;
+      if (stats && stats->iters && nexp < stats->iters_cap) stats->iters[nexp] = si.exp[e].iters;
+      total += si.exp[e].iters;
+      ++nexp;
+    }
+    if (rc != MAGNUS_OK) break;
+  }
+  CU_TRY(cudaEventRecord(ws->ev[3], st));
+  CU_TRY(cudaStreamSynchronize(st));
+  if (stats) {
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, ws->ev[2], ws->ev[3]);
+    stats->total_matvecs = total;
+    stats->n_exp = nexp;
+    stats->seconds_device = ms * 1e-3;
+    stats->seconds_leja = ws->leja_ms * 1e-3;
+    stats->seconds_commutator = h->comm_ms * 1e-3;
+    stats->kernel_launches = ws->launches - launches0;
+  }
+  return rc;
+}
+
+int leja_expmv(const magnus_matrix* H, const void* v_in, void* v_out, double h, double tol, void* stream,
+               magnus_expmv_info* info) {
+  int rc = check_matrix(H, "H");
+  if (rc) return rc;
+  if (!v_in || !v_out) { set_error("leja_expmv: NULL vector"); return MAGNUS_EINVAL; }
+  rc = require_device();
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  LejaParams prm;
+  prm.tol = tol > 0.0 ? tol : 1e-12;
+  prm.theta_max = 16.0;
+  prm.m_max = kMaxDegree;
+  Workspace ws;
+  rc = workspace_alloc(&ws, H->n);
+  if (rc) { cudaGetLastError(); workspace_free(&ws); set_error("leja_expmv: workspace allocation failed"); return rc; }
+  OpRef op;
+  if (H->format == MAGNUS_CSR) {
+    op.dense = false;
+    op.csr.n = H->n;
+    op.csr.nterms = 1;
+    op.csr.t[0] = csr_term(H, 1.0, 0.0);
+    op.csr.t[1] = op.csr.t[2] = op.csr.t[0];
+  } else {
+    op.dense = true;
+    op.dns.n = H->n;
+    op.dns.ld = dense_ld(H);
+    op.dns.M = (const cplx*)H->values;
+  }
+  double a = 0.0, b = 0.0;
+  rc = op_interval(op, &ws, st, &a, &b);
+  if (rc == MAGNUS_OK) rc = expmv_on_interval(op, a, b, (const cplx*)v_in, (cplx*)v_out, h, prm, &ws, st, info);
+  if (cudaStreamSynchronize(st) != cudaSuccess && rc == MAGNUS_OK) rc = MAGNUS_ECUDA;
+  workspace_free(&ws);
+  return rc;
+}
+
+// ---- host-buffer end-to-end call -------------------------------------------------
+static int upload_matrix(const magnus_matrix* Hh, magnus_matrix* Hd, cudaStream_t st) {
+  *Hd = *Hh;
+  Hd->values = nullptr;
+  Hd->col_idx = nullptr;
+  Hd->row_ptr = nullptr;
+  void* p = nullptr;
+  if (Hh->format == MAGNUS_CSR) {
+    const size_t nnz = (size_t)(Hh->nnz > 0 ? Hh->nnz : 1);
+    if (cudaMalloc(&p, sizeof(cplx) * nnz) != cudaSuccess) return MAGNUS_ENOMEM;
+    Hd->values = p;
+    if (cudaMalloc(&p, sizeof(int32_t) * nnz) != cudaSuccess) return MAGNUS_ENOMEM;
+    Hd->col_idx = (const int32_t*)p;
+    if (cudaMalloc(&p, sizeof(int32_t) * (size_t)(Hh->n + 1)) != cudaSuccess) return MAGNUS_ENOMEM;
+    Hd->row_ptr = (const int32_t*)p;
+    CU_TRY(cudaMemcpyAsync((void*)Hd->values, Hh->values, sizeof(cplx) * (size_t)Hh->nnz, cudaMemcpyHostToDevice, st));
+    CU_TRY(cudaMemcpyAsync((void*)Hd->col_idx, Hh->col_idx, sizeof(int32_t) * (size_t)Hh->nnz, cudaMemcpyHostToDevice, st));
+    CU_TRY(cudaMemcpyAsync((void*)Hd->row_ptr, Hh->row_ptr, sizeof(int32_t) * (size_t)(Hh->n + 1), cudaMemcpyHostToDevice, st));
+  } else {
+    const int64_t ld = dense_ld(Hh);
+    if (cudaMalloc(&p, sizeof(cplx) * (size_t)Hh->n * (size_t)Hh->n) != cudaSuccess) return MAGNUS_ENOMEM;
+    Hd->values = p;
+    Hd->ld = Hh->n;
+    CU_TRY(cudaMemcpy2DAsync(p, sizeof(cplx) * (size_t)Hh->n, Hh->values, sizeof(cplx) * (size_t)ld,
+                             sizeof(cplx) * (size_t)Hh->n, (size_t)Hh->n, cudaMemcpyHostToDevice, st));
+  }
+  return MAGNUS_OK;
+}
+
+static void free_uploaded(magnus_matrix* Hd) {
+  cudaFree((void*)Hd->values);
+  cudaFree((void*)Hd->col_idx);
+  cudaFree((void*)Hd->row_ptr);
+}
+
+int magnus_integrate_host(const magnus_matrix* H0_host, const magnus_matrix* H1_host, magnus_drive_fn f, void* user,
+                          int scheme, const magnus_options* opt, double t0, double t_end, int64_t nsteps,
+                          void* psi_host, magnus_stats* stats) {
+  int rc = check_matrix(H0_host, "H0");
+  if (rc) return rc;
+  rc = check_matrix(H1_host, "H1");
+  if (rc) return rc;
+  if (!psi_host) { set_error("psi_host is NULL"); return MAGNUS_EINVAL; }
+  rc = require_device();
+  if (rc) return rc;
+  cudaStream_t st = opt ? (cudaStream_t)opt->stream : (cudaStream_t)0;
+  magnus_matrix d0, d1;
+  std::memset(&d0, 0, sizeof d0);
+  std::memset(&d1, 0, sizeof d1);
+  cplx* psi = nullptr;
+  magnus_handle h = nullptr;
+  const size_t vb = sizeof(cplx) * (size_t)H0_host->n;
+  rc = upload_matrix(H0_host, &d0, st);
+  if (rc == MAGNUS_OK) rc = upload_matrix(H1_host, &d1, st);
+  if (rc == MAGNUS_OK && cudaMalloc(&psi, vb) != cudaSuccess) rc = MAGNUS_ENOMEM;
+  if (rc == MAGNUS_OK && cudaMemcpyAsync(psi, psi_host, vb, cudaMemcpyHostToDevice, st) != cudaSuccess) rc = MAGNUS_ECUDA;
+  if (rc == MAGNUS_OK) rc = magnus_create(&h, &d0, &d1, f, user, scheme, opt);
+  if (rc == MAGNUS_OK) rc = magnus_integrate(h, t0, t_end, nsteps, psi, stats);
+  if (rc == MAGNUS_OK && cudaMemcpyAsync(psi_host, psi, vb, cudaMemcpyDeviceToHost, st) != cudaSuccess) rc = MAGNUS_ECUDA;
+  if (cudaStreamSynchronize(st) != cudaSuccess && rc == MAGNUS_OK) rc = MAGNUS_ECUDA;
+  if (rc == MAGNUS_ENOMEM) { cudaGetLastError(); set_error("magnus_integrate_host: device allocation failed"); }
+  magnus_destroy(h);
+  cudaFree(psi);
+  free_uploaded(&d0);
+  free_uploaded(&d1);
+  return rc;
+}
+
+// ---- single kernels -----------------------------------------------------------------
+static int build_op(const magnus_matrix* H0, const magnus_matrix* H1, double g, OpRef* op, cplx** tmpM, Workspace* ws,
+                    cudaStream_t st, int* assemble_blocks) {
+  *tmpM = nullptr;
+  *assemble_blocks = -1;
+  if (H0->format == MAGNUS_CSR) {
+    op->dense = false;
+    op->csr.n = H0->n;
+    op->csr.nterms = H1 ? 2 : 1;
+    op->csr.t[0] = csr_term(H0, 1.0, 0.0);
+    op->csr.t[1] = H1 ? csr_term(H1, g, 0.0) : op->csr.t[0];
+    op->csr.t[2] = op->csr.t[0];
+  } else {
+    op->dense = true;
+    op->dns.n = H0->n;
+    if (H1) {
+      if (cudaMalloc(tmpM, sizeof(cplx) * (size_t)H0->n * (size_t)H0->n) != cudaSuccess) {
+        cudaGetLastError();
+        set_error("assembled matrix allocation failed");
+        return MAGNUS_ENOMEM;
+      }
+      *assemble_blocks = launch_dense_assemble(H0->n, (const cplx*)H0->values, dense_ld(H0), (const cplx*)H1->values,
+                                               dense_ld(H1), g, *tmpM, ws, st);
+      op->dns.ld = H0->n;
+      op->dns.M = *tmpM;
+    } else {
+      op->dns.ld = dense_ld(H0);
+      op->dns.M = (const cplx*)H0->values;
+    }
+  }
+  return MAGNUS_OK;
+}
+
+int magnus_gershgorin(const magnus_matrix* H0, const magnus_matrix* H1, double g, void* stream, double* ab_host) {
+  int rc = check_matrix(H0, "H0");
+  if (rc) return rc;
+  if (H1 && (rc = check_matrix(H1, "H1"))) return rc;
+  if (H1 && (H1->format != H0->format || H1->n != H0->n)) { set_error("H0 and H1 differ"); return MAGNUS_EINVAL; }
+  if (!ab_host) return MAGNUS_EINVAL;
+  rc = require_device();
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  Workspace ws;
+  rc = workspace_alloc(&ws, 1);
+  if (rc) { workspace_free(&ws); return rc; }
+  OpRef op;
+  cplx* tmp = nullptr;
+  int ab = -1;
+  rc = build_op(H0, H1, g, &op, &tmp, &ws, st, &ab);
+  if (rc == MAGNUS_OK)
+    rc = ab >= 0 ? read_interval(ab, &ws, st, &ab_host[0], &ab_host[1]) : op_interval(op, &ws, st, &ab_host[0], &ab_host[1]);
+  cudaFree(tmp);
+  workspace_free(&ws);
+  return rc;
+}
+
+int magnus_leja_iteration(const magnus_matrix* H0, const magnus_matrix* H1, double g, const void* w_in, void* w_out,
+                          void* p, double inv_gamma, double shift, double d_re, double d_im, void* stream,
+                          int csr_kernel, int reps, double* sums_host, float* ms_per_launch) {
+  int rc = check_matrix(H0, "H0");
+  if (rc) return rc;
+  if (H1 && (rc = check_matrix(H1, "H1"))) return rc;
+  if (H1 && (H1->format != H0->format || H1->n != H0->n)) { set_error("H0 and H1 differ"); return MAGNUS_EINVAL; }
+  if (!w_in || !w_out || !p || w_in == w_out) { set_error("magnus_leja_iteration: bad vectors"); return MAGNUS_EINVAL; }
+  if (reps < 1) reps = 1;
+  rc = require_device();
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  Workspace ws;
+  rc = workspace_alloc(&ws, 1);
+  if (rc) { workspace_free(&ws); return rc; }
+  ws.csr_kernel = csr_kernel;
+  OpRef op;
+  cplx* tmp = nullptr;
+  int ab = -1;
+  rc = build_op(H0, H1, g, &op, &tmp, &ws, st, &ab);
+  if (rc == MAGNUS_OK) {
+    cudaMemsetAsync(ws.status, 0, sizeof(LejaStatus), st);
+    int nblk = 0;
+    cudaEventRecord(ws.ev[0], st);
+    for (int r = 0; r < reps; ++r)
+      nblk = launch_iter(op, (const cplx*)w_in, (cplx*)w_out, (cplx*)p, inv_gamma, shift, make_double2(d_re, d_im), &ws, st);
+    cudaEventRecord(ws.ev[1], st);
+    launch_leja_finalize(nblk, 1.0, 0.0, &ws, st);
+    cudaMemcpyAsync(ws.status_host, ws.status, sizeof(LejaStatus), cudaMemcpyDeviceToHost, st);
+    if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) {
+      set_error("magnus_leja_iteration: kernel failed");
+      rc = MAGNUS_ECUDA;
+    } else {
+      float ms = 0.f;
+      cudaEventElapsedTime(&ms, ws.ev[0], ws.ev[1]);
+      if (ms_per_launch) *ms_per_launch = ms / (float)reps;
+      if (sums_host) {
+        sums_host[0] = ws.status_host->norm_w2;
+        sums_host[1] = ws.status_host->norm_p2;
+      }
+    }
+  }
+  cudaFree(tmp);
+  workspace_free(&ws);
+  return rc;
+}
+
+int magnus_zgemm(int64_t n, const void* A, int64_t lda, const void* B, int64_t ldb, void* C, int64_t ldc, void* stream,
+                 float* ms) {
+  if (n <= 0 || !A || !B || !C || C == A || C == B) { set_error("magnus_zgemm: bad arguments"); return MAGNUS_EINVAL; }
+  if (lda == 0) lda = n;
+  if (ldb == 0) ldb = n;
+  if (ldc == 0) ldc = n;
+  int rc = require_device();
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaEvent_t e0, e1;
+  CU_TRY(cudaEventCreate(&e0));
+  CU_TRY(cudaEventCreate(&e1));
+  cudaEventRecord(e0, st);
+  rc = launch_zgemm(n, (const cplx*)A, lda, (const cplx*)B, ldb, (cplx*)C, ldc, st);
+  cudaEventRecord(e1, st);
+  if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) {
+    set_error("magnus_zgemm: kernel failed");
+    rc = MAGNUS_ECUDA;
+  } else if (ms) {
+    cudaEventElapsedTime(ms, e0, e1);
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  return rc;
+}
+
+int magnus_commutator_dense(int64_t n, const void* A, const void* B, void* K, void* work, void* stream) {
+  if (n <= 0 || !A || !B || !K || !work || work == A || work == B || work == K) {
+    set_error("magnus_commutator_dense: bad arguments");
+    return MAGNUS_EINVAL;
+  }
+  int rc = require_device();
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  rc = launch_zgemm(n, (const cplx*)A, n, (const cplx*)B, n, (cplx*)work, n, st);   // P = A B
+  if (rc) return rc;
+  launch_dense_antiherm(n, (const cplx*)work, (cplx*)K, st);                        // K = P - P^H
+  CU_TRY(cudaStreamSynchronize(st));
+  CU_TRY(cudaGetLastError());
+  return MAGNUS_OK;
+}
+
+int magnus_commutator_csr(const magnus_matrix* A, const magnus_matrix* B, int64_t cap_nnz, int64_t* nnz_out,
+                          int32_t* row_ptr_out, int32_t* col_idx_out, void* values_out, void* stream) {
+  int rc = check_matrix(A, "A");
+  if (rc) return rc;
+  rc = check_matrix(B, "B");
+  if (rc) return rc;
+  if (A->format != MAGNUS_CSR || B->format != MAGNUS_CSR || A->n != B->n || !nnz_out) {
+    set_error("magnus_commutator_csr: needs two CSR matrices of equal n");
+    return MAGNUS_EINVAL;
+  }
+  if (cap_nnz > 0 && (!row_ptr_out || !col_idx_out || !values_out)) return MAGNUS_EINVAL;
+  rc = require_device();
+  if (rc) return rc;
+  return csr_commutator(A, B, cap_nnz, nnz_out, row_ptr_out, col_idx_out, (cplx*)values_out, (cudaStream_t)stream);
+}
+
+int magnus_fp64_peaks(double* dmma_tflops, double* dfma_tflops, void* stream) {
+  if (!dmma_tflops || !dfma_tflops) return MAGNUS_EINVAL;
+  int rc = require_device();
+  if (rc) return rc;
+  return fp64_peaks(dmma_tflops, dfma_tflops, (cudaStream_t)stream);
+}
+
+}  // extern "C"

@@ -1,0 +1,442 @@
+// CSR kernels: Gershgorin bounds of M = sum_t coef_t A_t (row S3), the fused
+// Leja iteration (row S6) and the setup-time sparse commutator (row S0).
+// P:n = PAPER.md line n; c1..c7 = readings in DESIGN.md section 3.
+#include "magnus_internal.h"
+#include "device_utils.cuh"
+
+#include <cub/device/device_scan.cuh>
+#include <limits.h>
+
+namespace magnus {
+
+// ---------------------------------------------------------------------------
+// S3 -- Gershgorin bounds ("an estimate on the spectrum of the matrix"; c4):
+// lo_i = Re M_ii - R_i, hi_i = Re M_ii + R_i, R_i = sum_{j != i} |M_ij| with
+// M_ij the SUMMED entry over the terms.  One thread walks one row with a k-way
+// merge over the (ascending) column lists, so overlapping patterns are summed
+// before the modulus is taken.  Block min/max go to ws->gersh.
+// ---------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) csr_gershgorin_kernel(CsrOp op, double* __restrict__ out) {
+  double lo = INFINITY, hi = -INFINITY;
+  for (int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; row < op.n;
+       row += (int64_t)gridDim.x * blockDim.x) {
+    int q[3], e[3];
+#pragma unroll
+    for (int t = 0; t < 3; ++t) {
+      q[t] = t < op.nterms ? op.t[t].rp[row] : 0;
+      e[t] = t < op.nterms ? op.t[t].rp[row + 1] : 0;
+    }
+    double R = 0.0, d = 0.0;
+    while (true) {
+      int c = INT_MAX;
+#pragma unroll
+      for (int t = 0; t < 3; ++t)
+        if (t < op.nterms && q[t] < e[t]) c = min(c, op.t[t].ci[q[t]]);
+      if (c == INT_MAX) break;
+      cplx z = make_double2(0.0, 0.0);
+#pragma unroll
+      for (int t = 0; t < 3; ++t)
+        if (t < op.nterms && q[t] < e[t] && op.t[t].ci[q[t]] == c) {
+          const cplx prod = cmul(op.t[t].coef, op.t[t].v[q[t]]);
+          z.x += prod.x;
+          z.y += prod.y;
+          ++q[t];
+        }
+      if ((int64_t)c == row) d = z.x; else R += hypot(z.x, z.y);
+    }
+    lo = fmin(lo, d - R);
+    hi = fmax(hi, d + R);
+  }
+  block_reduce_minmax<256>(lo, hi);
+  if (threadIdx.x == 0) {
+    out[2 * blockIdx.x] = lo;
+    out[2 * blockIdx.x + 1] = hi;
+  }
+}
+
+int launch_csr_gershgorin(const CsrOp& op, Workspace* ws, cudaStream_t st) {
+  int64_t g = (op.n + 255) / 256;
+  if (g > 148 * 8) g = 148 * 8;
+  csr_gershgorin_kernel<<<(int)g, 256, 0, st>>>(op, ws->gersh);
+  ws->launches += 1;
+  return (int)g;
+}
+
+// ---------------------------------------------------------------------------
+// S6 -- fused Leja iteration, generic kernel (any CSR): G lanes share one row.
+//   y_i   = sum_t coef_t sum_q A_t.v[q] w[A_t.ci[q]]            (SpMV of H(t) formed on the fly)
+//   w+_i  = inv_gamma y_i - shift w_i                            (fragment line 4; c5)
+//   p_i  += d_k w+_i                                             (fragment line 5)
+//   block partials of sum |w+|^2 and sum |p|^2                  (for S7)
+// Lanes of a row read consecutive 16-byte values (coalesced 128-bit loads with
+// L1 no-allocate / L2 evict-first), reduce with a shuffle tree, lane 0 does the
+// vector update.  Deterministic: fixed lane->entry map and fixed trees.
+// ---------------------------------------------------------------------------
+template <int G>
+__global__ void __launch_bounds__(256) csr_leja_iter_generic(CsrOp op, const cplx* __restrict__ w_in,
+                                                              cplx* __restrict__ w_out, cplx* __restrict__ p,
+                                                              double inv_gamma, double shift, cplx dk,
+                                                              const LejaStatus* __restrict__ status,
+                                                              double* __restrict__ partials) {
+  if (status->done) return;
+  constexpr int ROWS = 256 / G;
+  const int sub = threadIdx.x % G;
+  const int rib = threadIdx.x / G;
+  const uint64_t pol = policy_evict_first();
+  double sw = 0.0, sp = 0.0;
+  for (int64_t base = (int64_t)blockIdx.x * ROWS; base < op.n; base += (int64_t)gridDim.x * ROWS) {
+    const int64_t row = base + rib;
+    const bool valid = row < op.n;
+    cplx y = make_double2(0.0, 0.0);
+#pragma unroll
+    for (int t = 0; t < 3; ++t) {
+      if (t < op.nterms) {
+        const CsrTerm& T = op.t[t];
+        int qs = 0, qe = 0;
+        if (valid) {
+          qs = T.rp[row];
+          qe = T.rp[row + 1];
+        }
+        cplx a = make_double2(0.0, 0.0);
+        for (int q = qs + sub; q < qe; q += G) {
+          const cplx v = ld_stream(T.v + q, pol);
+          const int c = ld_stream_i32(T.ci + q, pol);
+          const cplx x = w_in[c];
+          cfma(a, v, x);
+        }
+        const cplx ca = cmul(T.coef, a);
+        y.x += ca.x;
+        y.y += ca.y;
+      }
+    }
+#pragma unroll
+    for (int o = G / 2; o > 0; o >>= 1) {
+      y.x += shfl_xor_d(y.x, o);
+      y.y += shfl_xor_d(y.y, o);
+    }
+    if (valid && sub == 0) {
+      const cplx wi = w_in[row];
+      cplx wn;
+      wn.x = inv_gamma * y.x - shift * wi.x;
+      wn.y = inv_gamma * y.y - shift * wi.y;
+      w_out[row] = wn;
+      cplx pi = p[row];
+      cfma(pi, dk, wn);
+      p[row] = pi;
+      sw += wn.x * wn.x + wn.y * wn.y;
+      sp += pi.x * pi.x + pi.y * pi.y;
+    }
+  }
+  block_reduce_sum2<256>(sw, sp);
+  if (threadIdx.x == 0) {
+    partials[2 * blockIdx.x] = sw;
+    partials[2 * blockIdx.x + 1] = sp;
+  }
+}
+
+template <int G>
+static int launch_generic(const CsrOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma, double shift,
+                          cplx dk, Workspace* ws, cudaStream_t st) {
+  constexpr int ROWS = 256 / G;
+  int64_t g = (op.n + ROWS - 1) / ROWS;
+  if (g > 148 * 8) g = 148 * 8;
+  csr_leja_iter_generic<G><<<(int)g, 256, 0, st>>>(op, w_in, w_out, p, inv_gamma, shift, dk, ws->status,
+                                                    ws->partials);
+  ws->launches += 1;
+  return (int)g;
+}
+
+int launch_csr_leja_iter_rowblock(const CsrOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma,
+                                  double shift, cplx dk, Workspace* ws, cudaStream_t st);
+bool csr_rowblock_supported(const CsrOp& op);
+
+int launch_csr_leja_iter(const CsrOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma, double shift,
+                         cplx dk, Workspace* ws, cudaStream_t st) {
+  if (ws->csr_kernel == 2 || (ws->csr_kernel == 0 && csr_rowblock_supported(op)))
+    return launch_csr_leja_iter_rowblock(op, w_in, w_out, p, inv_gamma, shift, dk, ws, st);
+  // lanes per row from the mean stored entries per row and term
+  double mean = 0.0;
+  for (int t = 0; t < op.nterms; ++t) mean += (double)op.t[t].nnz;
+  mean /= (double)op.n * (double)op.nterms;
+  if (mean > 48.0) return launch_generic<32>(op, w_in, w_out, p, inv_gamma, shift, dk, ws, st);
+  if (mean > 24.0) return launch_generic<16>(op, w_in, w_out, p, inv_gamma, shift, dk, ws, st);
+  if (mean > 6.0) return launch_generic<8>(op, w_in, w_out, p, inv_gamma, shift, dk, ws, st);
+  if (mean > 3.0) return launch_generic<4>(op, w_in, w_out, p, inv_gamma, shift, dk, ws, st);
+  return launch_generic<2>(op, w_in, w_out, p, inv_gamma, shift, dk, ws, st);
+}
+
+// ---------------------------------------------------------------------------
+// S0 -- sparse commutator C = A B - B A at setup time ("the commutators
+// ... are computed directly on the device"; P:262 l.6-8).  One block per row:
+// expand all products a_ik b_kj and -b_ik a_kj into shared memory, bitonic-sort
+// by column, sum equal columns in sorted order, drop exact zeros.  Pass 1
+// counts, an exclusive scan gives row_ptr, pass 2 writes.
+// ---------------------------------------------------------------------------
+const int kCommCap = 2048;     // candidate products per row held in shared memory
+const int kCommThreads = 128;
+
+struct CsrRaw {
+  const int32_t* rp;
+  const int32_t* ci;
+  const cplx* v;
+};
+
+__device__ __forceinline__ void comm_expand(const CsrRaw& A, const CsrRaw& B, int64_t row, double sign, int* keys,
+                                            cplx* vals, int& base, int* overflow) {
+  // += sign * sum_k A(row,k) B(k,:)
+  const int ps = A.rp[row], pe = A.rp[row + 1];
+  for (int pp = ps; pp < pe; ++pp) {
+    const int k = A.ci[pp];
+    const cplx a = A.v[pp];
+    const int qs = B.rp[k], len = B.rp[k + 1] - qs;
+    if (base + len > kCommCap) {
+      if (threadIdx.x == 0) *overflow = 1;
+      base = kCommCap + 1;
+      return;
+    }
+    for (int t = threadIdx.x; t < len; t += kCommThreads) {
+      const cplx b = B.v[qs + t];
+      cplx prod = cmul(a, b);
+      prod.x *= sign;
+      prod.y *= sign;
+      keys[base + t] = B.ci[qs + t];
+      vals[base + t] = prod;
+    }
+    base += len;
+  }
+}
+
+template <bool WRITE>
+__global__ void __launch_bounds__(kCommThreads) csr_commutator_kernel(CsrRaw A, CsrRaw B, int64_t n,
+                                                                       int32_t* __restrict__ counts,
+                                                                       const int32_t* __restrict__ rp_out,
+                                                                       int32_t* __restrict__ ci_out,
+                                                                       cplx* __restrict__ v_out, int* overflow) {
+  __shared__ int keys[kCommCap];
+  __shared__ cplx vals[kCommCap];
+  __shared__ int scan[kCommThreads + 1];
+  for (int64_t row = blockIdx.x; row < n; row += gridDim.x) {
+    int total = 0;
+    comm_expand(A, B, row, 1.0, keys, vals, total, overflow);
+    if (total <= kCommCap) comm_expand(B, A, row, -1.0, keys, vals, total, overflow);
+    if (total > kCommCap) {   // row too dense for the shared-memory path: flagged, host reports EINVAL
+      if (!WRITE && threadIdx.x == 0) counts[row] = 0;
+      __syncthreads();
+      continue;
+    }
+    int cap = 1;
+    while (cap < total) cap <<= 1;
+    for (int t = total + threadIdx.x; t < cap; t += kCommThreads) keys[t] = INT_MAX;
+    __syncthreads();
+    // bitonic sort on (key); equal keys end in a network-determined (fixed) order
+    for (int k = 2; k <= cap; k <<= 1) {
+      for (int j = k >> 1; j > 0; j >>= 1) {
+        for (int t = threadIdx.x; t < cap; t += kCommThreads) {
+          const int u = t ^ j;
+          if (u > t) {
+            const bool up = (t & k) == 0;
+            const int kt = keys[t], ku = keys[u];
+            if ((kt > ku) == up) {
+              keys[t] = ku;
+              keys[u] = kt;
+              const cplx tv = vals[t];
+              vals[t] = vals[u];
+              vals[u] = tv;
+            }
+          }
+        }
+        __syncthreads();
+      }
+    }
+    // each thread owns a contiguous slice; a "head" starts a run of equal columns
+    const int per = (total + kCommThreads - 1) / kCommThreads;
+    const int s0 = min(total, threadIdx.x * per), s1 = min(total, s0 + per);
+    int cnt = 0;
+    for (int t = s0; t < s1; ++t) {
+      if (t == 0 || keys[t] != keys[t - 1]) {
+        cplx z = vals[t];
+        for (int u = t + 1; u < total && keys[u] == keys[t]; ++u) {
+          z.x += vals[u].x;
+          z.y += vals[u].y;
+        }
+        if (z.x != 0.0 || z.y != 0.0) ++cnt;
+      }
+    }
+    scan[threadIdx.x + 1] = cnt;
+    if (threadIdx.x == 0) scan[0] = 0;
+    __syncthreads();
+    if (threadIdx.x == 0)
+      for (int t = 1; t <= kCommThreads; ++t) scan[t] += scan[t - 1];
+    __syncthreads();
+    if (!WRITE) {
+      if (threadIdx.x == 0) counts[row] = scan[kCommThreads];
+    } else {
+      int o = rp_out[row] + scan[threadIdx.x];
+      for (int t = s0; t < s1; ++t) {
+        if (t == 0 || keys[t] != keys[t - 1]) {
+          cplx z = vals[t];
+          for (int u = t + 1; u < total && keys[u] == keys[t]; ++u) {
+            z.x += vals[u].x;
+            z.y += vals[u].y;
+          }
+          if (z.x != 0.0 || z.y != 0.0) {
+            ci_out[o] = keys[t];
+            v_out[o] = z;
+            ++o;
+          }
+        }
+      }
+    }
+    __syncthreads();
+  }
+}
+
+// Builds C = AB - BA into freshly cudaMalloc'ed arrays (caller frees).
+int csr_commutator_build(const CsrRaw& A, const CsrRaw& B, int64_t n, int32_t** rp_out, int32_t** ci_out,
+                         cplx** v_out, int64_t* nnz_out, cudaStream_t st) {
+  int32_t* counts = nullptr;
+  int32_t* rp = nullptr;
+  int* overflow = nullptr;
+  void* tmp = nullptr;
+  size_t tmp_bytes = 0;
+  int rc = MAGNUS_OK;
+  *rp_out = nullptr;
+  *ci_out = nullptr;
+  *v_out = nullptr;
+  if (cudaMalloc(&counts, sizeof(int32_t) * (size_t)(n + 1)) != cudaSuccess ||
+      cudaMalloc(&rp, sizeof(int32_t) * (size_t)(n + 1)) != cudaSuccess ||
+      cudaMalloc(&overflow, sizeof(int)) != cudaSuccess) {
+    rc = MAGNUS_ENOMEM;
+  }
+  int grid = (int)(n < 148 * 16 ? n : 148 * 16);
+  int h_over = 0;
+  int32_t h_nnz = 0;
+  if (rc == MAGNUS_OK) {
+    cudaMemsetAsync(overflow, 0, sizeof(int), st);
+    cudaMemsetAsync(counts, 0, sizeof(int32_t) * (size_t)(n + 1), st);
+    csr_commutator_kernel<false><<<grid, kCommThreads, 0, st>>>(A, B, n, counts, nullptr, nullptr, nullptr, overflow);
+    cub::DeviceScan::ExclusiveSum(nullptr, tmp_bytes, counts, rp, (int)(n + 1), st);
+    if (cudaMalloc(&tmp, tmp_bytes) != cudaSuccess) rc = MAGNUS_ENOMEM;
+  }
+  if (rc == MAGNUS_OK) {
+    cub::DeviceScan::ExclusiveSum(tmp, tmp_bytes, counts, rp, (int)(n + 1), st);
+    cudaMemcpyAsync(&h_over, overflow, sizeof(int), cudaMemcpyDeviceToHost, st);
+    cudaMemcpyAsync(&h_nnz, rp + n, sizeof(int32_t), cudaMemcpyDeviceToHost, st);
+    if (cudaStreamSynchronize(st) != cudaSuccess) rc = MAGNUS_ECUDA;
+  }
+  if (rc == MAGNUS_OK && h_over) {
+    set_error("sparse commutator: a row needs more than %d candidate products", kCommCap);
+    rc = MAGNUS_EINVAL;
+  }
+  int32_t* ci = nullptr;
+  cplx* v = nullptr;
+  if (rc == MAGNUS_OK) {
+    const size_t cap = h_nnz > 0 ? (size_t)h_nnz : 1;
+    if (cudaMalloc(&ci, sizeof(int32_t) * cap) != cudaSuccess || cudaMalloc(&v, sizeof(cplx) * cap) != cudaSuccess)
+      rc = MAGNUS_ENOMEM;
+  }
+  if (rc == MAGNUS_OK) {
+    csr_commutator_kernel<true><<<grid, kCommThreads, 0, st>>>(A, B, n, nullptr, rp, ci, v, overflow);
+    if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) rc = MAGNUS_ECUDA;
+  }
+  cudaFree(counts);
+  cudaFree(overflow);
+  cudaFree(tmp);
+  if (rc != MAGNUS_OK) {
+    cudaFree(rp);
+    cudaFree(ci);
+    cudaFree(v);
+    return rc;
+  }
+  *rp_out = rp;
+  *ci_out = ci;
+  *v_out = v;
+  *nnz_out = h_nnz;
+  return MAGNUS_OK;
+}
+
+int csr_commutator_owned(const magnus_matrix* A, const magnus_matrix* B, int32_t** rp, int32_t** ci, cplx** v,
+                         int64_t* nnz, cudaStream_t st) {
+  CsrRaw a{A->row_ptr, A->col_idx, (const cplx*)A->values}, b{B->row_ptr, B->col_idx, (const cplx*)B->values};
+  return csr_commutator_build(a, b, A->n, rp, ci, v, nnz, st);
+}
+
+int csr_commutator(const magnus_matrix* A, const magnus_matrix* B, int64_t cap, int64_t* nnz_out, int32_t* rp_out,
+                   int32_t* ci_out, cplx* v_out, cudaStream_t st) {
+  int32_t* rp = nullptr;
+  int32_t* ci = nullptr;
+  cplx* v = nullptr;
+  int64_t nnz = 0;
+  int rc = csr_commutator_owned(A, B, &rp, &ci, &v, &nnz, st);
+  if (rc != MAGNUS_OK) return rc;
+  *nnz_out = nnz;
+  if (cap > 0) {
+    if (cap < nnz) {
+      set_error("magnus_commutator_csr: capacity %lld < nnz %lld", (long long)cap, (long long)nnz);
+      rc = MAGNUS_EINVAL;
+    } else {
+      cudaMemcpyAsync(rp_out, rp, sizeof(int32_t) * (size_t)(A->n + 1), cudaMemcpyDeviceToDevice, st);
+      cudaMemcpyAsync(ci_out, ci, sizeof(int32_t) * (size_t)nnz, cudaMemcpyDeviceToDevice, st);
+      cudaMemcpyAsync(v_out, v, sizeof(cplx) * (size_t)nnz, cudaMemcpyDeviceToDevice, st);
+      if (cudaStreamSynchronize(st) != cudaSuccess) rc = MAGNUS_ECUDA;
+    }
+  }
+  cudaFree(rp);
+  cudaFree(ci);
+  cudaFree(v);
+  return rc;
+}
+
+// ---------------------------------------------------------------------------
+// Sampled Hermitian check (magnus_create with check_hermitian): for a strided
+// sample of rows, every stored (i,j) must have a stored (j,i) = conj, found by
+// binary search.  Reports the largest violation.
+// ---------------------------------------------------------------------------
+__global__ void csr_hermitian_check_kernel(CsrRaw A, int64_t n, int64_t stride, double* __restrict__ worst) {
+  double bad = 0.0;
+  for (int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; s * stride < n;
+       s += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t i = s * stride;
+    for (int q = A.rp[i]; q < A.rp[i + 1]; ++q) {
+      const int j = A.ci[q];
+      const cplx a = A.v[q];
+      int lo = A.rp[j], hi = A.rp[j + 1] - 1;
+      cplx b = make_double2(0.0, 0.0);
+      while (lo <= hi) {
+        const int mid = (lo + hi) >> 1;
+        const int c = A.ci[mid];
+        if (c == (int)i) {
+          b = A.v[mid];
+          break;
+        }
+        if (c < (int)i) lo = mid + 1; else hi = mid - 1;
+      }
+      bad = fmax(bad, fmax(fabs(a.x - b.x), fabs(a.y + b.y)));
+    }
+  }
+  double dummy = -INFINITY;
+  double neg = -bad;
+  block_reduce_minmax<256>(neg, dummy);
+  if (threadIdx.x == 0) worst[blockIdx.x] = -neg;
+}
+
+int csr_hermitian_check(const magnus_matrix* A, cudaStream_t st, double* max_violation) {
+  CsrRaw a{A->row_ptr, A->col_idx, (const cplx*)A->values};
+  const int64_t n = A->n;
+  const int64_t stride = n > 65536 ? n / 65536 : 1;
+  const int grid = 64;
+  double* worst = nullptr;
+  if (cudaMalloc(&worst, sizeof(double) * grid) != cudaSuccess) return MAGNUS_ENOMEM;
+  csr_hermitian_check_kernel<<<grid, 256, 0, st>>>(a, n, stride, worst);
+  double h[64];
+  cudaMemcpyAsync(h, worst, sizeof(double) * grid, cudaMemcpyDeviceToHost, st);
+  const cudaError_t e = cudaStreamSynchronize(st);
+  cudaFree(worst);
+  if (e != cudaSuccess) return MAGNUS_ECUDA;
+  double m = 0.0;
+  for (int i = 0; i < grid; ++i) m = h[i] > m ? h[i] : m;
+  *max_violation = m;
+  return MAGNUS_OK;
+}
+
+}  // namespace magnus

@@ -1,0 +1,171 @@
+// S6 -- fused Leja iteration, CSR "row-block" kernel tuned for the spin-chain
+// structure (about N+1 stored entries per row, column = row XOR a small set of
+// masks), but valid for any CSR matrix.
+//
+// Problem with the textbook mappings on this structure: lanes-along-a-row reads
+// the matrix coalesced but gathers w from 32 different cache lines per
+// instruction (one L1 wavefront per stored entry, which is slower than HBM can
+// deliver the matrix); one-thread-per-row gathers w coalesced (32 consecutive
+// rows with the same XOR mask touch 512 contiguous bytes) but reads the matrix
+// with a row-length stride.  This kernel does both coalesced:
+//   1. a warp owns 32 consecutive rows; their entries are one contiguous range of
+//      the CSR arrays, which the warp streams HBM -> shared memory with 16-byte
+//      cp.async (values) and 4-byte cp.async (columns), L2 evict-first;
+//   2. the shared-memory slot of entry e is e + e/8 (one 16-byte pad every
+//      128 bytes), so that the row-strided reads of step 3 spread over the banks;
+//   3. lane l walks row r0+l out of shared memory and gathers w[col] from
+//      global/L1 -- for equal slot numbers the 32 lanes hit one or a few aligned
+//      512-byte segments;
+//   4. the lane finishes its row: w+ = inv_gamma*y - shift*w, p += d_k w+, and
+//      accumulates |w+|^2, |p|^2 (coalesced 16-byte accesses).
+// Deterministic: fixed row->warp map, sequential sum along a row, fixed trees.
+#include "magnus_internal.h"
+#include "device_utils.cuh"
+
+namespace magnus {
+
+namespace {
+
+constexpr int RB_WARPS = 4;                     // warps per CTA
+constexpr int RB_CAP = 768;                     // entries per warp staging buffer
+constexpr int RB_SLOTS = RB_CAP + RB_CAP / 8;   // padded
+constexpr int RB_BYTES_PER_WARP = RB_SLOTS * (int)(sizeof(cplx) + sizeof(int32_t));
+constexpr int RB_SMEM = RB_WARPS * RB_BYTES_PER_WARP;
+constexpr int RB_UNROLL = 8;
+
+__device__ __forceinline__ int rb_slot(int e) { return e + (e >> 3); }
+
+__device__ __forceinline__ void cp_async16(void* dst_smem, const void* src, uint64_t pol) {
+  const unsigned s = (unsigned)__cvta_generic_to_shared(dst_smem);
+  asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;" ::"r"(s), "l"(src), "l"(pol)
+               : "memory");
+}
+__device__ __forceinline__ void cp_async4(void* dst_smem, const void* src, uint64_t pol) {
+  const unsigned s = (unsigned)__cvta_generic_to_shared(dst_smem);
+  asm volatile("cp.async.ca.shared.global.L2::cache_hint [%0], [%1], 4, %2;" ::"r"(s), "l"(src), "l"(pol)
+               : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+__global__ void __launch_bounds__(RB_WARPS * 32, 3)
+    csr_leja_iter_rowblock_kernel(CsrOp op, const cplx* __restrict__ w_in, cplx* __restrict__ w_out,
+                                  cplx* __restrict__ p, double inv_gamma, double shift, cplx dk,
+                                  const LejaStatus* __restrict__ status, double* __restrict__ partials) {
+  if (status->done) return;
+  extern __shared__ __align__(16) unsigned char rb_smem[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  cplx* sv = reinterpret_cast<cplx*>(rb_smem + (size_t)warp * RB_BYTES_PER_WARP);
+  int32_t* sc = reinterpret_cast<int32_t*>(sv + RB_SLOTS);
+  const uint64_t pol = policy_evict_first();
+  const int64_t n = op.n;
+  const int64_t nblocks = (n + 31) >> 5;
+  const int64_t total_warps = (int64_t)gridDim.x * RB_WARPS;
+  double sw = 0.0, sp = 0.0;
+
+  for (int64_t blk = (int64_t)blockIdx.x * RB_WARPS + warp; blk < nblocks; blk += total_warps) {
+    const int64_t row = (blk << 5) + lane;
+    const bool valid = row < n;
+    cplx y = make_double2(0.0, 0.0);
+    for (int t = 0; t < op.nterms; ++t) {
+      const int32_t* __restrict__ rp = op.t[t].rp;
+      const int32_t* __restrict__ ci = op.t[t].ci;
+      const cplx* __restrict__ vv = op.t[t].v;
+      const int rs = rp[valid ? row : n];
+      const int re = rp[valid ? row + 1 : n];
+      cplx a = make_double2(0.0, 0.0);
+      int first = 0;   // first lane (row) of the block not yet consumed
+      while (first < 32) {
+        const int base = __shfl_sync(0xffffffffu, rs, first);
+        const bool fits = (re - base) <= RB_CAP;            // monotone in the lane: re ascends
+        const unsigned nofit = ~__ballot_sync(0xffffffffu, fits || lane < first);
+        const int last = nofit ? (__ffs(nofit) - 1) : 32;   // first lane whose row does not fit any more
+        if (last == first) {
+          // one row longer than the staging buffer: the whole warp strides over it
+          const int e0 = base, e1 = __shfl_sync(0xffffffffu, re, first);
+          cplx b = make_double2(0.0, 0.0);
+          for (int q = e0 + lane; q < e1; q += 32) cfma(b, ld_stream(vv + q, pol), w_in[ld_stream_i32(ci + q, pol)]);
+#pragma unroll
+          for (int o = 16; o > 0; o >>= 1) {
+            b.x += shfl_xor_d(b.x, o);
+            b.y += shfl_xor_d(b.y, o);
+          }
+          if (lane == first) {
+            a.x += b.x;
+            a.y += b.y;
+          }
+          first += 1;
+          continue;
+        }
+        const int len = __shfl_sync(0xffffffffu, re, last - 1) - base;
+        for (int e = lane; e < len; e += 32) {
+          const int s = rb_slot(e);
+          cp_async16(sv + s, vv + base + e, pol);
+          cp_async4(sc + s, ci + base + e, pol);
+        }
+        cp_async_wait_all();
+        __syncwarp();
+        const bool mine = lane >= first && lane < last;
+        const int qs = rs - base;
+        const int mylen = mine ? re - rs : 0;
+        const int maxlen = __reduce_max_sync(0xffffffffu, mylen);
+        for (int j = 0; j < maxlen; j += RB_UNROLL) {
+          cplx xv[RB_UNROLL], mv[RB_UNROLL];
+#pragma unroll
+          for (int u = 0; u < RB_UNROLL; ++u) {
+            const bool ok = j + u < mylen;
+            const int s = ok ? rb_slot(qs + j + u) : 0;
+            mv[u] = ok ? sv[s] : make_double2(0.0, 0.0);
+            const int64_t c = ok ? (int64_t)sc[s] : (valid ? row : 0);
+            xv[u] = w_in[c];
+          }
+#pragma unroll
+          for (int u = 0; u < RB_UNROLL; ++u) cfma(a, mv[u], xv[u]);
+        }
+        __syncwarp();   // everyone done reading before the buffer is refilled
+        first = last;
+      }
+      const cplx ca = cmul(op.t[t].coef, a);
+      y.x += ca.x;
+      y.y += ca.y;
+    }
+    if (valid) {
+      const cplx wi = w_in[row];
+      cplx wn;
+      wn.x = inv_gamma * y.x - shift * wi.x;
+      wn.y = inv_gamma * y.y - shift * wi.y;
+      w_out[row] = wn;
+      cplx pi = p[row];
+      cfma(pi, dk, wn);
+      p[row] = pi;
+      sw += wn.x * wn.x + wn.y * wn.y;
+      sp += pi.x * pi.x + pi.y * pi.y;
+    }
+  }
+  block_reduce_sum2<RB_WARPS * 32>(sw, sp);
+  if (threadIdx.x == 0) {
+    partials[2 * blockIdx.x] = sw;
+    partials[2 * blockIdx.x + 1] = sp;
+  }
+}
+
+}  // namespace
+
+bool csr_rowblock_supported(const CsrOp& op) { return op.n >= 32768; }
+
+int launch_csr_leja_iter_rowblock(const CsrOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma,
+                                  double shift, cplx dk, Workspace* ws, cudaStream_t st) {
+  static bool configured = false;
+  if (!configured) {
+    cudaFuncSetAttribute(csr_leja_iter_rowblock_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, RB_SMEM);
+    configured = true;
+  }
+  const int64_t nblocks = (op.n + 31) >> 5;
+  int64_t g = (nblocks + RB_WARPS - 1) / RB_WARPS;
+  if (g > 148 * 3) g = 148 * 3;
+  csr_leja_iter_rowblock_kernel<<<(int)g, RB_WARPS * 32, RB_SMEM, st>>>(op, w_in, w_out, p, inv_gamma, shift, dk,
+                                                                      ws->status, ws->partials);
+  ws->launches += 1;
+  return (int)g;
+}
+
+}  // namespace magnus

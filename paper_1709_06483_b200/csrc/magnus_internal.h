@@ -1,0 +1,140 @@
+// Internal declarations shared by the translation units of libmagnus_b200.so.
+// Not installed; the public surface is include/magnus.h.
+#ifndef MAGNUS_INTERNAL_H
+#define MAGNUS_INTERNAL_H
+
+#include <complex>
+#include <cstdint>
+
+#include "../../include/magnus.h"
+
+namespace magnus {
+
+const int kMaxDegree = 128;   // m_max (reading c6)
+
+// ---- host_leja.cpp -------------------------------------------------------
+const double* leja_points();                                  // kMaxDegree + 1 points
+void divided_differences(double theta, int m, std::complex<double>* out);
+void snap_interval(double* a, double* b);
+int step_coefficients(int scheme, magnus_drive_fn f, void* user, double t, double tau,
+                      double* coef_h1, double* h_scale, double* kappa);
+
+// ---- error plumbing (api.cu) ----------------------------------------------
+void set_error(const char* fmt, ...);
+
+}  // namespace magnus
+
+#ifdef __CUDACC__
+#include <cuda_runtime.h>
+
+namespace magnus {
+
+typedef double2 cplx;   // (x, y) = (re, im), 16-byte aligned: one LDG.128 / STG.128
+
+// M = sum_t coef[t] * A_t, up to three CSR terms sharing n (H0, H1 and, for M4, C = [H0,H1]).
+struct CsrTerm {
+  const int32_t* rp;
+  const int32_t* ci;
+  const cplx* v;
+  cplx coef;
+  int64_t nnz;
+};
+struct CsrOp {
+  int64_t n;
+  int nterms;
+  CsrTerm t[3];
+};
+
+struct DenseOp {
+  int64_t n;
+  int64_t ld;
+  const cplx* M;
+};
+
+// Device-resident control block of one exponential (row S7): written by the
+// finalize kernel after every iteration, read by the next iteration kernel
+// (early exit) and by the host at chunk boundaries.
+struct LejaStatus {
+  int32_t done;      // 1 once the two-term test was met
+  int32_t iters;     // mat-vecs actually performed (all sub-steps)
+  int32_t k;         // degree reached in the current sub-step
+  int32_t pad;
+  double e_prev;     // e_{k-1} = |d_{k-1}| ||w_{k-1}||
+  double err_est;    // e_k + e_{k-1} at the last test
+  double norm_w2;    // sum |w_k|^2
+  double norm_p2;    // sum |p_k|^2
+};
+
+const int kMaxPartials = 4096;   // upper bound on blocks that write partial sums
+
+struct Workspace {
+  int64_t n = 0;
+  cplx* w[2] = {nullptr, nullptr};   // ping-pong (row i gathers other rows' old w)
+  cplx* p = nullptr;
+  double* partials = nullptr;        // [2 * kMaxPartials]: sum|w|^2, sum|p|^2 per block
+  double* gersh = nullptr;           // [2 * kMaxPartials]: min / max per block, then [0..1] final
+  LejaStatus* status = nullptr;      // device
+  LejaStatus* status_host = nullptr; // pinned
+  double* ab_host = nullptr;         // pinned [2]
+  cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+  int csr_kernel = 0;
+  int64_t launches = 0;
+  double leja_ms = 0.0;
+  bool time_leja = false;
+};
+
+int workspace_alloc(Workspace* ws, int64_t n);
+void workspace_free(Workspace* ws);
+
+struct LejaParams {
+  double tol;
+  double theta_max;
+  int m_max;
+};
+
+// ---- kernels_common.cu ------------------------------------------------------
+void launch_leja_init(const cplx* v, cplx* w, cplx* p, int64_t n, cplx d0, double abs_d0, Workspace* ws,
+                      cudaStream_t st);
+void launch_leja_finalize(int nblk, double abs_dk, double tol, Workspace* ws, cudaStream_t st);
+void launch_leja_finish(const cplx* p, cplx* out, int64_t n, cplx phase, cudaStream_t st, Workspace* ws);
+void launch_minmax_finalize(int nblk, Workspace* ws, cudaStream_t st);
+void launch_scale_copy(const cplx* in, cplx* out, int64_t n, cplx phase, cudaStream_t st, Workspace* ws);
+
+// ---- kernels_csr.cu ---------------------------------------------------------
+// returns the number of blocks that wrote partials
+int launch_csr_gershgorin(const CsrOp& op, Workspace* ws, cudaStream_t st);
+int launch_csr_leja_iter(const CsrOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma, double shift,
+                         cplx dk, Workspace* ws, cudaStream_t st);
+int csr_commutator(const magnus_matrix* A, const magnus_matrix* B, int64_t cap, int64_t* nnz_out, int32_t* rp_out,
+                   int32_t* ci_out, cplx* v_out, cudaStream_t st);
+// same, handing over freshly cudaMalloc'ed arrays (caller frees with cudaFree)
+int csr_commutator_owned(const magnus_matrix* A, const magnus_matrix* B, int32_t** rp, int32_t** ci, cplx** v,
+                         int64_t* nnz, cudaStream_t st);
+int csr_hermitian_check(const magnus_matrix* A, cudaStream_t st, double* max_violation);
+
+// ---- kernels_dense.cu -------------------------------------------------------
+int launch_dense_gershgorin(const DenseOp& op, Workspace* ws, cudaStream_t st);
+// M = A + g*B (elementwise) fused with the Gershgorin row bounds of M
+int launch_dense_assemble(int64_t n, const cplx* A, int64_t lda, const cplx* B, int64_t ldb, double g, cplx* M,
+                          Workspace* ws, cudaStream_t st);
+// A1 = H0 + f1 H1, A2 = H0 + f2 H1 in one pass
+void launch_dense_assemble2(int64_t n, const cplx* H0, int64_t ld0, const cplx* H1, int64_t ld1, double f1, double f2,
+                            cplx* A1, cplx* A2, Workspace* ws, cudaStream_t st);
+// Om = (A1 + A2)/2 - i kappa (P - P^H), written over A1, fused with Gershgorin bounds (row D4)
+int launch_dense_omega(int64_t n, cplx* A1, const cplx* A2, const cplx* P, double kappa, Workspace* ws,
+                       cudaStream_t st);
+// K = P - P^H
+void launch_dense_antiherm(int64_t n, const cplx* P, cplx* K, cudaStream_t st);
+int launch_dense_leja_iter(const DenseOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma, double shift,
+                           cplx dk, Workspace* ws, cudaStream_t st);
+int dense_hermitian_check(const DenseOp& op, cudaStream_t st, double* max_violation);
+
+// ---- zgemm_dmma.cu ----------------------------------------------------------
+int launch_zgemm(int64_t n, const cplx* A, int64_t lda, const cplx* B, int64_t ldb, cplx* C, int64_t ldc,
+                 cudaStream_t st);
+int fp64_peaks(double* dmma_tflops, double* dfma_tflops, cudaStream_t st);
+
+}  // namespace magnus
+#endif  // __CUDACC__
+
+#endif  // MAGNUS_INTERNAL_H

@@ -1,0 +1,425 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C-ABI binding,
+against the CPU oracle on the same seeded inputs.
+
+Bars (BASELINE.json north_star):
+  * integer work (iteration counts, CSR structure of the commutator): exact;
+  * final psi: relative 2-norm error <= 1e-9 at Leja tol 1e-12;
+  * a single fused iteration / mat-vec / GEMM: elementwise, tolerance derived
+    from the summation length (n_terms * eps * magnitude).
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+import torch
+
+import workloads as W
+from workloads import dense, rng, xxz
+
+pytestmark = pytest.mark.gpu
+
+DEV = "cuda"
+
+
+@pytest.fixture(scope="module")
+def M():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_1709_06483_b200 as pkg
+    pkg.lib()
+    return pkg
+
+
+def relerr(a, b):
+    return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
+
+
+def to_dev(x):
+    return x.to(DEV) if hasattr(x, "to") else x
+
+
+def host(x):
+    return x.cpu().numpy()
+
+
+def random_sparse_hermitian(n, density, seed, long_row=None):
+    """General (not XXZ) Hermitian CSR: ragged rows, some empty rows, optionally one long row."""
+    import scipy.sparse as sp
+    r = np.random.default_rng(seed)
+    A = sp.random(n, n, density=density, random_state=np.random.RandomState(seed), format="lil", dtype=np.float64)
+    A = A.tocsr().astype(np.complex128)
+    A.data = r.normal(size=A.nnz) + 1j * r.normal(size=A.nnz)
+    if long_row is not None:
+        row = sp.lil_matrix((n, n), dtype=np.complex128)
+        cols = r.choice(n, size=long_row[1], replace=False)
+        row[long_row[0], cols] = r.normal(size=len(cols)) + 1j * r.normal(size=len(cols))
+        A = A + row.tocsr()
+    H = (A + A.getH()) * 0.5
+    H = H.tolil()
+    empty = r.choice(n, size=max(1, n // 50), replace=False)
+    for e in empty:
+        if long_row is not None and e == long_row[0]:
+            continue
+        H[e, :] = 0
+        H[:, e] = 0
+    H = H.tocsr()
+    H.eliminate_zeros()
+    H.sort_indices()
+    return H
+
+
+def csr_from_scipy(S, device=DEV):
+    return xxz.CSR(S.shape[0], torch.from_numpy(S.indptr.astype(np.int32)).to(device),
+                   torch.from_numpy(S.indices.astype(np.int32)).to(device),
+                   torch.from_numpy(S.data.astype(np.complex128)).to(device))
+
+
+def rand_vec(n, seed):
+    r = np.random.default_rng(seed)
+    v = r.normal(size=n) + 1j * r.normal(size=n)
+    return v / np.linalg.norm(v)
+
+
+# ------------------------------------------------------------------ Gershgorin (S3)
+@pytest.mark.parametrize("N,g", [(6, 0.0), (10, 0.7), (12, -0.31)])
+def test_gershgorin_csr_xxz(M, oracle, N, g):
+    H0, H1 = xxz.xxz_h0(N), xxz.xxz_h1(N)
+    a, b = M.magnus_gershgorin(H0.to(DEV), H1.to(DEV), g)
+    S = (H0.to_scipy() + g * H1.to_scipy()).tocsr()
+    S.sort_indices()
+    (ra, rb), _ = oracle.gershgorin(oracle.CsrHost(S.shape[0], S.indptr.astype(np.int32), S.indices.astype(np.int32),
+                                                   S.data.astype(complex)))
+    assert math.isclose(a, ra, rel_tol=1e-13) and math.isclose(b, rb, rel_tol=1e-13)
+    assert math.isclose(a, -(2.5 + abs(g)) * N, rel_tol=1e-13) and math.isclose(b, (1.5 + abs(g)) * N, rel_tol=1e-13)
+
+
+def test_gershgorin_csr_overlapping_patterns(M, oracle):
+    """H0 and H1 with overlapping patterns: the modulus is taken of the SUMMED entry (c4)."""
+    A = random_sparse_hermitian(700, 0.01, 1)
+    B = random_sparse_hermitian(700, 0.01, 2) + 0.5 * A
+    B = B.tocsr(); B.sort_indices()
+    g = -0.83
+    a, b = M.magnus_gershgorin(csr_from_scipy(A), csr_from_scipy(B), g)
+    S = (A + g * B).tocsr(); S.sort_indices()
+    (ra, rb), _ = oracle.gershgorin(oracle.CsrHost(700, S.indptr.astype(np.int32), S.indices.astype(np.int32),
+                                                   S.data.astype(complex)))
+    assert math.isclose(a, ra, rel_tol=1e-12) and math.isclose(b, rb, rel_tol=1e-12)
+
+
+@pytest.mark.parametrize("n", [1, 7, 200, 777])
+def test_gershgorin_dense(M, oracle, n):
+    H0 = dense.random_hermitian(n, stream=11)
+    H1 = dense.random_hermitian(n, stream=12)
+    a, b = M.magnus_gershgorin(H0.to(DEV), H1.to(DEV), 0.37)
+    (ra, rb), _ = oracle.gershgorin((H0 + 0.37 * H1).numpy())
+    assert math.isclose(a, ra, rel_tol=1e-12, abs_tol=1e-14) and math.isclose(b, rb, rel_tol=1e-12, abs_tol=1e-14)
+    a, b = M.magnus_gershgorin(H0.to(DEV))
+    (ra, rb), _ = oracle.gershgorin(H0.numpy())
+    assert math.isclose(a, ra, rel_tol=1e-12, abs_tol=1e-14) and math.isclose(b, rb, rel_tol=1e-12, abs_tol=1e-14)
+
+
+# ------------------------------------------------------------------ one fused iteration (S6)
+def expected_iteration(oracle, Mh, w, p, inv_gamma, shift, d):
+    y = oracle.matvec(Mh, w)
+    wn = inv_gamma * y - shift * w
+    pn = p + d * wn
+    return wn, pn
+
+
+@pytest.mark.parametrize("N,kernel", [(8, 1), (12, 1), (12, 2), (15, 2), (16, 0)])
+def test_fused_iteration_csr_xxz(M, oracle, N, kernel):
+    n = 1 << N
+    H0, H1 = xxz.xxz_h0(N), xxz.xxz_h1(N)
+    g = 0.61
+    w = rand_vec(n, 1)
+    p = rand_vec(n, 2)
+    S = (H0.to_scipy() + g * H1.to_scipy()).tocsr(); S.sort_indices()
+    Mh = oracle.CsrHost(n, S.indptr.astype(np.int32), S.indices.astype(np.int32), S.data.astype(complex))
+    inv_gamma, shift, d = 1.0 / (0.675 * N), -0.3 + 1.1547, 0.3 - 0.2j
+    wn, pn = expected_iteration(oracle, Mh, w, p, inv_gamma, shift, d)
+    wi, wo, pd = torch.from_numpy(w).to(DEV), torch.zeros(n, dtype=torch.complex128, device=DEV), torch.from_numpy(p).to(DEV)
+    sw, sp, _ = M.magnus_leja_iteration(H0.to(DEV), H1.to(DEV), g, wi, wo, pd, inv_gamma, shift, d, csr_kernel=kernel)
+    tol = 64 * N * np.finfo(float).eps
+    assert np.max(np.abs(host(wo) - wn)) <= tol * np.max(np.abs(wn)) + 1e-300
+    assert np.max(np.abs(host(pd) - pn)) <= tol * np.max(np.abs(pn))
+    assert math.isclose(sw, np.sum(np.abs(wn) ** 2), rel_tol=1e-12)
+    assert math.isclose(sp, np.sum(np.abs(pn) ** 2), rel_tol=1e-12)
+
+
+@pytest.mark.parametrize("kernel", [1, 2])
+def test_fused_iteration_csr_general_ragged(M, oracle, kernel):
+    """Non-power-of-two n, empty rows, one row longer than the row-block staging buffer."""
+    n = 3001
+    S = random_sparse_hermitian(n, 0.004, 5, long_row=(17, 1900))
+    Mh = oracle.CsrHost(n, S.indptr.astype(np.int32), S.indices.astype(np.int32), S.data.astype(complex))
+    w, p = rand_vec(n, 3), rand_vec(n, 4)
+    inv_gamma, shift, d = 0.05, 0.7, -0.11 + 0.4j
+    wn, pn = expected_iteration(oracle, Mh, w, p, inv_gamma, shift, d)
+    wi, wo, pd = torch.from_numpy(w).to(DEV), torch.zeros(n, dtype=torch.complex128, device=DEV), torch.from_numpy(p).to(DEV)
+    sw, sp, _ = M.magnus_leja_iteration(csr_from_scipy(S), None, 0.0, wi, wo, pd, inv_gamma, shift, d, csr_kernel=kernel)
+    assert np.max(np.abs(host(wo) - wn)) <= 1e-13 * max(1.0, np.max(np.abs(wn)))
+    assert np.max(np.abs(host(pd) - pn)) <= 1e-13 * max(1.0, np.max(np.abs(pn)))
+    assert math.isclose(sw, np.sum(np.abs(wn) ** 2), rel_tol=1e-12)
+
+
+@pytest.mark.parametrize("n", [1, 33, 500, 1237])
+def test_fused_iteration_dense(M, oracle, n):
+    H0 = dense.random_hermitian(n, stream=21)
+    H1 = dense.random_hermitian(n, stream=22)
+    g = -0.45
+    Mh = (H0 + g * H1).numpy()
+    w, p = rand_vec(n, 5), rand_vec(n, 6)
+    inv_gamma, shift, d = 0.11, -0.9, 0.02 + 0.5j
+    wn, pn = expected_iteration(oracle, Mh, w, p, inv_gamma, shift, d)
+    wi, wo, pd = torch.from_numpy(w).to(DEV), torch.zeros(n, dtype=torch.complex128, device=DEV), torch.from_numpy(p).to(DEV)
+    sw, sp, _ = M.magnus_leja_iteration(H0.to(DEV), H1.to(DEV), g, wi, wo, pd, inv_gamma, shift, d)
+    tol = 8 * max(n, 16) * np.finfo(float).eps
+    assert np.max(np.abs(host(wo) - wn)) <= tol * max(np.max(np.abs(wn)), np.max(np.abs(w)))
+    assert np.max(np.abs(host(pd) - pn)) <= tol * max(np.max(np.abs(pn)), 1e-3)
+    assert math.isclose(sw, np.sum(np.abs(wn) ** 2), rel_tol=1e-12)
+    assert math.isclose(sp, np.sum(np.abs(pn) ** 2), rel_tol=1e-12)
+
+
+# ------------------------------------------------------------------ leja_expmv (S3-S8)
+@pytest.mark.parametrize("N,h", [(6, 0.3), (10, 0.05), (10, -0.4), (14, 0.1), (16, 0.05)])
+def test_expmv_csr_vs_oracle(M, oracle, N, h):
+    n = 1 << N
+    S = (xxz.xxz_h0(N).to_scipy() + 0.77 * xxz.xxz_h1(N).to_scipy()).tocsr(); S.sort_indices()
+    Mh = oracle.CsrHost(n, S.indptr.astype(np.int32), S.indices.astype(np.int32), S.data.astype(complex))
+    v = rand_vec(n, 7)
+    ref, rinfo = oracle.leja_expmv(Mh, v, h, 1e-12)
+    vi = torch.from_numpy(v).to(DEV)
+    vo = torch.empty_like(vi)
+    info = M.leja_expmv(csr_from_scipy(S), vi, vo, h, 1e-12)
+    assert info["iters"] == rinfo["iters"] and info["substeps"] == rinfo["substeps"]
+    assert info["a"] == rinfo["a"] and info["b"] == rinfo["b"] and info["theta"] == rinfo["theta"]
+    assert relerr(host(vo), ref) <= 1e-12
+    assert abs(np.linalg.norm(host(vo)) - 1.0) < 1e-10
+    # in place
+    info2 = M.leja_expmv(csr_from_scipy(S), vi, vi, h, 1e-12)
+    assert info2["iters"] == info["iters"] and torch.equal(vi, vo)
+
+
+@pytest.mark.parametrize("n,h,scale", [(1, 0.7, 1.0), (2, 1.0, 1.0), (64, 0.3, 0.7), (300, 0.1, 1.0), (1111, -0.05, 1.0)])
+def test_expmv_dense_vs_oracle_and_eigh(M, oracle, n, h, scale):
+    H = (dense.random_hermitian(n, stream=31) * scale).contiguous()
+    v = rand_vec(n, 8)
+    ref, rinfo = oracle.leja_expmv(H.numpy(), v, h, 1e-12)
+    vi = torch.from_numpy(v).to(DEV)
+    vo = torch.empty_like(vi)
+    info = M.leja_expmv(H.to(DEV), vi, vo, h, 1e-12)
+    assert info["iters"] == rinfo["iters"] and info["a"] == rinfo["a"] and info["b"] == rinfo["b"]
+    assert relerr(host(vo), ref) <= 1e-12
+    lam, U = np.linalg.eigh(H.numpy())
+    exact = U @ (np.exp(-1j * h * lam) * (U.conj().T @ v))
+    assert np.linalg.norm(host(vo) - exact) <= 1e-11          # 10 tol (pin c-P3)
+
+
+def test_expmv_degenerate_cases(M, oracle):
+    # M = c I: gamma = 0, zero iterations, exact phase
+    n = 5
+    H = (2.5 * torch.eye(n, dtype=torch.complex128)).to(DEV)
+    v = torch.from_numpy(rand_vec(n, 9)).to(DEV)
+    out = torch.empty_like(v)
+    info = M.leja_expmv(H, v, out, 0.4)
+    assert info["iters"] == 0 and np.allclose(host(out), np.exp(-1j) * host(v), atol=1e-15)
+    # h = 0: exactly two iterations (d_k = 0 for k >= 1), result == input
+    H = dense.random_hermitian(40, stream=41).to(DEV)
+    v = torch.from_numpy(rand_vec(40, 10)).to(DEV)
+    info = M.leja_expmv(H, v, out := torch.empty_like(v), 0.0)
+    assert info["iters"] == 2 and torch.equal(out, v)
+    # theta > theta_max: sub-steps
+    Hh = dense.random_hermitian(24, stream=42) * 3.0
+    (_, _), (sa, sb) = oracle.gershgorin(Hh.numpy())
+    hbig = 40.0 / ((sb - sa) / 4)
+    vv = rand_vec(24, 11)
+    ref, rinfo = oracle.leja_expmv(Hh.numpy(), vv, hbig, 1e-12)
+    vi = torch.from_numpy(vv).to(DEV)
+    info = M.leja_expmv(Hh.to(DEV), vi, vo := torch.empty_like(vi), hbig)
+    assert info["substeps"] == rinfo["substeps"] == 3 and info["iters"] == rinfo["iters"]
+    assert relerr(host(vo), ref) <= 1e-11
+    # diagonal CSR (no off-diagonal entries): componentwise phases
+    import scipy.sparse as sp
+    x = np.array([-1.5, 0.2, 0.9, 3.0])
+    D = sp.diags(x.astype(complex)).tocsr()
+    vv = rand_vec(4, 12)
+    vi = torch.from_numpy(vv).to(DEV)
+    M.leja_expmv(csr_from_scipy(D), vi, vo := torch.empty_like(vi), 0.8)
+    assert np.allclose(host(vo), np.exp(-0.8j * x) * vv, atol=1e-12)
+
+
+def test_expmv_reports_nonconvergence(M):
+    n = 64
+    H = dense.random_hermitian(n, stream=43).to(DEV)
+    v = torch.from_numpy(rand_vec(n, 13)).to(DEV)
+    with pytest.raises(M.MagnusError) as e:
+        M.leja_expmv(H, v, torch.empty_like(v), 0.5, 1e-40)      # unreachable tolerance
+    assert e.value.code == -4
+
+
+# ------------------------------------------------------------------ commutators (S0, D3)
+@pytest.mark.parametrize("n", [8, 64, 130, 257, 600])
+def test_zgemm_dmma_vs_oracle_product(M, oracle, n):
+    A = dense.random_hermitian(n, stream=51)
+    B = dense.random_hermitian(n, stream=52) + 0.1j * torch.triu(torch.ones(n, n, dtype=torch.complex128), 1)
+    Cd = torch.empty(n, n, dtype=torch.complex128, device=DEV)
+    M.magnus_zgemm(A.to(DEV), B.to(DEV), Cd)
+    ref = oracle.matmul(A.numpy(), B.numpy())
+    assert np.max(np.abs(host(Cd) - ref)) <= 8 * n * np.finfo(float).eps * np.max(np.abs(ref)) + 1e-300
+
+
+@pytest.mark.parametrize("n", [48, 200, 333])
+def test_dense_commutator_vs_oracle(M, oracle, n):
+    A = dense.random_hermitian(n, stream=53)
+    B = dense.random_hermitian(n, stream=54)
+    K = torch.empty(n, n, dtype=torch.complex128, device=DEV)
+    work = torch.empty_like(K)
+    M.magnus_commutator_dense(A.to(DEV), B.to(DEV), K, work)
+    ref = oracle.commutator(A.numpy(), B.numpy())           # plain definition AB - BA
+    assert np.max(np.abs(host(K) - ref)) <= 16 * n * np.finfo(float).eps * max(np.max(np.abs(ref)), 1.0)
+    assert np.max(np.abs(host(K) + host(K).conj().T)) == 0.0   # exactly anti-Hermitian by construction
+
+
+@pytest.mark.parametrize("N", [4, 7, 10])
+def test_sparse_commutator_vs_oracle(M, oracle, N):
+    H0, H1 = xxz.xxz_h0(N), xxz.xxz_h1(N)
+    rp, ci, v = M.magnus_commutator_csr(H0.to(DEV), H1.to(DEV))
+    K = oracle.commutator(oracle.CsrHost.of(H0), oracle.CsrHost.of(H1))
+    import scipy.sparse as sp
+    n = 1 << N
+    ref = sp.csr_matrix((K.values, K.col_idx, K.row_ptr), shape=(n, n)); ref.eliminate_zeros(); ref.sort_indices()
+    got = sp.csr_matrix((host(v), host(ci), host(rp)), shape=(n, n))
+    assert got.nnz == N * 2 ** (N - 1) == ref.nnz           # exact zeros dropped (pin c-P11)
+    assert np.array_equal(got.indptr, ref.indptr) and np.array_equal(got.indices, ref.indices)
+    assert np.array_equal(got.data, ref.data)               # small integers: exact
+
+
+def test_sparse_commutator_general(M, oracle):
+    A = random_sparse_hermitian(400, 0.02, 21)
+    B = random_sparse_hermitian(400, 0.02, 22)
+    rp, ci, v = M.magnus_commutator_csr(csr_from_scipy(A), csr_from_scipy(B))
+    import scipy.sparse as sp
+    got = sp.csr_matrix((host(v), host(ci), host(rp)), shape=(400, 400)).toarray()
+    K = oracle.commutator(oracle.CsrHost(400, A.indptr.astype(np.int32), A.indices.astype(np.int32), A.data.astype(complex)),
+                          oracle.CsrHost(400, B.indptr.astype(np.int32), B.indices.astype(np.int32), B.data.astype(complex)))
+    ref = sp.csr_matrix((K.values, K.col_idx, K.row_ptr), shape=(400, 400)).toarray()
+    assert np.max(np.abs(got - ref)) <= 1e-13 * max(1.0, np.max(np.abs(ref)))
+
+
+# ------------------------------------------------------------------ magnus_step / magnus_integrate
+def run_config(M, oracle, cfg, scheme, device_inputs=None):
+    H0, H1, psi0, f = W.build(cfg)
+    if cfg.kind == "xxz":
+        o0, o1 = oracle.CsrHost.of(H0), oracle.CsrHost.of(H1)
+        d0, d1 = H0.to(DEV), H1.to(DEV)
+    else:
+        o0, o1 = H0.numpy(), H1.numpy()
+        d0, d1 = H0.to(DEV), H1.to(DEV)
+    ref, riters = oracle.magnus_integrate(o0, o1, f, scheme, cfg.t0, cfg.t_end, cfg.nsteps, psi0.numpy(), cfg.tol)
+    psi = psi0.to(DEV).clone()
+    with M.magnus_create(d0, d1, f, scheme, tol=cfg.tol) as h:
+        st = h.integrate(cfg.t0, cfg.t_end, cfg.nsteps, psi)
+    return host(psi), st, ref, riters
+
+
+@pytest.mark.parametrize("scheme", ["cf4", "m4"])
+def test_cfg1_full(M, oracle, scheme):
+    """BASELINE config 1 at full size: XXZ N=10, Neel state, T=1, 100 steps."""
+    psi, st, ref, riters = run_config(M, oracle, W.CONFIGS["cfg1"], scheme)
+    assert np.array_equal(st["iters"], riters)              # identical Leja iteration counts
+    assert relerr(psi, ref) <= 1e-9
+    assert abs(np.linalg.norm(psi) - 1) < 1e-10
+
+
+@pytest.mark.parametrize("scheme", ["cf4", "m4"])
+@pytest.mark.parametrize("n,nsteps", [(96, 6), (515, 4)])
+def test_cfg2_scaled(M, oracle, scheme, n, nsteps):
+    """Config 2's recipe (dense random Hermitian, f = sin 3t, tau = 0.02) at sizes with ragged tiles."""
+    cfg = W.scaled(W.CONFIGS["cfg2"], n, nsteps)
+    psi, st, ref, riters = run_config(M, oracle, cfg, scheme)
+    assert np.array_equal(st["iters"], riters)
+    assert relerr(psi, ref) <= 1e-9
+    assert abs(np.linalg.norm(psi) - 1) < 1e-10
+
+
+def test_cfg2_full_cf4(M, oracle):
+    cfg = W.CONFIGS["cfg2"]
+    psi, st, ref, riters = run_config(M, oracle, cfg, "cf4")
+    assert np.array_equal(st["iters"], riters)
+    assert relerr(psi, ref) <= 1e-9
+
+
+def test_cfg2_full_m4_three_steps(M, oracle):
+    """Full n = 2048 with the DMMA commutator; 3 of the 50 steps (the oracle's plain-definition
+    products cost 1.4e11 flop per step on the host)."""
+    cfg = W.scaled(W.CONFIGS["cfg2"], 2048, 3)
+    psi, st, ref, riters = run_config(M, oracle, cfg, "m4")
+    assert np.array_equal(st["iters"], riters)
+    assert relerr(psi, ref) <= 1e-9
+
+
+@pytest.mark.parametrize("scheme", ["cf4", "m4"])
+def test_cfg3_scaled(M, oracle, scheme):
+    """Config 3's recipe (XXZ, random psi0, tau = 0.05) at N = 16: row-block CSR kernel, several waves."""
+    cfg = W.scaled(W.CONFIGS["cfg3"], 16, 4)
+    psi, st, ref, riters = run_config(M, oracle, cfg, scheme)
+    assert np.array_equal(st["iters"], riters)
+    assert relerr(psi, ref) <= 1e-9
+    assert abs(np.linalg.norm(psi) - 1) < 1e-10
+
+
+def test_cfg3_full_two_steps(M, oracle):
+    """Config 3 at full size (N = 20, 32.5M stored entries), 2 of the 20 steps, CF4."""
+    cfg = W.scaled(W.CONFIGS["cfg3"], 20, 2)
+    psi, st, ref, riters = run_config(M, oracle, cfg, "cf4")
+    assert np.array_equal(st["iters"], riters)
+    assert relerr(psi, ref) <= 1e-9
+
+
+def test_step_info_and_time_reversal(M):
+    """Pin c-P10 on the GPU path: step(t, tau) then step(t + tau, -tau) returns psi."""
+    cfg = W.scaled(W.CONFIGS["cfg1"], 8, 1)
+    H0, H1, _, f = W.build(cfg)
+    psi0 = rng.random_unit_vector(256)
+    for scheme in ("cf4", "m4", "m2", "cf4:3"):
+        psi = psi0.to(DEV).clone()
+        with M.magnus_create(H0.to(DEV), H1.to(DEV), f, scheme) as h:
+            infos = h.step(0.2, 0.1, psi)
+            assert len(infos) == {"cf4": 2, "m4": 1, "m2": 1, "cf4:3": 3}[scheme]
+            assert all(i["iters"] > 0 and i["status"] == 0 for i in infos)
+            h.step(0.3, -0.1, psi)
+        assert np.linalg.norm(host(psi) - psi0.numpy()) < 1e-11
+
+
+def test_order_four_on_gpu_path(M):
+    """Pin c-P8 through the CUDA path: step-halving slope 4 for CF4, M4 and CF4:3, 2 for M2."""
+    N = 6
+    H0, H1 = xxz.xxz_h0(N).to(DEV), xxz.xxz_h1(N).to(DEV)
+    psi0 = xxz.neel_state(N)
+    T = 0.5
+
+    def run(scheme, ns, tol=1e-14):
+        psi = psi0.to(DEV).clone()
+        with M.magnus_create(H0, H1, xxz.f_cos2t, scheme, tol=tol) as h:
+            h.integrate(0.0, T, ns, psi)
+        return host(psi)
+
+    for scheme, order in (("cf4", 4), ("m4", 4), ("cf4:3", 4), ("m2", 2)):
+        ref = run(scheme, 512 if order == 4 else 4096)
+        errs = [np.linalg.norm(run(scheme, ns) - ref) for ns in (4, 8, 16)]
+        slopes = [math.log2(errs[i] / errs[i + 1]) for i in range(2)]
+        assert all(order - 0.25 < s < order + 0.25 for s in slopes), (scheme, errs, slopes)
+
+
+def test_integrate_host_end_to_end(M, oracle):
+    cfg = W.CONFIGS["cfg1"]
+    H0, H1, psi0, f = W.build(cfg)
+    ref, riters = oracle.magnus_integrate(oracle.CsrHost.of(H0), oracle.CsrHost.of(H1), f, "cf4", 0.0, 0.1, 10,
+                                          psi0.numpy(), 1e-12)
+    pin = lambda t: t.pin_memory()
+    H0p = xxz.CSR(H0.n, pin(H0.row_ptr), pin(H0.col_idx), pin(H0.values))
+    H1p = xxz.CSR(H1.n, pin(H1.row_ptr), pin(H1.col_idx), pin(H1.values))
+    psi = pin(psi0.clone())
+    st = M.magnus_integrate_host(H0p, H1p, f, "cf4", 0.0, 0.1, 10, psi)
+    assert np.array_equal(st["iters"], riters) and relerr(psi.numpy(), ref) <= 1e-9

@@ -170,6 +170,15 @@ def test_commutator_identities(oracle):
     assert np.allclose(K21, (f1 - f2) * oracle.commutator(A, B), atol=1e-12)
 
 
+def test_dense_product_is_not_transposed(oracle):
+    n = 23
+    A = rand_herm(n, 30) + 0.2j * np.triu(np.ones((n, n)), 2)     # not Hermitian: A@B != (B@A)^H
+    B = rand_herm(n, 31) - 0.4 * np.tril(np.ones((n, n)), -1)
+    assert np.allclose(oracle.matmul(A, B), A @ B, rtol=0, atol=1e-13)
+    assert not np.allclose(oracle.matmul(A, B), B @ A, atol=1e-3)
+    assert not np.allclose(oracle.matmul(A, B), A.T @ B.T, atol=1e-3)
+
+
 def test_sparse_commutator_matches_dense(oracle):
     N = 5
     H0, H1 = csr_pair(oracle, N)
