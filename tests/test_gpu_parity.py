@@ -254,7 +254,9 @@ def test_expmv_reports_nonconvergence(M):
     H = dense.random_hermitian(n, stream=43).to(DEV)
     v = torch.from_numpy(rand_vec(n, 13)).to(DEV)
     with pytest.raises(M.MagnusError) as e:
-        M.leja_expmv(H, v, torch.empty_like(v), 0.5, 1e-40)      # unreachable tolerance
+        # |d_k| decays like theta^k / k!, so the two-term estimate drops below any moderate tol well before
+        # m_max = 128; only a tolerance under the size of d_128 (about 1e-100 at theta = 7) is unreachable
+        M.leja_expmv(H, v, torch.empty_like(v), 2.0, 1e-300)
     assert e.value.code == -4
 
 
