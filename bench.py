@@ -1,0 +1,392 @@
+#!/usr/bin/env python
+"""bench.py -- Magnus steps/s of the CUDA hot path on B200, with its roofline and the oracle beside it.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg5] [--scheme cf4]
+    python bench.py --impl reference ...        # the CPU oracle on the same metric/config (rank 0 only)
+
+A "step" is one Magnus time step t -> t + tau (rows S1..S8 of SURVEY.md section 8(a); D3/D4 too
+for M4 on dense H) through the C-ABI call magnus_integrate on a synthetic workload of
+BASELINE.json (workloads/configs.py).  Default workload: cfg5, the largest single-GPU config
+(XXZ chain N=24, 620,756,992 stored entries, 12.4 GB of CSR: far larger than the 126 MB L2, so no
+flush is needed between timed steps).  Rank 0 prints ONE JSON line.
+
+  value      steps/s, inputs resident in HBM, CUDA events on the launching stream, max over ranks
+  e2e        steps/s of magnus_integrate_host: HOST (pinned) H0, H1, psi -> H2D -> create -> K steps
+             -> D2H psi, all inside the timed region (wall clock around the blocking call)
+  roofline   fused Leja iteration kernel (dense: the GEMV variant; with --scheme m4 on dense H the
+             DMMA commutator): algorithmic bytes (flops) per launch / mean launch time measured
+             live with CUDA events inside the timed region, against MEASURED_PEAKS.json
+  cpu_baseline  the oracle (oracle/, test infrastructure) timed on this box's host cores on a bounded sample
+
+Multi-GPU: the path does not shard ("replicas only"); --gpus N runs N
+independent replicas, one process per GPU, no data-path collective, scaling "weak".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "magnus_steps_per_s"
+UNIT = "steps/s"
+
+
+# ----------------------------------------------------------------------------- helpers
+def load_peaks():
+    """MEASURED_PEAKS.json (driver-written) or the fallback of B200_PROFILING.md."""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as fh:
+            p = json.load(fh)
+        return {"hbm_gbs": float(p["hbm_gbs"]), "source": "measured (MEASURED_PEAKS.json)"}
+    except Exception:
+        return {"hbm_gbs": 6650.0, "source": "fallback (B200_PROFILING.md)"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.lines = []
+        self.thread = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "200"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._pump, daemon=True)
+        self.thread.start()
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)     # at least one sample even for a very short region
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            parts = [x.strip() for x in ln.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0]))
+                mx.append(float(parts[1]))
+                pw.append(float(parts[2]))
+            except ValueError:
+                continue
+            for nm, val in zip(names, parts[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def dist_env():
+    return int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+
+
+def workload_description(cfg, scheme):
+    if cfg.kind == "xxz":
+        N = cfg.size
+        return (f"{cfg.name}: periodic XXZ chain N={N} (dim 2^{N}) + cos(2t) transverse field, CSR complex128/int32, "
+                f"nnz {(1 << N) * (3 * N + 2) // 2}, {scheme.upper()}, tau={cfg.tau:g}, tol={cfg.tol:g}")
+    return (f"{cfg.name}: dense random Hermitian H0 + sin(3t) H1, n={cfg.size} complex128 row-major, "
+            f"{scheme.upper()}, tau={cfg.tau:g}, tol={cfg.tol:g}")
+
+
+def algorithmic_bytes_per_iteration(cfg, scheme):
+    """SURVEY.md section 8(d) / DESIGN.md section 5: what one fused Leja iteration must move."""
+    n = cfg.n
+    if cfg.kind == "xxz":
+        N = cfg.size
+        nnz = (1 << N) * (3 * N + 2) // 2            # H0 + H1 (disjoint patterns)
+        terms = 2
+        if scheme == "m4":
+            nnz += N * (1 << (N - 1))                # cached C = [H0, H1]
+            terms = 3
+        return 20 * nnz + 4 * (n + 1) * terms + 64 * n
+    return 16 * n * n + 64 * n
+
+
+# ----------------------------------------------------------------------------- reference arm (CPU oracle)
+def oracle_sample(cfg, scheme, max_size=None):
+    """The bounded sample the oracle is timed on: ONE Magnus step of the workload's recipe.  The sparse
+    configs and the dense CF4 run at full size where that is tens of seconds; dense M4 by the plain
+    definition (two n^3 products) and the 2^24 chain are reduced, and the sample says so."""
+    import workloads as W
+    size = cfg.size
+    if max_size is not None:
+        size = min(size, max_size)
+    elif cfg.kind == "dense":
+        size = min(size, 2048 if scheme == "m4" else 8192)
+    else:
+        size = min(size, 22)
+    return W.scaled(cfg, size, 1)
+
+
+def time_oracle(cfg, scheme, steps, warmup, max_size=None):
+    """Times `steps` single Magnus steps of the oracle as it stands (OpenMP over rows, plain loops)."""
+    import numpy as np
+    import torch
+    import workloads as W
+    from oracle import oracle as O
+    sample = oracle_sample(cfg, scheme, max_size)
+    dev = "cuda" if torch.cuda.is_available() else "cpu"     # generators only; the oracle gets host arrays
+    H0, H1, psi0, f = W.build(sample, device=dev)
+    if sample.kind == "xxz":
+        o0, o1 = O.CsrHost.of(H0), O.CsrHost.of(H1)
+    else:
+        o0, o1 = H0.cpu().numpy(), H1.cpu().numpy()
+    psi = psi0.cpu().numpy()
+    del H0, H1
+    cores = O.num_threads()
+    times = []
+    for i in range(warmup + steps):
+        t = sample.t0 + i * sample.tau
+        t0 = time.perf_counter()
+        psi, _ = O.magnus_step(o0, o1, f, scheme, t, sample.tau, psi, sample.tol)
+        dt = time.perf_counter() - t0
+        if i >= warmup:
+            times.append(dt)
+    sec = sum(times) / len(times)
+    desc = (f"{len(times)} Magnus step(s) ({scheme.upper()}, tau={sample.tau:g}) of the {cfg.name} recipe at "
+            f"{'N' if sample.kind == 'xxz' else 'n'}={sample.size}"
+            f"{'' if sample.size == cfg.size else f' (reduced from {cfg.size})'}, {sec:.2f} s per step")
+    return {"value": 1.0 / sec, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
+            "sample_size": sample.size, "full_size": cfg.size}
+
+
+def run_reference(args):
+    rank, _, world = dist_env()
+    if rank != 0:
+        return
+    import workloads as W
+    cfg = W.CONFIGS[args.workload]
+    scheme = args.scheme or cfg.schemes[0]
+    base = time_oracle(cfg, scheme, max(1, min(args.steps, 3)), min(args.warmup, 1), args.oracle_max_size)
+    line = {"impl": "reference", "metric": METRIC, "value": base["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 / base["value"], "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "complex128 (f64)", "data": "synthetic",
+            "config": {"workload": workload_description(cfg, scheme), "scheme": scheme,
+                       "note": "CPU oracle (oracle/), rank 0 only; each timed step is one Magnus step of the bounded sample"},
+            "cpu_baseline": {k: base[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "e2e": {"value": base["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ----------------------------------------------------------------------------- our arm
+def measure_workload(M, W, torch, cfg, scheme, steps, warmup, dev, barrier, sampler=None):
+    """Warm up, then time exactly `steps` Magnus steps with inputs resident in HBM."""
+    H0, H1, psi0, f = W.build(cfg, device=dev)
+    stream = torch.cuda.current_stream()
+    out = {}
+    with M.magnus_create(H0, H1, f, scheme, tol=cfg.tol, stream=stream) as h:
+        psi = psi0.clone()
+        if warmup > 0:
+            h.integrate(cfg.t0, cfg.t0 + warmup * cfg.tau, warmup, psi)
+        psi.copy_(psi0)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        torch.cuda.synchronize()
+        if sampler:
+            sampler.start()
+        e0.record(stream)
+        st = h.integrate(cfg.t0, cfg.t0 + steps * cfg.tau, steps, psi)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        barrier()
+        out["clocks"] = sampler.stop() if sampler else None
+        out["seconds"] = e0.elapsed_time(e1) * 1e-3
+        out["stats"] = st
+        out["norm"] = float(torch.linalg.vector_norm(psi))
+    out["inputs"] = (H0, H1, psi0, f)
+    return out
+
+
+def matrix_bytes(H):
+    if hasattr(H, "row_ptr"):
+        return H.values.numel() * 16 + H.col_idx.numel() * 4 + H.row_ptr.numel() * 4
+    return H.numel() * 16
+
+
+def measure_e2e(M, torch, cfg, scheme, steps, inputs):
+    """magnus_integrate_host with pinned HOST buffers: H2D + create + K steps + D2H inside the timed region."""
+    from workloads import xxz
+    H0, H1, psi0, f = inputs
+
+    def pinned(t):
+        return torch.empty(t.shape, dtype=t.dtype, pin_memory=True).copy_(t)
+
+    if hasattr(H0, "row_ptr"):
+        P0 = xxz.CSR(H0.n, pinned(H0.row_ptr), pinned(H0.col_idx), pinned(H0.values))
+        P1 = xxz.CSR(H1.n, pinned(H1.row_ptr), pinned(H1.col_idx), pinned(H1.values))
+    else:
+        P0, P1 = pinned(H0), pinned(H1)
+    psi = pinned(psi0)
+    h2d = matrix_bytes(H0) + matrix_bytes(H1) + psi0.numel() * 16
+    d2h = psi0.numel() * 16
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    st = M.magnus_integrate_host(P0, P1, f, scheme, cfg.t0, cfg.t0 + steps * cfg.tau, steps, psi, tol=cfg.tol,
+                                 stream=torch.cuda.current_stream())
+    torch.cuda.synchronize()
+    sec = time.perf_counter() - t0
+    return {"value": steps / sec, "unit": UNIT, "h2d_bytes_per_step": h2d / steps, "d2h_bytes_per_step": d2h / steps,
+            "seconds": sec, "matvecs": st["total_matvecs"],
+            "region": "one magnus_integrate_host call: H2D of H0, H1, psi0 from pinned host memory (inputs go to the "
+                      "device once per integration, PAPER.md l.209), magnus_create, K steps, D2H of psi"}
+
+
+def roofline_for(cfg, scheme, st, peaks, fp64_peak_tflops):
+    """Dominant kernel of the step: the fused Leja iteration (HBM) or, for M4 on dense H, the DMMA commutator."""
+    leja_s, comm_s, mv = st["seconds_leja"], st["seconds_commutator"], max(1, st["total_matvecs"])
+    nsteps_exp = max(1, st["n_exp"])
+    if cfg.kind == "dense" and scheme == "m4" and comm_s > leja_s:
+        flops = 8.0 * cfg.n ** 3                       # one complex product P = A2 A1 (K = P - P^H)
+        achieved = flops * nsteps_exp / comm_s / 1e12
+        return {"kernel": "zgemm_dmma_kernel", "bound": "tensor", "achieved": achieved, "peak": fp64_peak_tflops,
+                "unit": "TFLOP/s", "frac": achieved / fp64_peak_tflops if fp64_peak_tflops else None, "traffic": None,
+                "peak_source": "FP64 DMMA m8n8k4 register-resident micro-benchmark (magnus_fp64_peaks) run in this process; "
+                               "MEASURED_PEAKS.json has no FP64 figure and the guide gives no bf16->fp64 ratio",
+                "flops_per_launch": flops}
+    nbytes = algorithmic_bytes_per_iteration(cfg, scheme)
+    ms = leja_s / mv * 1e3
+    achieved = nbytes / (ms * 1e-3) / 1e9
+    kernel = "dense_leja_iter_kernel" if cfg.kind == "dense" else "csr_leja_iter_rowblock_kernel"
+    return {"kernel": kernel, "bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+            "frac": achieved / peaks["hbm_gbs"], "traffic": None, "peak_source": peaks["source"],
+            "bytes_per_launch": nbytes, "ms_per_launch": ms,
+            "how": "CUDA events around every Leja sweep (init .. stop) inside the timed region / matvecs: an upper "
+                   "bound on the kernel time (it includes the init, stop-test and early-exit launches)",
+            "frac_of_nominal_8TBs": achieved / 8000.0}
+
+
+def run_ours(args):
+    import torch
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback "
+                         "(use --impl reference for the oracle)")
+    torch.cuda.set_device(local_rank)
+    dev = f"cuda:{local_rank}"
+    use_dist = world > 1
+    if use_dist:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+
+        def barrier():
+            dist.barrier()
+    else:
+        def barrier():
+            pass
+
+    import paper_1709_06483_b200 as M     # raises if the CUDA library is missing
+    import workloads as W
+    M.lib()
+    cfg = W.CONFIGS[args.workload]
+    scheme = args.scheme or cfg.schemes[0]
+    peaks = load_peaks()
+    dmma_tf, dfma_tf = M.magnus_fp64_peaks()
+
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    res = measure_workload(M, W, torch, cfg, scheme, args.steps, args.warmup, dev, barrier, sampler)
+    sec = res["seconds"]
+    if use_dist:
+        t = torch.tensor([sec], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        sec = float(t.item())
+    st = res["stats"]
+
+    e2e = None
+    if not args.no_e2e:
+        e2e = measure_e2e(M, torch, cfg, scheme, args.steps, res["inputs"])
+        if use_dist:
+            t = torch.tensor([e2e["seconds"]], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e2e["seconds"] = float(t.item())
+            e2e["value"] = world * args.steps / e2e["seconds"]
+    res["inputs"] = None
+    torch.cuda.empty_cache()
+
+    if rank == 0:
+        roof = roofline_for(cfg, scheme, st, peaks, dmma_tf)
+        line = {"metric": METRIC, "value": world * args.steps / sec, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": sec / args.steps * 1e3, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "complex128 (f64)", "data": "synthetic",
+                "config": {"workload": workload_description(cfg, scheme), "scheme": scheme,
+                           "parallelism": "replicas only (no sharding, no collective)" if world > 1 else "1 GPU",
+                           "l2": "inputs larger than L2 (no flush needed)" if matrix_bytes_cfg(cfg) > 256e6 else
+                                 "working set fits the 126 MB L2; steps/s is launch/latency bound, not HBM bound",
+                           "matvecs": st["total_matvecs"], "exponentials": st["n_exp"],
+                           "seconds_leja": st["seconds_leja"], "seconds_commutator": st["seconds_commutator"],
+                           "psi_norm_after": res["norm"]},
+                "clocks": res["clocks"], "gpu_launches": st["kernel_launches"], "roofline": roof,
+                "fp64_peaks_measured_tflops": {"dmma": dmma_tf, "dfma": dfma_tf}}
+        if e2e:
+            line["e2e"] = {k: e2e[k] for k in ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step", "region")}
+        if world == 1 and not args.no_cpu_baseline:
+            base = time_oracle(cfg, scheme, 1, 0, args.oracle_max_size)
+            line["cpu_baseline"] = {k: base[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        print(json.dumps(line), flush=True)
+    if use_dist:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def matrix_bytes_cfg(cfg):
+    if cfg.kind == "xxz":
+        return 20 * (1 << cfg.size) * (3 * cfg.size + 2) // 2
+    return 2 * 16 * cfg.size * cfg.size
+
+
+def main():
+    ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--workload", default="cfg5", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
+    ap.add_argument("--scheme", default=None, choices=["cf4", "m4"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--oracle-max-size", type=int, default=None,
+                    help="cap N (xxz) or n (dense) of the oracle's bounded sample")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        if args.warmup < 3:
+            sys.stderr.write("bench.py: note: fewer than 3 warm-up steps\n")
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
