@@ -66,12 +66,29 @@ __global__ void __launch_bounds__(RB_WARPS * 32, 3)
     const int64_t row = (blk << 5) + lane;
     const bool valid = row < n;
     cplx y = make_double2(0.0, 0.0);
-    for (int t = 0; t < op.nterms; ++t) {
-      const int32_t* __restrict__ rp = op.t[t].rp;
+    // issued now, consumed after the last term: row pointers of every term and this row's w, p
+    // (round-1 ncu: 20 % of the stall samples were these dependent loads)
+    int rs_t[3], re_t[3];
+#pragma unroll
+    for (int t = 0; t < 3; ++t) {
+      rs_t[t] = re_t[t] = 0;
+      if (t < op.nterms) {
+        rs_t[t] = op.t[t].rp[valid ? row : n];
+        re_t[t] = op.t[t].rp[valid ? row + 1 : n];
+      }
+    }
+    cplx wi = make_double2(0.0, 0.0), pi = make_double2(0.0, 0.0);
+    if (valid) {
+      wi = w_in[row];
+      pi = p[row];
+    }
+#pragma unroll
+    for (int t = 0; t < 3; ++t) {
+      if (t >= op.nterms) break;
       const int32_t* __restrict__ ci = op.t[t].ci;
       const cplx* __restrict__ vv = op.t[t].v;
-      const int rs = rp[valid ? row : n];
-      const int re = rp[valid ? row + 1 : n];
+      const int rs = rs_t[t];
+      const int re = re_t[t];
       cplx a = make_double2(0.0, 0.0);
       int first = 0;   // first lane (row) of the block not yet consumed
       while (first < 32) {
@@ -129,12 +146,10 @@ __global__ void __launch_bounds__(RB_WARPS * 32, 3)
       y.y += ca.y;
     }
     if (valid) {
-      const cplx wi = w_in[row];
       cplx wn;
       wn.x = inv_gamma * y.x - shift * wi.x;
       wn.y = inv_gamma * y.y - shift * wi.y;
       w_out[row] = wn;
-      cplx pi = p[row];
       cfma(pi, dk, wn);
       p[row] = pi;
       sw += wn.x * wn.x + wn.y * wn.y;
