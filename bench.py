@@ -39,6 +39,10 @@ if ROOT not in sys.path:
 METRIC = "magnus_steps_per_s"
 UNIT = "steps/s"
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+# `ncu --set full` captures (profiles/r1_csr_rowblock_ncu.md, profiles/r1_dense_gemv_ncu.md); None = not captured.
+NCU_TRAFFIC_BYTES = {("cfg5", "cf4"): 15.093e9, ("cfg4", "cf4"): 4.299e9}
+
 
 # ----------------------------------------------------------------------------- helpers
 def load_peaks():
@@ -266,6 +270,13 @@ def measure_e2e(M, torch, cfg, scheme, steps, inputs):
 
 
 def roofline_for(cfg, scheme, st, peaks, fp64_peak_tflops):
+    r = _roofline_for(cfg, scheme, st, peaks, fp64_peak_tflops)
+    if r["bound"] == "hbm":
+        r["traffic"] = NCU_TRAFFIC_BYTES.get((cfg.name, scheme))
+    return r
+
+
+def _roofline_for(cfg, scheme, st, peaks, fp64_peak_tflops):
     """Dominant kernel of the step: the fused Leja iteration (HBM) or, for M4 on dense H, the DMMA commutator."""
     leja_s, comm_s, mv = st["seconds_leja"], st["seconds_commutator"], max(1, st["total_matvecs"])
     nsteps_exp = max(1, st["n_exp"])
