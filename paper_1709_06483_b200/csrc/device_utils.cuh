@@ -13,6 +13,14 @@ typedef double2 cplx;
 __device__ __forceinline__ cplx cmul(cplx a, cplx b) {
   return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
 }
+// |z| for the Gershgorin radii: exact for purely real or imaginary entries (the spin-chain case),
+// one fma + sqrt otherwise (no hypot scaling: |M_ij| of a Hamiltonian is far from over/underflow;
+// the last-ulp difference to hypot is absorbed by the interval snapping, reading c4).
+__device__ __forceinline__ double cabs_fast(cplx z) {
+  if (z.y == 0.0) return fabs(z.x);
+  if (z.x == 0.0) return fabs(z.y);
+  return sqrt(fma(z.x, z.x, z.y * z.y));
+}
 // acc += a * b
 __device__ __forceinline__ void cfma(cplx& acc, cplx a, cplx b) {
   acc.x = fma(a.x, b.x, acc.x);
@@ -57,6 +65,23 @@ __device__ __forceinline__ void ld_stream256(const cplx* p, cplx& a, cplx& b) {
 __device__ __forceinline__ void st_stream(cplx* p, cplx v) {
   asm volatile("st.global.cs.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(v.x), "d"(v.y) : "memory");
 }
+
+// ---- row-block staging (kernels_csr_rowblock.cu, csr_gershgorin_staged_kernel) ----
+// Shared-memory slot of staged entry e: one 16-byte pad every 8 entries, so that 32 lanes reading
+// at a row-length stride spread over the banks.
+__device__ __forceinline__ int rb_slot(int e) { return e + (e >> 3); }
+
+__device__ __forceinline__ void cp_async16(void* dst_smem, const void* src, uint64_t pol) {
+  const unsigned s = (unsigned)__cvta_generic_to_shared(dst_smem);
+  asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;" ::"r"(s), "l"(src), "l"(pol)
+               : "memory");
+}
+__device__ __forceinline__ void cp_async4(void* dst_smem, const void* src, uint64_t pol) {
+  const unsigned s = (unsigned)__cvta_generic_to_shared(dst_smem);
+  asm volatile("cp.async.ca.shared.global.L2::cache_hint [%0], [%1], 4, %2;" ::"r"(s), "l"(src), "l"(pol)
+               : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 __device__ __forceinline__ double shfl_xor_d(double v, int m) { return __shfl_xor_sync(0xffffffffu, v, m); }
 __device__ __forceinline__ double shfl_down_d(double v, int d) { return __shfl_down_sync(0xffffffffu, v, d); }

@@ -42,7 +42,7 @@ __global__ void __launch_bounds__(256) csr_gershgorin_kernel(CsrOp op, double* _
           z.y += prod.y;
           ++q[t];
         }
-      if ((int64_t)c == row) d = z.x; else R += hypot(z.x, z.y);
+      if ((int64_t)c == row) d = z.x; else R += cabs_fast(z);
     }
     lo = fmin(lo, d - R);
     hi = fmax(hi, d + R);
@@ -54,7 +54,115 @@ __global__ void __launch_bounds__(256) csr_gershgorin_kernel(CsrOp op, double* _
   }
 }
 
+// The same bounds for large n with every access coalesced: a warp owns 32 consecutive rows,
+// streams the contiguous entry ranges of ALL terms for those rows into shared memory with
+// cp.async (as the row-block Leja kernel does for one term), then lane l runs the same k-way
+// merge as above over row l out of shared memory.  Same arithmetic and summation order as
+// csr_gershgorin_kernel.  A row block whose entries do not fit the buffer is merged straight
+// from global memory.
+const int GS_WARPS = 6;
+const int GS_CAP = 1600;                    // staged entries per warp, all terms together
+const int GS_SLOTS = GS_CAP + GS_CAP / 8;
+const int GS_BYTES_PER_WARP = GS_SLOTS * (int)(sizeof(cplx) + sizeof(int32_t));
+const int GS_SMEM = GS_WARPS * GS_BYTES_PER_WARP;
+
+__global__ void __launch_bounds__(GS_WARPS * 32, 1) csr_gershgorin_staged_kernel(CsrOp op, double* __restrict__ out) {
+  extern __shared__ __align__(16) unsigned char gs_smem[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  cplx* sv = reinterpret_cast<cplx*>(gs_smem + (size_t)warp * GS_BYTES_PER_WARP);
+  int32_t* sc = reinterpret_cast<int32_t*>(sv + GS_SLOTS);
+  const uint64_t pol = policy_evict_first();
+  const int64_t n = op.n;
+  const int64_t nblocks = (n + 31) >> 5;
+  const int64_t total_warps = (int64_t)gridDim.x * GS_WARPS;
+  double lo = INFINITY, hi = -INFINITY;
+  for (int64_t blk = (int64_t)blockIdx.x * GS_WARPS + warp; blk < nblocks; blk += total_warps) {
+    const int64_t row = (blk << 5) + lane;
+    const bool valid = row < n;
+    int rs[3], re[3], base[3], off[3];
+    int total = 0;
+#pragma unroll
+    for (int t = 0; t < 3; ++t) {
+      rs[t] = re[t] = base[t] = off[t] = 0;
+      if (t < op.nterms) {
+        rs[t] = op.t[t].rp[valid ? row : n];
+        re[t] = op.t[t].rp[valid ? row + 1 : n];
+        base[t] = __shfl_sync(0xffffffffu, rs[t], 0);
+        off[t] = total;
+        total += __shfl_sync(0xffffffffu, re[t], 31) - base[t];
+      }
+    }
+    const bool staged = total <= GS_CAP;
+    if (staged) {
+#pragma unroll
+      for (int t = 0; t < 3; ++t) {
+        if (t < op.nterms) {
+          const int len = (t + 1 < op.nterms ? off[t + 1] : total) - off[t];
+          const cplx* __restrict__ vv = op.t[t].v + base[t];
+          const int32_t* __restrict__ ci = op.t[t].ci + base[t];
+          for (int e = lane; e < len; e += 32) {
+            const int s = rb_slot(off[t] + e);
+            cp_async16(sv + s, vv + e, pol);
+            cp_async4(sc + s, ci + e, pol);
+          }
+        }
+      }
+      cp_async_wait_all();
+      __syncwarp();
+    }
+    int q[3], e[3];
+#pragma unroll
+    for (int t = 0; t < 3; ++t) {
+      q[t] = staged ? off[t] + rs[t] - base[t] : rs[t];
+      e[t] = staged ? off[t] + re[t] - base[t] : re[t];
+    }
+    double R = 0.0, d = 0.0;
+    while (true) {
+      int c = INT_MAX;
+      int cc[3];
+#pragma unroll
+      for (int t = 0; t < 3; ++t) {
+        cc[t] = INT_MAX;
+        if (t < op.nterms && q[t] < e[t]) cc[t] = staged ? sc[rb_slot(q[t])] : op.t[t].ci[q[t]];
+        c = min(c, cc[t]);
+      }
+      if (c == INT_MAX) break;
+      cplx z = make_double2(0.0, 0.0);
+#pragma unroll
+      for (int t = 0; t < 3; ++t)
+        if (cc[t] == c) {
+          const cplx v = staged ? sv[rb_slot(q[t])] : op.t[t].v[q[t]];
+          const cplx prod = cmul(op.t[t].coef, v);
+          z.x += prod.x;
+          z.y += prod.y;
+          ++q[t];
+        }
+      if ((int64_t)c == row) d = z.x; else R += cabs_fast(z);
+    }
+    if (staged) __syncwarp();   // everyone done reading before the buffer is refilled
+    if (valid) {
+      lo = fmin(lo, d - R);
+      hi = fmax(hi, d + R);
+    }
+  }
+  block_reduce_minmax<GS_WARPS * 32>(lo, hi);
+  if (threadIdx.x == 0) {
+    out[2 * blockIdx.x] = lo;
+    out[2 * blockIdx.x + 1] = hi;
+  }
+}
+
 int launch_csr_gershgorin(const CsrOp& op, Workspace* ws, cudaStream_t st) {
+  if (op.n >= 32768) {
+    static bool configured = false;
+    if (!configured) {
+      cudaFuncSetAttribute(csr_gershgorin_staged_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GS_SMEM);
+      configured = true;
+    }
+    csr_gershgorin_staged_kernel<<<148, GS_WARPS * 32, GS_SMEM, st>>>(op, ws->gersh);
+    ws->launches += 1;
+    return 148;
+  }
   int64_t g = (op.n + 255) / 256;
   if (g > 148 * 8) g = 148 * 8;
   csr_gershgorin_kernel<<<(int)g, 256, 0, st>>>(op, ws->gersh);

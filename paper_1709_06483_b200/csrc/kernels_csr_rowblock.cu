@@ -33,20 +33,6 @@ constexpr int RB_BYTES_PER_WARP = RB_SLOTS * (int)(sizeof(cplx) + sizeof(int32_t
 constexpr int RB_SMEM = RB_WARPS * RB_BYTES_PER_WARP;
 constexpr int RB_UNROLL = 8;
 
-__device__ __forceinline__ int rb_slot(int e) { return e + (e >> 3); }
-
-__device__ __forceinline__ void cp_async16(void* dst_smem, const void* src, uint64_t pol) {
-  const unsigned s = (unsigned)__cvta_generic_to_shared(dst_smem);
-  asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;" ::"r"(s), "l"(src), "l"(pol)
-               : "memory");
-}
-__device__ __forceinline__ void cp_async4(void* dst_smem, const void* src, uint64_t pol) {
-  const unsigned s = (unsigned)__cvta_generic_to_shared(dst_smem);
-  asm volatile("cp.async.ca.shared.global.L2::cache_hint [%0], [%1], 4, %2;" ::"r"(s), "l"(src), "l"(pol)
-               : "memory");
-}
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
-
 __global__ void __launch_bounds__(RB_WARPS * 32, 3)
     csr_leja_iter_rowblock_kernel(CsrOp op, const cplx* __restrict__ w_in, cplx* __restrict__ w_out,
                                   cplx* __restrict__ p, double inv_gamma, double shift, cplx dk,

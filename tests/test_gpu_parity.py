@@ -82,7 +82,7 @@ def rand_vec(n, seed):
 
 
 # ------------------------------------------------------------------ Gershgorin (S3)
-@pytest.mark.parametrize("N,g", [(6, 0.0), (10, 0.7), (12, -0.31)])
+@pytest.mark.parametrize("N,g", [(6, 0.0), (10, 0.7), (12, -0.31), (16, 0.45), (18, -1.3)])   # N >= 15: staged kernel
 def test_gershgorin_csr_xxz(M, oracle, N, g):
     H0, H1 = xxz.xxz_h0(N), xxz.xxz_h1(N)
     a, b = M.magnus_gershgorin(H0.to(DEV), H1.to(DEV), g)
@@ -94,15 +94,16 @@ def test_gershgorin_csr_xxz(M, oracle, N, g):
     assert math.isclose(a, -(2.5 + abs(g)) * N, rel_tol=1e-13) and math.isclose(b, (1.5 + abs(g)) * N, rel_tol=1e-13)
 
 
-def test_gershgorin_csr_overlapping_patterns(M, oracle):
+@pytest.mark.parametrize("n,density", [(700, 0.01), (40001, 0.0002)])   # small kernel / staged kernel with a ragged tail
+def test_gershgorin_csr_overlapping_patterns(M, oracle, n, density):
     """H0 and H1 with overlapping patterns: the modulus is taken of the SUMMED entry (c4)."""
-    A = random_sparse_hermitian(700, 0.01, 1)
-    B = random_sparse_hermitian(700, 0.01, 2) + 0.5 * A
+    A = random_sparse_hermitian(n, density, 1, long_row=(5, 2500) if n > 32768 else None)
+    B = random_sparse_hermitian(n, density, 2) + 0.5 * A
     B = B.tocsr(); B.sort_indices()
     g = -0.83
     a, b = M.magnus_gershgorin(csr_from_scipy(A), csr_from_scipy(B), g)
     S = (A + g * B).tocsr(); S.sort_indices()
-    (ra, rb), _ = oracle.gershgorin(oracle.CsrHost(700, S.indptr.astype(np.int32), S.indices.astype(np.int32),
+    (ra, rb), _ = oracle.gershgorin(oracle.CsrHost(n, S.indptr.astype(np.int32), S.indices.astype(np.int32),
                                                    S.data.astype(complex)))
     assert math.isclose(a, ra, rel_tol=1e-12) and math.isclose(b, rb, rel_tol=1e-12)
 
