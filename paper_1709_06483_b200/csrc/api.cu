@@ -80,7 +80,7 @@ struct OpRef {
 };
 
 static int read_interval(int nblk, Workspace* ws, cudaStream_t st, double* a, double* b) {
-  launch_minmax_finalize(nblk, ws, st);
+  (void)nblk;   // the min/max over blocks is taken by the last block of the producing kernel
   CU_TRY(cudaMemcpyAsync(ws->ab_host, ws->gersh + 2 * kMaxPartials, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
   CU_TRY(cudaStreamSynchronize(st));
   *a = ws->ab_host[0];
@@ -94,9 +94,9 @@ static int op_interval(const OpRef& op, Workspace* ws, cudaStream_t st, double* 
 }
 
 static int launch_iter(const OpRef& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma, double shift,
-                       cplx dk, Workspace* ws, cudaStream_t st) {
-  return op.dense ? launch_dense_leja_iter(op.dns, w_in, w_out, p, inv_gamma, shift, dk, ws, st)
-                  : launch_csr_leja_iter(op.csr, w_in, w_out, p, inv_gamma, shift, dk, ws, st);
+                       cplx dk, double abs_dk, double tol, Workspace* ws, cudaStream_t st) {
+  return op.dense ? launch_dense_leja_iter(op.dns, w_in, w_out, p, inv_gamma, shift, dk, abs_dk, tol, ws, st)
+                  : launch_csr_leja_iter(op.csr, w_in, w_out, p, inv_gamma, shift, dk, abs_dk, tol, ws, st);
 }
 
 // ---------------------------------------------------------------------------
@@ -105,8 +105,8 @@ static int launch_iter(const OpRef& op, const cplx* w_in, cplx* w_out, cplx* p, 
 //   w_0 = v, p_0 = d_0 v;  w_k = (1/gamma) M w_{k-1} - (c/gamma + l_{k-1}) w_{k-1};
 //   p_k = p_{k-1} + d_k w_k                                                          (c5)
 //   stop at the first k >= 1 with e_k + e_{k-1} <= tol ||p_k||, e_k = |d_k| ||w_k||    (c6)
-// The stop test is evaluated on the device after every iteration; iteration
-// kernels launched after it fired return immediately.  The host launches a
+// The stop test is evaluated on the device by the last block of every iteration
+// kernel; iteration kernels launched after it fired return immediately.  The host launches a
 // first chunk sized from the table alone (|d_k| + |d_{k-1}| <= tol) plus two,
 // then polls the device status every four iterations.
 // ---------------------------------------------------------------------------
@@ -172,9 +172,8 @@ static int expmv_on_interval(const OpRef& op, double a_raw, double b_raw, const 
         ++k;
         need(k);
         const double shift = c_over_gamma + l[k - 1];
-        const int nblk = launch_iter(op, ws->w[(k - 1) & 1], ws->w[k & 1], ws->p, inv_gamma, shift,
-                                     make_double2(d[k].real(), d[k].imag()), ws, st);
-        launch_leja_finalize(nblk, std::abs(d[k]), prm.tol, ws, st);
+        launch_iter(op, ws->w[(k - 1) & 1], ws->w[k & 1], ws->p, inv_gamma, shift,
+                    make_double2(d[k].real(), d[k].imag()), std::abs(d[k]), prm.tol, ws, st);
       }
       if (ws->time_leja) CU_TRY(cudaEventRecord(ws->ev[1], st));
       CU_TRY(cudaMemcpyAsync(ws->status_host, ws->status, sizeof(LejaStatus), cudaMemcpyDeviceToHost, st));
@@ -660,12 +659,10 @@ int magnus_leja_iteration(const magnus_matrix* H0, const magnus_matrix* H1, doub
   rc = build_op(H0, H1, g, &op, &tmp, &ws, st, &ab);
   if (rc == MAGNUS_OK) {
     cudaMemsetAsync(ws.status, 0, sizeof(LejaStatus), st);
-    int nblk = 0;
     cudaEventRecord(ws.ev[0], st);
-    for (int r = 0; r < reps; ++r)
-      nblk = launch_iter(op, (const cplx*)w_in, (cplx*)w_out, (cplx*)p, inv_gamma, shift, make_double2(d_re, d_im), &ws, st);
+    for (int r = 0; r < reps; ++r)   // |d_k| = 1, tol = 0: the fused stop test only records the norms
+      launch_iter(op, (const cplx*)w_in, (cplx*)w_out, (cplx*)p, inv_gamma, shift, make_double2(d_re, d_im), 1.0, 0.0, &ws, st);
     cudaEventRecord(ws.ev[1], st);
-    launch_leja_finalize(nblk, 1.0, 0.0, &ws, st);
     cudaMemcpyAsync(ws.status_host, ws.status, sizeof(LejaStatus), cudaMemcpyDeviceToHost, st);
     if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) {
       set_error("magnus_leja_iteration: kernel failed");

@@ -3,6 +3,7 @@
 // P:n = PAPER.md line n; c1..c7 = readings in DESIGN.md section 3.
 #include "magnus_internal.h"
 #include "device_utils.cuh"
+#include "leja_finalize.cuh"
 
 #include <cub/device/device_scan.cuh>
 #include <limits.h>
@@ -16,7 +17,7 @@ namespace magnus {
 // merge over the (ascending) column lists, so overlapping patterns are summed
 // before the modulus is taken.  Block min/max go to ws->gersh.
 // ---------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) csr_gershgorin_kernel(CsrOp op, double* __restrict__ out) {
+__global__ void __launch_bounds__(256) csr_gershgorin_kernel(CsrOp op, double* out, unsigned* ticket) {
   double lo = INFINITY, hi = -INFINITY;
   for (int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; row < op.n;
        row += (int64_t)gridDim.x * blockDim.x) {
@@ -52,6 +53,7 @@ __global__ void __launch_bounds__(256) csr_gershgorin_kernel(CsrOp op, double* _
     out[2 * blockIdx.x] = lo;
     out[2 * blockIdx.x + 1] = hi;
   }
+  if (last_block_ticket(ticket)) minmax_finalize_warp0(out, gridDim.x, out + 2 * kMaxPartials);
 }
 
 // The same bounds for large n with every access coalesced: a warp owns 32 consecutive rows,
@@ -66,7 +68,7 @@ const int GS_SLOTS = GS_CAP + GS_CAP / 8;
 const int GS_BYTES_PER_WARP = GS_SLOTS * (int)(sizeof(cplx) + sizeof(int32_t));
 const int GS_SMEM = GS_WARPS * GS_BYTES_PER_WARP;
 
-__global__ void __launch_bounds__(GS_WARPS * 32, 1) csr_gershgorin_staged_kernel(CsrOp op, double* __restrict__ out) {
+__global__ void __launch_bounds__(GS_WARPS * 32, 1) csr_gershgorin_staged_kernel(CsrOp op, double* out, unsigned* ticket) {
   extern __shared__ __align__(16) unsigned char gs_smem[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   cplx* sv = reinterpret_cast<cplx*>(gs_smem + (size_t)warp * GS_BYTES_PER_WARP);
@@ -150,6 +152,7 @@ __global__ void __launch_bounds__(GS_WARPS * 32, 1) csr_gershgorin_staged_kernel
     out[2 * blockIdx.x] = lo;
     out[2 * blockIdx.x + 1] = hi;
   }
+  if (last_block_ticket(ticket)) minmax_finalize_warp0(out, gridDim.x, out + 2 * kMaxPartials);
 }
 
 int launch_csr_gershgorin(const CsrOp& op, Workspace* ws, cudaStream_t st) {
@@ -159,13 +162,13 @@ int launch_csr_gershgorin(const CsrOp& op, Workspace* ws, cudaStream_t st) {
       cudaFuncSetAttribute(csr_gershgorin_staged_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GS_SMEM);
       configured = true;
     }
-    csr_gershgorin_staged_kernel<<<148, GS_WARPS * 32, GS_SMEM, st>>>(op, ws->gersh);
+    csr_gershgorin_staged_kernel<<<148, GS_WARPS * 32, GS_SMEM, st>>>(op, ws->gersh, ws->tickets + 1);
     ws->launches += 1;
     return 148;
   }
   int64_t g = (op.n + 255) / 256;
   if (g > 148 * 8) g = 148 * 8;
-  csr_gershgorin_kernel<<<(int)g, 256, 0, st>>>(op, ws->gersh);
+  csr_gershgorin_kernel<<<(int)g, 256, 0, st>>>(op, ws->gersh, ws->tickets + 1);
   ws->launches += 1;
   return (int)g;
 }
@@ -184,8 +187,8 @@ template <int G>
 __global__ void __launch_bounds__(256) csr_leja_iter_generic(CsrOp op, const cplx* __restrict__ w_in,
                                                               cplx* __restrict__ w_out, cplx* __restrict__ p,
                                                               double inv_gamma, double shift, cplx dk,
-                                                              const LejaStatus* __restrict__ status,
-                                                              double* __restrict__ partials) {
+                                                              double abs_dk, double tol, LejaStatus* status,
+                                                              double* partials, unsigned* ticket) {
   if (status->done) return;
   constexpr int ROWS = 256 / G;
   const int sub = threadIdx.x % G;
@@ -240,37 +243,38 @@ __global__ void __launch_bounds__(256) csr_leja_iter_generic(CsrOp op, const cpl
     partials[2 * blockIdx.x] = sw;
     partials[2 * blockIdx.x + 1] = sp;
   }
+  if (last_block_ticket(ticket)) leja_finalize_warp0(partials, gridDim.x, abs_dk, tol, false, status);   // S7
 }
 
 template <int G>
 static int launch_generic(const CsrOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma, double shift,
-                          cplx dk, Workspace* ws, cudaStream_t st) {
+                          cplx dk, double abs_dk, double tol, Workspace* ws, cudaStream_t st) {
   constexpr int ROWS = 256 / G;
   int64_t g = (op.n + ROWS - 1) / ROWS;
   if (g > 148 * 8) g = 148 * 8;
-  csr_leja_iter_generic<G><<<(int)g, 256, 0, st>>>(op, w_in, w_out, p, inv_gamma, shift, dk, ws->status,
-                                                    ws->partials);
+  csr_leja_iter_generic<G><<<(int)g, 256, 0, st>>>(op, w_in, w_out, p, inv_gamma, shift, dk, abs_dk, tol,
+                                                    ws->status, ws->partials, ws->tickets);
   ws->launches += 1;
   return (int)g;
 }
 
 int launch_csr_leja_iter_rowblock(const CsrOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma,
-                                  double shift, cplx dk, Workspace* ws, cudaStream_t st);
+                                  double shift, cplx dk, double abs_dk, double tol, Workspace* ws, cudaStream_t st);
 bool csr_rowblock_supported(const CsrOp& op);
 
 int launch_csr_leja_iter(const CsrOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma, double shift,
-                         cplx dk, Workspace* ws, cudaStream_t st) {
+                         cplx dk, double abs_dk, double tol, Workspace* ws, cudaStream_t st) {
   if (ws->csr_kernel == 2 || (ws->csr_kernel == 0 && csr_rowblock_supported(op)))
-    return launch_csr_leja_iter_rowblock(op, w_in, w_out, p, inv_gamma, shift, dk, ws, st);
+    return launch_csr_leja_iter_rowblock(op, w_in, w_out, p, inv_gamma, shift, dk, abs_dk, tol, ws, st);
   // lanes per row from the mean stored entries per row and term
   double mean = 0.0;
   for (int t = 0; t < op.nterms; ++t) mean += (double)op.t[t].nnz;
   mean /= (double)op.n * (double)op.nterms;
-  if (mean > 48.0) return launch_generic<32>(op, w_in, w_out, p, inv_gamma, shift, dk, ws, st);
-  if (mean > 24.0) return launch_generic<16>(op, w_in, w_out, p, inv_gamma, shift, dk, ws, st);
-  if (mean > 6.0) return launch_generic<8>(op, w_in, w_out, p, inv_gamma, shift, dk, ws, st);
-  if (mean > 3.0) return launch_generic<4>(op, w_in, w_out, p, inv_gamma, shift, dk, ws, st);
-  return launch_generic<2>(op, w_in, w_out, p, inv_gamma, shift, dk, ws, st);
+  if (mean > 48.0) return launch_generic<32>(op, w_in, w_out, p, inv_gamma, shift, dk, abs_dk, tol, ws, st);
+  if (mean > 24.0) return launch_generic<16>(op, w_in, w_out, p, inv_gamma, shift, dk, abs_dk, tol, ws, st);
+  if (mean > 6.0) return launch_generic<8>(op, w_in, w_out, p, inv_gamma, shift, dk, abs_dk, tol, ws, st);
+  if (mean > 3.0) return launch_generic<4>(op, w_in, w_out, p, inv_gamma, shift, dk, abs_dk, tol, ws, st);
+  return launch_generic<2>(op, w_in, w_out, p, inv_gamma, shift, dk, abs_dk, tol, ws, st);
 }
 
 // ---------------------------------------------------------------------------

@@ -21,6 +21,7 @@
 // Deterministic: fixed row->warp map, sequential sum along a row, fixed trees.
 #include "magnus_internal.h"
 #include "device_utils.cuh"
+#include "leja_finalize.cuh"
 
 namespace magnus {
 
@@ -36,7 +37,8 @@ constexpr int RB_UNROLL = 8;
 __global__ void __launch_bounds__(RB_WARPS * 32, 3)
     csr_leja_iter_rowblock_kernel(CsrOp op, const cplx* __restrict__ w_in, cplx* __restrict__ w_out,
                                   cplx* __restrict__ p, double inv_gamma, double shift, cplx dk,
-                                  const LejaStatus* __restrict__ status, double* __restrict__ partials) {
+                                  double abs_dk, double tol, LejaStatus* status, double* partials,
+                                  unsigned* ticket) {
   if (status->done) return;
   extern __shared__ __align__(16) unsigned char rb_smem[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -147,6 +149,7 @@ __global__ void __launch_bounds__(RB_WARPS * 32, 3)
     partials[2 * blockIdx.x] = sw;
     partials[2 * blockIdx.x + 1] = sp;
   }
+  if (last_block_ticket(ticket)) leja_finalize_warp0(partials, gridDim.x, abs_dk, tol, false, status);   // S7
 }
 
 }  // namespace
@@ -154,7 +157,7 @@ __global__ void __launch_bounds__(RB_WARPS * 32, 3)
 bool csr_rowblock_supported(const CsrOp& op) { return op.n >= 32768; }
 
 int launch_csr_leja_iter_rowblock(const CsrOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma,
-                                  double shift, cplx dk, Workspace* ws, cudaStream_t st) {
+                                  double shift, cplx dk, double abs_dk, double tol, Workspace* ws, cudaStream_t st) {
   static bool configured = false;
   if (!configured) {
     cudaFuncSetAttribute(csr_leja_iter_rowblock_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, RB_SMEM);
@@ -163,8 +166,8 @@ int launch_csr_leja_iter_rowblock(const CsrOp& op, const cplx* w_in, cplx* w_out
   const int64_t nblocks = (op.n + 31) >> 5;
   int64_t g = (nblocks + RB_WARPS - 1) / RB_WARPS;
   if (g > 148 * 3) g = 148 * 3;
-  csr_leja_iter_rowblock_kernel<<<(int)g, RB_WARPS * 32, RB_SMEM, st>>>(op, w_in, w_out, p, inv_gamma, shift, dk,
-                                                                      ws->status, ws->partials);
+  csr_leja_iter_rowblock_kernel<<<(int)g, RB_WARPS * 32, RB_SMEM, st>>>(
+      op, w_in, w_out, p, inv_gamma, shift, dk, abs_dk, tol, ws->status, ws->partials, ws->tickets);
   ws->launches += 1;
   return (int)g;
 }

@@ -4,6 +4,7 @@
 // P:n = PAPER.md line n; c1..c7 = readings in DESIGN.md section 3.
 #include "magnus_internal.h"
 #include "device_utils.cuh"
+#include "leja_finalize.cuh"
 
 namespace magnus {
 
@@ -20,7 +21,7 @@ constexpr int DW = 8;   // warps per block; one row per warp
 template <bool HAS_B, bool WRITE>
 __global__ void __launch_bounds__(DW * 32) dense_assemble_kernel(int64_t n, const cplx* __restrict__ A, int64_t lda,
                                                                   const cplx* __restrict__ B, int64_t ldb, double g,
-                                                                  cplx* __restrict__ M, double* __restrict__ out) {
+                                                                  cplx* __restrict__ M, double* out, unsigned* ticket) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   double lo = INFINITY, hi = -INFINITY;
   for (int64_t row = (int64_t)blockIdx.x * DW + warp; row < n; row += (int64_t)gridDim.x * DW) {
@@ -52,6 +53,7 @@ __global__ void __launch_bounds__(DW * 32) dense_assemble_kernel(int64_t n, cons
     out[2 * blockIdx.x] = lo;
     out[2 * blockIdx.x + 1] = hi;
   }
+  if (last_block_ticket(ticket)) minmax_finalize_warp0(out, gridDim.x, out + 2 * kMaxPartials);
 }
 
 // A1 = H0 + f1 H1, A2 = H0 + f2 H1 (P:262 l.3-4), one pass over H0 and H1.
@@ -75,8 +77,8 @@ __global__ void __launch_bounds__(256) dense_assemble2_kernel(int64_t n, const c
 // Block = 32 x 8 threads, owns a strip of 32 rows.
 // ---------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) dense_omega_kernel(int64_t n, cplx* __restrict__ A1, const cplx* __restrict__ A2,
-                                                           const cplx* __restrict__ P, double kappa,
-                                                           double* __restrict__ out) {
+                                                           const cplx* __restrict__ P, double kappa, double* out,
+                                                           unsigned* ticket) {
   __shared__ cplx tile[32][33];
   const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
   double lo = INFINITY, hi = -INFINITY;
@@ -127,6 +129,7 @@ __global__ void __launch_bounds__(256) dense_omega_kernel(int64_t n, cplx* __res
     out[2 * blockIdx.x] = lo;
     out[2 * blockIdx.x + 1] = hi;
   }
+  if (last_block_ticket(ticket)) minmax_finalize_warp0(out, gridDim.x, out + 2 * kMaxPartials);
 }
 
 // K = P - P^H (for the standalone dense commutator entry point).
@@ -164,8 +167,8 @@ constexpr int GU = 8;   // independent 128-bit loads in flight per lane
 __global__ void __launch_bounds__(DW * 32) dense_leja_iter_kernel(DenseOp op, const cplx* __restrict__ w_in,
                                                                    cplx* __restrict__ w_out, cplx* __restrict__ p,
                                                                    double inv_gamma, double shift, cplx dk,
-                                                                   const LejaStatus* __restrict__ status,
-                                                                   double* __restrict__ partials) {
+                                                                   double abs_dk, double tol, LejaStatus* status,
+                                                                   double* partials, unsigned* ticket) {
   if (status->done) return;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint64_t pol = policy_evict_first();
@@ -209,6 +212,7 @@ __global__ void __launch_bounds__(DW * 32) dense_leja_iter_kernel(DenseOp op, co
     partials[2 * blockIdx.x] = sw;
     partials[2 * blockIdx.x + 1] = sp;
   }
+  if (last_block_ticket(ticket)) leja_finalize_warp0(partials, gridDim.x, abs_dk, tol, false, status);   // S7
 }
 
 // Sampled Hermitian check: pseudo-random (i, j) pairs, largest |M_ij - conj(M_ji)|.
@@ -238,7 +242,8 @@ int row_grid(int64_t n) {
 
 int launch_dense_gershgorin(const DenseOp& op, Workspace* ws, cudaStream_t st) {
   const int g = row_grid(op.n);
-  dense_assemble_kernel<false, false><<<g, DW * 32, 0, st>>>(op.n, op.M, op.ld, nullptr, 0, 0.0, nullptr, ws->gersh);
+  dense_assemble_kernel<false, false><<<g, DW * 32, 0, st>>>(op.n, op.M, op.ld, nullptr, 0, 0.0, nullptr, ws->gersh,
+                                                             ws->tickets + 1);
   ws->launches += 1;
   return g;
 }
@@ -246,7 +251,7 @@ int launch_dense_gershgorin(const DenseOp& op, Workspace* ws, cudaStream_t st) {
 int launch_dense_assemble(int64_t n, const cplx* A, int64_t lda, const cplx* B, int64_t ldb, double g, cplx* M,
                           Workspace* ws, cudaStream_t st) {
   const int grid = row_grid(n);
-  dense_assemble_kernel<true, true><<<grid, DW * 32, 0, st>>>(n, A, lda, B, ldb, g, M, ws->gersh);
+  dense_assemble_kernel<true, true><<<grid, DW * 32, 0, st>>>(n, A, lda, B, ldb, g, M, ws->gersh, ws->tickets + 1);
   ws->launches += 1;
   return grid;
 }
@@ -263,7 +268,7 @@ int launch_dense_omega(int64_t n, cplx* A1, const cplx* A2, const cplx* P, doubl
                        cudaStream_t st) {
   int64_t g = (n + 31) / 32;
   if (g > kMaxPartials) g = kMaxPartials;
-  dense_omega_kernel<<<(int)g, 256, 0, st>>>(n, A1, A2, P, kappa, ws->gersh);
+  dense_omega_kernel<<<(int)g, 256, 0, st>>>(n, A1, A2, P, kappa, ws->gersh, ws->tickets + 1);
   ws->launches += 1;
   return (int)g;
 }
@@ -274,9 +279,10 @@ void launch_dense_antiherm(int64_t n, const cplx* P, cplx* K, cudaStream_t st) {
 }
 
 int launch_dense_leja_iter(const DenseOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma, double shift,
-                           cplx dk, Workspace* ws, cudaStream_t st) {
+                           cplx dk, double abs_dk, double tol, Workspace* ws, cudaStream_t st) {
   const int g = row_grid(op.n);
-  dense_leja_iter_kernel<<<g, DW * 32, 0, st>>>(op, w_in, w_out, p, inv_gamma, shift, dk, ws->status, ws->partials);
+  dense_leja_iter_kernel<<<g, DW * 32, 0, st>>>(op, w_in, w_out, p, inv_gamma, shift, dk, abs_dk, tol, ws->status,
+                                                ws->partials, ws->tickets);
   ws->launches += 1;
   return g;
 }

@@ -74,6 +74,7 @@ struct Workspace {
   double* partials = nullptr;        // [2 * kMaxPartials]: sum|w|^2, sum|p|^2 per block
   double* gersh = nullptr;           // [2 * kMaxPartials]: min / max per block, then [0..1] final
   LejaStatus* status = nullptr;      // device
+  unsigned* tickets = nullptr;       // device [2]: last-block tickets of the Leja and Gershgorin kernels
   LejaStatus* status_host = nullptr; // pinned
   double* ab_host = nullptr;         // pinned [2]
   cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
@@ -95,16 +96,15 @@ struct LejaParams {
 // ---- kernels_common.cu ------------------------------------------------------
 void launch_leja_init(const cplx* v, cplx* w, cplx* p, int64_t n, cplx d0, double abs_d0, Workspace* ws,
                       cudaStream_t st);
-void launch_leja_finalize(int nblk, double abs_dk, double tol, Workspace* ws, cudaStream_t st);
 void launch_leja_finish(const cplx* p, cplx* out, int64_t n, cplx phase, cudaStream_t st, Workspace* ws);
-void launch_minmax_finalize(int nblk, Workspace* ws, cudaStream_t st);
 void launch_scale_copy(const cplx* in, cplx* out, int64_t n, cplx phase, cudaStream_t st, Workspace* ws);
 
 // ---- kernels_csr.cu ---------------------------------------------------------
+// The iteration kernels also run the stop test (S7) in their last block: abs_dk = |d_k|, tol (c6).
 // returns the number of blocks that wrote partials
 int launch_csr_gershgorin(const CsrOp& op, Workspace* ws, cudaStream_t st);
 int launch_csr_leja_iter(const CsrOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma, double shift,
-                         cplx dk, Workspace* ws, cudaStream_t st);
+                         cplx dk, double abs_dk, double tol, Workspace* ws, cudaStream_t st);
 int csr_commutator(const magnus_matrix* A, const magnus_matrix* B, int64_t cap, int64_t* nnz_out, int32_t* rp_out,
                    int32_t* ci_out, cplx* v_out, cudaStream_t st);
 // same, handing over freshly cudaMalloc'ed arrays (caller frees with cudaFree)
@@ -126,7 +126,7 @@ int launch_dense_omega(int64_t n, cplx* A1, const cplx* A2, const cplx* P, doubl
 // K = P - P^H
 void launch_dense_antiherm(int64_t n, const cplx* P, cplx* K, cudaStream_t st);
 int launch_dense_leja_iter(const DenseOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma, double shift,
-                           cplx dk, Workspace* ws, cudaStream_t st);
+                           cplx dk, double abs_dk, double tol, Workspace* ws, cudaStream_t st);
 int dense_hermitian_check(const DenseOp& op, cudaStream_t st, double* max_violation);
 
 // ---- zgemm_dmma.cu ----------------------------------------------------------
