@@ -232,10 +232,62 @@ struct magnus_context {
   int32_t* c_ci = nullptr;
   cplx* c_v = nullptr;
   int64_t c_nnz = 0;
+  // CSR: cached per-term row statistics for the Gershgorin bounds (valid while the terms' patterns are disjoint)
+  double* gs_r[3] = {nullptr, nullptr, nullptr};
+  cplx* gs_diag[3] = {nullptr, nullptr, nullptr};
+  bool gs_disjoint2 = false;   // H0, H1 share no (row, column)
+  bool gs_disjoint3 = false;   // H0, H1, C share none either
   cudaEvent_t ev_comm[2] = {nullptr, nullptr};
   double comm_ms = 0.0;
   bool time_comm = false;
 };
+
+// Row statistics r^t, diag^t of every CSR term and the overlap flags (see csr_gershgorin_cached_kernel).
+static int csr_cache_rowstats(magnus_context* h) {
+  const int64_t n = h->n;
+  CsrTerm T[3];
+  T[0] = csr_term(&h->H0, 1.0, 0.0);
+  T[1] = csr_term(&h->H1, 1.0, 0.0);
+  int nterms = 2;
+  if (h->scheme == MAGNUS_M4 && h->c_nnz > 0) {
+    T[2].rp = h->c_rp;
+    T[2].ci = h->c_ci;
+    T[2].v = h->c_v;
+    T[2].coef = make_double2(1.0, 0.0);
+    T[2].nnz = h->c_nnz;
+    nterms = 3;
+  }
+  int* flags = nullptr;
+  if (cudaMalloc(&flags, 2 * sizeof(int)) != cudaSuccess) { cudaGetLastError(); return MAGNUS_ENOMEM; }
+  cudaMemsetAsync(flags, 0, 2 * sizeof(int), h->stream);
+  for (int t = 0; t < nterms; ++t) {
+    if (cudaMalloc(&h->gs_r[t], sizeof(double) * (size_t)n) != cudaSuccess ||
+        cudaMalloc(&h->gs_diag[t], sizeof(cplx) * (size_t)n) != cudaSuccess) {
+      cudaGetLastError();
+      cudaFree(flags);
+      set_error("row-statistics allocation failed (n=%lld)", (long long)n);
+      return MAGNUS_ENOMEM;
+    }
+    launch_csr_rowstats(T[t], n, h->gs_r[t], h->gs_diag[t], h->stream);
+  }
+  CsrOp op;
+  op.n = n;
+  for (int t = 0; t < 3; ++t) op.t[t] = T[t < nterms ? t : 0];
+  op.nterms = 2;
+  launch_csr_overlap(op, flags, h->stream);
+  if (nterms == 3) {
+    op.nterms = 3;
+    launch_csr_overlap(op, flags + 1, h->stream);
+  }
+  int hf[2] = {1, 1};
+  cudaMemcpyAsync(hf, flags, 2 * sizeof(int), cudaMemcpyDeviceToHost, h->stream);
+  const cudaError_t e = cudaStreamSynchronize(h->stream);
+  cudaFree(flags);
+  if (e != cudaSuccess || cudaGetLastError() != cudaSuccess) { set_error("row-statistics kernels failed"); return MAGNUS_ECUDA; }
+  h->gs_disjoint2 = hf[0] == 0;
+  h->gs_disjoint3 = nterms == 3 && hf[1] == 0;
+  return MAGNUS_OK;
+}
 
 extern "C" {
 
@@ -290,6 +342,10 @@ int magnus_destroy(magnus_handle h) {
   cudaFree(h->c_rp);
   cudaFree(h->c_ci);
   cudaFree(h->c_v);
+  for (int t = 0; t < 3; ++t) {
+    cudaFree(h->gs_r[t]);
+    cudaFree(h->gs_diag[t]);
+  }
   for (int i = 0; i < 2; ++i)
     if (h->ev_comm[i]) cudaEventDestroy(h->ev_comm[i]);
   delete h;
@@ -366,6 +422,10 @@ int magnus_create(magnus_handle* out, const magnus_matrix* H0, const magnus_matr
     if (rc) { magnus_destroy(h); return rc; }
     h->c_nnz = nnz;
   }
+  if (h->format == MAGNUS_CSR) {
+    rc = csr_cache_rowstats(h);
+    if (rc) { magnus_destroy(h); return rc; }
+  }
   if (cudaStreamSynchronize(h->stream) != cudaSuccess) { magnus_destroy(h); return MAGNUS_ECUDA; }
   *out = h;
   return MAGNUS_OK;
@@ -407,7 +467,12 @@ int magnus_step(magnus_handle h, double t, double tau, void* psi_, magnus_step_i
         op.csr.t[1] = csr_term(&h->H1, coef[e], 0.0);
         op.csr.t[2] = op.csr.t[1];
       }
-      rc = op_interval(op, ws, st, &a, &b);                                                        // S3
+      if ((op.csr.nterms == 2 && h->gs_disjoint2) || (op.csr.nterms == 3 && h->gs_disjoint3)) {     // S3
+        const int nblk = launch_csr_gershgorin_cached(op.csr, h->gs_r, h->gs_diag, ws, st);
+        rc = read_interval(nblk, ws, st, &a, &b);
+      } else {
+        rc = op_interval(op, ws, st, &a, &b);
+      }
     } else {
       op.dense = true;
       const cplx* H0v = (const cplx*)h->H0.values;

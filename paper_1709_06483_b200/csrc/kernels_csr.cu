@@ -174,6 +174,121 @@ int launch_csr_gershgorin(const CsrOp& op, Workspace* ws, cudaStream_t st) {
 }
 
 // ---------------------------------------------------------------------------
+// S3 with cached row statistics.  When no column of a row is stored in more than one term
+// (checked once at magnus_create by csr_terms_disjoint), the modulus of the summed entry
+// separates, |sum_t c_t v_t| = |c_t| |v_t| for the one term that holds it, so
+//   R_i = sum_t |c_t| r_i^t,  r_i^t = sum_{j != i} |A_t,ij|;   Re M_ii = sum_t Re(c_t A_t,ii)
+// and the bounds of every exponential follow from the per-term vectors r^t, diag^t (computed
+// once) in one pass over 24 n bytes per term instead of the whole matrix.  Same quantity as
+// csr_gershgorin_kernel up to summation order, which the interval snapping (c4) absorbs.
+// ---------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) csr_rowstats_kernel(CsrTerm T, int64_t n, double* __restrict__ r,
+                                                            cplx* __restrict__ diag) {
+  for (int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; row < n; row += (int64_t)gridDim.x * blockDim.x) {
+    double R = 0.0;
+    cplx d = make_double2(0.0, 0.0);
+    for (int q = T.rp[row]; q < T.rp[row + 1]; ++q) {
+      const cplx v = T.v[q];
+      if ((int64_t)T.ci[q] == row) d = v; else R += cabs_fast(v);
+    }
+    r[row] = R;
+    diag[row] = d;
+  }
+}
+
+// flag |= 1 if some (row, column) is stored in more than one of the terms
+__global__ void __launch_bounds__(256) csr_overlap_kernel(CsrOp op, int* __restrict__ flag) {
+  bool hit = false;
+  for (int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; row < op.n;
+       row += (int64_t)gridDim.x * blockDim.x) {
+    int q[3], e[3];
+#pragma unroll
+    for (int t = 0; t < 3; ++t) {
+      q[t] = t < op.nterms ? op.t[t].rp[row] : 0;
+      e[t] = t < op.nterms ? op.t[t].rp[row + 1] : 0;
+    }
+    while (true) {
+      int c = INT_MAX;
+#pragma unroll
+      for (int t = 0; t < 3; ++t)
+        if (t < op.nterms && q[t] < e[t]) c = min(c, op.t[t].ci[q[t]]);
+      if (c == INT_MAX) break;
+      int cnt = 0;
+#pragma unroll
+      for (int t = 0; t < 3; ++t)
+        if (t < op.nterms && q[t] < e[t] && op.t[t].ci[q[t]] == c) {
+          ++cnt;
+          ++q[t];
+        }
+      hit |= cnt > 1;
+    }
+  }
+  if (hit) atomicOr(flag, 1);
+}
+
+struct RowStats {
+  const double* r[3];
+  const cplx* diag[3];
+  cplx coef[3];
+  int nterms;
+};
+
+__global__ void __launch_bounds__(256) csr_gershgorin_cached_kernel(RowStats S, int64_t n, double* out,
+                                                                     unsigned* ticket) {
+  double lo = INFINITY, hi = -INFINITY;
+  double ac[3];
+#pragma unroll
+  for (int t = 0; t < 3; ++t) ac[t] = t < S.nterms ? cabs_fast(S.coef[t]) : 0.0;
+  for (int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; row < n; row += (int64_t)gridDim.x * blockDim.x) {
+    double R = 0.0, d = 0.0;
+#pragma unroll
+    for (int t = 0; t < 3; ++t)
+      if (t < S.nterms) {
+        const cplx dg = S.diag[t][row];
+        R = fma(ac[t], S.r[t][row], R);
+        d += S.coef[t].x * dg.x - S.coef[t].y * dg.y;
+      }
+    lo = fmin(lo, d - R);
+    hi = fmax(hi, d + R);
+  }
+  block_reduce_minmax<256>(lo, hi);
+  if (threadIdx.x == 0) {
+    out[2 * blockIdx.x] = lo;
+    out[2 * blockIdx.x + 1] = hi;
+  }
+  if (last_block_ticket(ticket)) minmax_finalize_warp0(out, gridDim.x, out + 2 * kMaxPartials);
+}
+
+static int row_grid256(int64_t n) {
+  int64_t g = (n + 255) / 256;
+  if (g > 148 * 8) g = 148 * 8;
+  return (int)g;
+}
+
+void launch_csr_rowstats(const CsrTerm& T, int64_t n, double* r, cplx* diag, cudaStream_t st) {
+  csr_rowstats_kernel<<<row_grid256(n), 256, 0, st>>>(T, n, r, diag);
+}
+
+void launch_csr_overlap(const CsrOp& op, int* flag, cudaStream_t st) {
+  csr_overlap_kernel<<<row_grid256(op.n), 256, 0, st>>>(op, flag);
+}
+
+int launch_csr_gershgorin_cached(const CsrOp& op, const double* const* r, const cplx* const* diag, Workspace* ws,
+                                 cudaStream_t st) {
+  RowStats S;
+  S.nterms = op.nterms;
+  for (int t = 0; t < 3; ++t) {
+    S.r[t] = r[t < op.nterms ? t : 0];
+    S.diag[t] = diag[t < op.nterms ? t : 0];
+    S.coef[t] = op.t[t < op.nterms ? t : 0].coef;
+  }
+  const int g = row_grid256(op.n);
+  csr_gershgorin_cached_kernel<<<g, 256, 0, st>>>(S, op.n, ws->gersh, ws->tickets + 1);
+  ws->launches += 1;
+  return g;
+}
+
+// ---------------------------------------------------------------------------
 // S6 -- fused Leja iteration, generic kernel (any CSR): G lanes share one row.
 //   y_i   = sum_t coef_t sum_q A_t.v[q] w[A_t.ci[q]]            (SpMV of H(t) formed on the fly)
 //   w+_i  = inv_gamma y_i - shift w_i                            (fragment line 4; c5)

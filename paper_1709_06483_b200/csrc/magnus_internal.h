@@ -103,6 +103,11 @@ void launch_scale_copy(const cplx* in, cplx* out, int64_t n, cplx phase, cudaStr
 // The iteration kernels also run the stop test (S7) in their last block: abs_dk = |d_k|, tol (c6).
 // returns the number of blocks that wrote partials
 int launch_csr_gershgorin(const CsrOp& op, Workspace* ws, cudaStream_t st);
+// cached row statistics of one term / overlap test of the terms / bounds from the cached statistics
+void launch_csr_rowstats(const CsrTerm& T, int64_t n, double* r, cplx* diag, cudaStream_t st);
+void launch_csr_overlap(const CsrOp& op, int* flag, cudaStream_t st);
+int launch_csr_gershgorin_cached(const CsrOp& op, const double* const* r, const cplx* const* diag, Workspace* ws,
+                                 cudaStream_t st);
 int launch_csr_leja_iter(const CsrOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma, double shift,
                          cplx dk, double abs_dk, double tol, Workspace* ws, cudaStream_t st);
 int csr_commutator(const magnus_matrix* A, const magnus_matrix* B, int64_t cap, int64_t* nnz_out, int32_t* rp_out,

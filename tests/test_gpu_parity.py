@@ -47,23 +47,21 @@ def random_sparse_hermitian(n, density, seed, long_row=None):
     """General (not XXZ) Hermitian CSR: ragged rows, some empty rows, optionally one long row."""
     import scipy.sparse as sp
     r = np.random.default_rng(seed)
-    A = sp.random(n, n, density=density, random_state=np.random.RandomState(seed), format="lil", dtype=np.float64)
-    A = A.tocsr().astype(np.complex128)
-    A.data = r.normal(size=A.nnz) + 1j * r.normal(size=A.nnz)
+    k = int(density * n * n)
+    A = sp.csr_matrix((r.normal(size=k) + 1j * r.normal(size=k), (r.integers(0, n, size=k), r.integers(0, n, size=k))),
+                      shape=(n, n))          # duplicate positions are summed
     if long_row is not None:
-        row = sp.lil_matrix((n, n), dtype=np.complex128)
         cols = r.choice(n, size=long_row[1], replace=False)
-        row[long_row[0], cols] = r.normal(size=len(cols)) + 1j * r.normal(size=len(cols))
-        A = A + row.tocsr()
-    H = (A + A.getH()) * 0.5
-    H = H.tolil()
+        vals = r.normal(size=len(cols)) + 1j * r.normal(size=len(cols))
+        A = A + sp.csr_matrix((vals, (np.full(len(cols), long_row[0]), cols)), shape=(n, n))
+    H = ((A + A.getH()) * 0.5).tocsr()
     empty = r.choice(n, size=max(1, n // 50), replace=False)
-    for e in empty:
-        if long_row is not None and e == long_row[0]:
-            continue
-        H[e, :] = 0
-        H[:, e] = 0
-    H = H.tocsr()
+    keep = np.ones(n)
+    keep[empty] = 0.0                       # empty rows (and, to stay Hermitian, columns)
+    if long_row is not None:
+        keep[long_row[0]] = 1.0
+    D = sp.diags(keep)
+    H = (D @ H @ D).tocsr()
     H.eliminate_zeros()
     H.sort_indices()
     return H
@@ -426,3 +424,24 @@ def test_integrate_host_end_to_end(M, oracle):
     psi = pin(psi0.clone())
     st = M.magnus_integrate_host(H0p, H1p, f, "cf4", 0.0, 0.1, 10, psi)
     assert np.array_equal(st["iters"], riters) and relerr(psi.numpy(), ref) <= 1e-9
+
+
+@pytest.mark.parametrize("scheme", ["cf4", "m4"])
+def test_step_csr_overlapping_patterns(M, oracle, scheme):
+    """General CSR H0, H1 whose patterns OVERLAP: the handle must not use the cached separable row
+    statistics for the Gershgorin bounds (modulus of the summed entry, c4) and must still match the oracle."""
+    n = 900
+    A = random_sparse_hermitian(n, 0.01, 31)
+    B = (random_sparse_hermitian(n, 0.01, 32) + 0.5 * A).tocsr()
+    B.sort_indices()
+    f = lambda t: math.cos(1.3 * t) - 0.2
+    psi0 = rand_vec(n, 33)
+    oA = oracle.CsrHost(n, A.indptr.astype(np.int32), A.indices.astype(np.int32), A.data.astype(complex))
+    oB = oracle.CsrHost(n, B.indptr.astype(np.int32), B.indices.astype(np.int32), B.data.astype(complex))
+    ref, rinfo = oracle.magnus_step(oA, oB, f, scheme, 0.1, 0.05, psi0, 1e-12)
+    psi = torch.from_numpy(psi0).to(DEV)
+    with M.magnus_create(csr_from_scipy(A), csr_from_scipy(B), f, scheme) as h:
+        info = h.step(0.1, 0.05, psi)
+    assert [i["iters"] for i in info] == [i["iters"] for i in rinfo]
+    assert all(i["a"] == r["a"] and i["b"] == r["b"] for i, r in zip(info, rinfo))
+    assert relerr(host(psi), ref) <= 1e-9
