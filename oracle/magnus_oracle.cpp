@@ -364,12 +364,54 @@ const double kC2 = 0.5 + std::sqrt(3.0) / 6.0;
 const double kAlpha1 = (3.0 - 2.0 * std::sqrt(3.0)) / 12.0;
 const double kAlpha2 = (3.0 + 2.0 * std::sqrt(3.0)) / 12.0;
 
-// Scheme codes: 0 = Cf4, 1 = M4, 101 = M4 with the commutator sign flipped
+// Scheme codes: 0 = Cf4, 1 = M4, 2 = M2, 3 = Cf4:3, 101 = M4 with the commutator sign flipped
 // (a NEGATIVE CONTROL for the order test only: it must drop to order 2).
 double m4_kappa(int scheme, double tau) {
   double kappa = std::sqrt(3.0) * tau / 12.0;
   return scheme == 101 ? -kappa : kappa;
 }
+
+// Commutator-free schemes as a list of exponentials exp(-i h_e (H0 + g_e H1)), in the order
+// they ACT on psi (the right-most factor of the printed product first).  With A_j = -i H(t_j),
+// H = H0 + f H1:  exp(tau sum_j a_ij A_j) = exp(-i tau s_i (H0 + (sum_j a_ij f_j / s_i) H1)),
+// s_i = sum_j a_ij.
+//   scheme 0, Cf4: rows (a1, a2) and (a2, a1); the row (a2, a1) acts first.
+//   scheme 2, M2:   one exponential, h = tau, g = f(t + tau/2).
+//   scheme 3, Cf4:3: nodes c = 1/2 -+ sqrt(15)/10 and 1/2, the printed 3x3 alpha;
+//                                row 3 acts first.
+// Returns the number of exponentials, 0 if the scheme is not commutator-free.
+int cf_exponentials(int scheme, drive_fn f, void* user, double t, double tau, double* h, double* g) {
+  if (scheme == 0) {
+    const double f1 = f(t + kC1 * tau, user), f2 = f(t + kC2 * tau, user);
+    // alpha1 + alpha2 = 1/2 exactly (reading c1): h = tau/2, g_a = 2(a2 f1 + a1 f2), g_b = 2(a1 f1 + a2 f2)
+    h[0] = h[1] = 0.5 * tau;
+    g[0] = 2.0 * (kAlpha2 * f1 + kAlpha1 * f2);
+    g[1] = 2.0 * (kAlpha1 * f1 + kAlpha2 * f2);
+    return 2;
+  }
+  if (scheme == 2) {
+    h[0] = tau;
+    g[0] = f(t + 0.5 * tau, user);
+    return 1;
+  }
+  if (scheme == 3) {
+    const double r15 = std::sqrt(15.0);
+    const double fn[3] = {f(t + (0.5 - r15 / 10.0) * tau, user), f(t + 0.5 * tau, user),
+                          f(t + (0.5 + r15 / 10.0) * tau, user)};
+    const double am = 37.0 / 240.0 - 10.0 * r15 / 261.0, ap = 37.0 / 240.0 + 10.0 * r15 / 261.0;
+    const double alpha[3][3] = {{am, -1.0 / 30.0, ap}, {-11.0 / 360.0, 23.0 / 45.0, -11.0 / 360.0}, {ap, -1.0 / 30.0, am}};
+    for (int e = 0; e < 3; ++e) {
+      const double* row = alpha[2 - e];                                    // row 3 acts first
+      const double s = row[0] + row[1] + row[2];
+      h[e] = tau * s;
+      g[e] = (row[0] * fn[0] + row[1] * fn[1] + row[2] * fn[2]) / s;
+    }
+    return 3;
+  }
+  return 0;
+}
+
+int exponentials_per_step(int scheme) { return scheme == 0 ? 2 : scheme == 3 ? 3 : 1; }
 
 // One step on dense H0, H1.  Cf4: P:132-134 with A = -iH (c1): first
 // exp(-i tau/2 (H0 + g_a H1)), g_a = 2(alpha2 f1 + alpha1 f2), then
@@ -378,19 +420,20 @@ double m4_kappa(int scheme, double tau) {
 // Omega_H = (A1 + A2)/2 - i (sqrt(3) tau / 12) K, psi <- exp(-i tau Omega_H) psi.
 int step_dense(int64_t n, const cplx* H0, const cplx* H1, drive_fn f, void* user, int scheme,
                double t, double tau, cplx* psi, double tol, oracle_expmv_info* infos) {
-  const double f1 = f(t + kC1 * tau, user), f2 = f(t + kC2 * tau, user);
   const int64_t nn = n * n;
-  if (scheme == 0) {
-    const double g[2] = {2.0 * (kAlpha2 * f1 + kAlpha1 * f2), 2.0 * (kAlpha1 * f1 + kAlpha2 * f2)};
+  double hh[3], gg[3];
+  const int ncf = cf_exponentials(scheme, f, user, t, tau, hh, gg);
+  if (ncf > 0) {
     std::vector<cplx> M(nn);
-    for (int e = 0; e < 2; ++e) {
+    for (int e = 0; e < ncf; ++e) {
 #pragma omp parallel for schedule(static)
-      for (int64_t q = 0; q < nn; ++q) M[q] = H0[q] + g[e] * H1[q];
-      int rc = leja_expmv(DenseView(n, M.data()), psi, psi, 0.5 * tau, tol, infos ? infos + e : nullptr);
+      for (int64_t q = 0; q < nn; ++q) M[q] = H0[q] + gg[e] * H1[q];
+      int rc = leja_expmv(DenseView(n, M.data()), psi, psi, hh[e], tol, infos ? infos + e : nullptr);
       if (rc) return rc;
     }
     return 0;
   }
+  const double f1 = f(t + kC1 * tau, user), f2 = f(t + kC2 * tau, user);
   std::vector<cplx> A1(nn), A2(nn), P21(nn), P12(nn), Om(nn);
 #pragma omp parallel for schedule(static)
   for (int64_t q = 0; q < nn; ++q) { A1[q] = H0[q] + f1 * H1[q]; A2[q] = H0[q] + f2 * H1[q]; }
@@ -404,16 +447,17 @@ int step_dense(int64_t n, const cplx* H0, const cplx* H1, drive_fn f, void* user
 
 int step_csr(const CsrView& H0, const CsrView& H1, drive_fn f, void* user, int scheme,
              double t, double tau, cplx* psi, double tol, oracle_expmv_info* infos) {
-  const double f1 = f(t + kC1 * tau, user), f2 = f(t + kC2 * tau, user);
-  if (scheme == 0) {
-    const double g[2] = {2.0 * (kAlpha2 * f1 + kAlpha1 * f2), 2.0 * (kAlpha1 * f1 + kAlpha2 * f2)};
-    for (int e = 0; e < 2; ++e) {
-      SpMat M = sp_axpby(1.0, H0, g[e], H1);
-      int rc = leja_expmv(M.view(), psi, psi, 0.5 * tau, tol, infos ? infos + e : nullptr);
+  double hh[3], gg[3];
+  const int ncf = cf_exponentials(scheme, f, user, t, tau, hh, gg);
+  if (ncf > 0) {
+    for (int e = 0; e < ncf; ++e) {
+      SpMat M = sp_axpby(1.0, H0, gg[e], H1);
+      int rc = leja_expmv(M.view(), psi, psi, hh[e], tol, infos ? infos + e : nullptr);
       if (rc) return rc;
     }
     return 0;
   }
+  const double f1 = f(t + kC1 * tau, user), f2 = f(t + kC2 * tau, user);
   SpMat A1 = sp_axpby(1.0, H0, f1, H1), A2 = sp_axpby(1.0, H0, f2, H1);
   SpMat P21 = sp_mul(A2.view(), A1.view()), P12 = sp_mul(A1.view(), A2.view());
   SpMat K = sp_axpby(1.0, P21.view(), -1.0, P12.view());
@@ -525,7 +569,7 @@ int oracle_commutator_csr(int64_t n, const int32_t* arp, const int32_t* aci, con
   return 0;
 }
 
-// One step t -> t + tau.  infos: room for 2 entries (Cf4 uses both, M4 the first).
+// One step t -> t + tau.  infos: room for 3 entries (Cf4:3 uses all, Cf4 two, M4 and M2 the first).
 int oracle_magnus_step_dense(int64_t n, const double* H0, const double* H1, drive_fn f, void* user,
                              int scheme, double t, double tau, double* psi, double tol,
                              oracle_expmv_info* infos) {
@@ -548,9 +592,9 @@ int oracle_magnus_integrate_dense(int64_t n, const double* H0, const double* H1,
                                   int scheme, double t0, double t_end, int64_t nsteps, double* psi,
                                   double tol, int32_t* iters_out, int64_t iters_cap) {
   const double tau = (t_end - t0) / (double)nsteps;
-  const int per = scheme == 0 ? 2 : 1;
+  const int per = exponentials_per_step(scheme);
   for (int64_t s = 0; s < nsteps; ++s) {
-    oracle_expmv_info infos[2];
+    oracle_expmv_info infos[3];
     int rc = oracle_magnus_step_dense(n, H0, H1, f, user, scheme, t0 + (double)s * tau, tau, psi, tol, infos);
     if (rc) return rc;
     for (int e = 0; e < per; ++e)
@@ -564,9 +608,9 @@ int oracle_magnus_integrate_csr(int64_t n, const int32_t* rp0, const int32_t* ci
                                 int scheme, double t0, double t_end, int64_t nsteps, double* psi,
                                 double tol, int32_t* iters_out, int64_t iters_cap) {
   const double tau = (t_end - t0) / (double)nsteps;
-  const int per = scheme == 0 ? 2 : 1;
+  const int per = exponentials_per_step(scheme);
   for (int64_t s = 0; s < nsteps; ++s) {
-    oracle_expmv_info infos[2];
+    oracle_expmv_info infos[3];
     int rc = oracle_magnus_step_csr(n, rp0, ci0, v0, rp1, ci1, v1, f, user, scheme, t0 + (double)s * tau, tau,
                                     psi, tol, infos);
     if (rc) return rc;

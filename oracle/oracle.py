@@ -13,8 +13,9 @@ import numpy as np
 
 from . import build as _build
 
-CF4, M4, M4_WRONG_SIGN = 0, 1, 101
-SCHEMES = {"cf4": CF4, "m4": M4, "m4_wrong_sign": M4_WRONG_SIGN}
+CF4, M4, M2, CF4_3, M4_WRONG_SIGN = 0, 1, 2, 3, 101
+SCHEMES = {"cf4": CF4, "m4": M4, "m2": M2, "cf4:3": CF4_3, "m4_wrong_sign": M4_WRONG_SIGN}
+N_EXP = {CF4: 2, M4: 1, M2: 1, CF4_3: 3, M4_WRONG_SIGN: 1}
 
 DRIVE = C.CFUNCTYPE(C.c_double, C.c_double, C.c_void_p)
 
@@ -162,7 +163,7 @@ def _drive(f: Callable[[float], float]):
 
 def magnus_step(H0, H1, f, scheme: str, t: float, tau: float, psi, tol: float = 1e-12):
     psi = _c(psi, np.complex128).copy()
-    infos = (ExpmvInfo * 2)()
+    infos = (ExpmvInfo * 3)()
     cb = _drive(f)
     sc = C.c_int(SCHEMES[scheme])
     if isinstance(H0, CsrHost):
@@ -172,14 +173,14 @@ def magnus_step(H0, H1, f, scheme: str, t: float, tau: float, psi, tol: float = 
         rc = lib().oracle_magnus_step_dense(C.c_int64(H0.shape[0]), _p(H0), _p(H1), cb, None, sc, C.c_double(t), C.c_double(tau), _p(psi), C.c_double(tol), infos)
     if rc != 0:
         raise RuntimeError(f"oracle magnus_step failed rc={rc}")
-    nexp = 2 if SCHEMES[scheme] == CF4 else 1
+    nexp = N_EXP[SCHEMES[scheme]]
     return psi, [infos[i].as_dict() for i in range(nexp)]
 
 
 def magnus_integrate(H0, H1, f, scheme: str, t0: float, t_end: float, nsteps: int, psi, tol: float = 1e-12):
     """Returns (psi_final, iteration counts per exponential in call order)."""
     psi = _c(psi, np.complex128).copy()
-    nexp = (2 if SCHEMES[scheme] == CF4 else 1) * nsteps
+    nexp = N_EXP[SCHEMES[scheme]] * nsteps
     iters = np.zeros(nexp, dtype=np.int32)
     cb = _drive(f)
     sc = C.c_int(SCHEMES[scheme])

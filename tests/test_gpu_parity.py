@@ -445,3 +445,17 @@ def test_step_csr_overlapping_patterns(M, oracle, scheme):
     assert [i["iters"] for i in info] == [i["iters"] for i in rinfo]
     assert all(i["a"] == r["a"] and i["b"] == r["b"] for i, r in zip(info, rinfo))
     assert relerr(host(psi), ref) <= 1e-9
+
+
+# ------------------------------------------------------------------ M2 and Cf4:3 against the oracle
+@pytest.mark.parametrize("scheme", ["m2", "cf4:3"])
+@pytest.mark.parametrize("name,size,nsteps", [("cfg1", 10, 20), ("cfg3", 16, 3), ("cfg2", 515, 4)])
+def test_m2_cf43_vs_oracle(M, oracle, scheme, name, size, nsteps):
+    """The other two commutator-free schemes of the paper through the same kernels:
+    identical iteration counts per exponential (1 resp. 3 per step), psi within 1e-9."""
+    cfg = W.scaled(W.CONFIGS[name], size, nsteps)
+    psi, st, ref, riters = run_config(M, oracle, cfg, scheme)
+    assert len(riters) == nsteps * {"m2": 1, "cf4:3": 3}[scheme]
+    assert np.array_equal(st["iters"], riters)
+    assert relerr(psi, ref) <= 1e-9
+    assert abs(np.linalg.norm(psi) - 1) < 1e-10

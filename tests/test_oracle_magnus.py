@@ -247,3 +247,71 @@ def test_cfg1_totals_are_stable(oracle):
     assert 1e-10 < np.linalg.norm(out["cf4"][0] - out["m4"][0]) < 1e-8
     gold = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "cfg1_oracle.json")))
     assert out["cf4"][1] == gold["cf4"]["total_matvecs"] and out["m4"][1] == gold["m4"]["total_matvecs"]
+
+
+# ------------------------------------------------------------------ M2 and Cf4:3
+def _exact_propagator_reference(H0, H1, f, t0, T, fine=30000):
+    """Brute force: exponential midpoint with EXACT (eigh) exponentials on a very fine grid."""
+    psi = None
+    tau = (T - t0) / fine
+    U = np.eye(H0.shape[0], dtype=complex)
+    for s in range(fine):
+        lam, V = np.linalg.eigh(H0 + f(t0 + (s + 0.5) * tau) * H1)
+        U = (V * np.exp(-1j * tau * lam)) @ V.conj().T @ U
+    return U
+
+
+@pytest.mark.parametrize("scheme,order", [("m2", 2), ("cf4:3", 4)])
+def test_order_of_m2_and_cf43(oracle, scheme, order):
+    """P:95 "which is of order two"; "optimized commutator-free method of order 4": step-halving slope
+    against a brute-force reference that does not use the oracle."""
+    n = 12
+    r = np.random.default_rng(3)
+    def herm():
+        G = r.normal(size=(n, n)) + 1j * r.normal(size=(n, n))
+        return (G + G.conj().T) / 2
+    H0, H1 = herm(), herm()
+    f = lambda t: math.sin(3 * t) + 0.3 * t
+    psi0 = r.normal(size=n) + 1j * r.normal(size=n); psi0 /= np.linalg.norm(psi0)
+    T = 0.4
+    exact = _exact_propagator_reference(H0, H1, f, 0.0, T) @ psi0
+    errs = []
+    for ns in (4, 8, 16):      # the order-2 brute-force reference is good to about 1e-10
+        psi, _ = oracle.magnus_integrate(H0, H1, f, scheme, 0.0, T, ns, psi0, 1e-14)
+        errs.append(np.linalg.norm(psi - exact))
+    slopes = [math.log2(errs[i] / errs[i + 1]) for i in range(2)]
+    assert all(order - 0.3 < s < order + 0.35 for s in slopes), (errs, slopes)
+
+
+def test_cf43_smaller_error_constant_than_cf4(oracle):
+    """Cf4:3 has a smaller error constant than Cf4 (same order)."""
+    n = 10
+    r = np.random.default_rng(4)
+    G = r.normal(size=(n, n)) + 1j * r.normal(size=(n, n)); H0 = (G + G.conj().T) / 2
+    G = r.normal(size=(n, n)) + 1j * r.normal(size=(n, n)); H1 = (G + G.conj().T) / 2
+    f = lambda t: math.cos(2 * t)
+    psi0 = np.zeros(n, complex); psi0[0] = 1
+    exact = _exact_propagator_reference(H0, H1, f, 0.0, 0.5) @ psi0
+    e = {}
+    for scheme in ("cf4", "cf4:3"):
+        psi, _ = oracle.magnus_integrate(H0, H1, f, scheme, 0.0, 0.5, 10, psi0, 1e-14)
+        e[scheme] = np.linalg.norm(psi - exact)
+    assert e["cf4:3"] < e["cf4"]
+
+
+@pytest.mark.parametrize("scheme", ["m2", "cf4:3"])
+def test_m2_cf43_time_independent_and_reversal(oracle, scheme):
+    """f = const: every scheme is the exact exponential (row sums of alpha add up to 1); and
+    step(t, tau) followed by step(t + tau, -tau) is the identity (both schemes are self-adjoint)."""
+    n = 16
+    r = np.random.default_rng(6)
+    G = r.normal(size=(n, n)) + 1j * r.normal(size=(n, n)); H0 = (G + G.conj().T) / 2
+    G = r.normal(size=(n, n)) + 1j * r.normal(size=(n, n)); H1 = (G + G.conj().T) / 2
+    psi0 = r.normal(size=n) + 1j * r.normal(size=n); psi0 /= np.linalg.norm(psi0)
+    psi, _ = oracle.magnus_integrate(H0, H1, lambda t: 0.7, scheme, 0.0, 0.6, 3, psi0, 1e-13)
+    lam, V = np.linalg.eigh(H0 + 0.7 * H1)
+    assert np.linalg.norm(psi - V @ (np.exp(-0.6j * lam) * (V.conj().T @ psi0))) < 1e-11
+    f = lambda t: math.sin(3 * t)
+    a, _ = oracle.magnus_step(H0, H1, f, scheme, 0.2, 0.1, psi0, 1e-13)
+    b, _ = oracle.magnus_step(H0, H1, f, scheme, 0.3, -0.1, a, 1e-13)
+    assert np.linalg.norm(b - psi0) < 1e-11
