@@ -158,8 +158,50 @@ static int expmv_on_interval(const OpRef& op, double a_raw, double b_raw, const 
 
   const double inv_gamma = 1.0 / gamma, c_over_gamma = c / gamma;
   const cplx phase = make_double2(std::cos(hs * c), -std::sin(hs * c));
-  CU_TRY(cudaMemsetAsync(ws->status, 0, sizeof(LejaStatus), st));
   float ms = 0.f;
+  if (!op.dense && n <= kSmallSweepMaxN && ws->csr_kernel == 0) {
+    // small CSR problem: each sub-step sweep is ONE launch (kernels_csr_small.cu); the table first
+    // covers `have` terms and is extended to m_max only if the sweep asks for more
+    SweepTable tab;
+    for (int sub = 0; sub < s; ++sub) {
+      const cplx* src = sub == 0 ? v_in : v_out;
+      int m_try = std::min(prm.m_max, std::max(have - 1, first_chunk));
+      while (true) {
+        need(m_try);
+        for (int k = 0; k <= m_try; ++k) {
+          tab.d[k] = make_double2(d[k].real(), d[k].imag());
+          tab.l[k] = l[k];
+        }
+        CU_TRY(cudaMemsetAsync(ws->status, 0, sizeof(LejaStatus), st));
+        if (ws->time_leja) CU_TRY(cudaEventRecord(ws->ev[0], st));
+        launch_csr_leja_sweep_small(op.csr, src, v_out, inv_gamma, c_over_gamma, prm.tol, m_try, phase, tab, ws, st);
+        if (ws->time_leja) CU_TRY(cudaEventRecord(ws->ev[1], st));
+        CU_TRY(cudaMemcpyAsync(ws->status_host, ws->status, sizeof(LejaStatus), cudaMemcpyDeviceToHost, st));
+        CU_TRY(cudaStreamSynchronize(st));
+        if (ws->time_leja) {
+          CU_TRY(cudaEventElapsedTime(&ms, ws->ev[0], ws->ev[1]));
+          ws->leja_ms += ms;
+        }
+        loc.err_est = ws->status_host->err_est;
+        if (ws->status_host->done) {
+          loc.iters += ws->status_host->k;
+          break;
+        }
+        if (m_try >= prm.m_max) {
+          loc.iters += ws->status_host->k;
+          loc.status = MAGNUS_ENOCONV;
+          if (info) *info = loc;
+          set_error("Leja interpolation did not reach tol=%g within m_max=%d (theta=%g)", prm.tol, prm.m_max, theta);
+          return MAGNUS_ENOCONV;
+        }
+        m_try = prm.m_max;   // the input vector is untouched (nothing is written without convergence): redo in full
+      }
+    }
+    CU_TRY(cudaGetLastError());
+    if (info) *info = loc;
+    return MAGNUS_OK;
+  }
+  CU_TRY(cudaMemsetAsync(ws->status, 0, sizeof(LejaStatus), st));
   for (int sub = 0; sub < s; ++sub) {
     const cplx* src = sub == 0 ? v_in : v_out;
     if (ws->time_leja) CU_TRY(cudaEventRecord(ws->ev[0], st));

@@ -65,6 +65,13 @@ struct LejaStatus {
   double norm_p2;    // sum |p_k|^2
 };
 
+// Small CSR problems run a whole Leja sweep in one single-CTA launch (kernels_csr_small.cu).
+const int kSmallSweepMaxN = 4096;
+struct SweepTable {
+  cplx d[kMaxDegree + 1];     // divided differences d_k (c3)
+  double l[kMaxDegree + 1];   // Leja points l_k (c2)
+};
+
 const int kMaxPartials = 4096;   // upper bound on blocks that write partial sums
 
 struct Workspace {
@@ -116,6 +123,13 @@ int csr_commutator(const magnus_matrix* A, const magnus_matrix* B, int64_t cap, 
 int csr_commutator_owned(const magnus_matrix* A, const magnus_matrix* B, int32_t** rp, int32_t** ci, cplx** v,
                          int64_t* nnz, cudaStream_t st);
 int csr_hermitian_check(const magnus_matrix* A, cudaStream_t st, double* max_violation);
+
+// ---- kernels_csr_small.cu ---------------------------------------------------
+// one sub-step sweep (S5-S8) in one launch; on success status->done = 1, status->k = iterations and out is
+// written; if tab's m_max iterations do not meet tol, status->pad = 1 and out is left untouched
+void launch_csr_leja_sweep_small(const CsrOp& op, const cplx* v, cplx* out, double inv_gamma, double c_over_gamma,
+                                 double tol, int m_max, cplx phase, const SweepTable& tab, Workspace* ws,
+                                 cudaStream_t st);
 
 // ---- kernels_dense.cu -------------------------------------------------------
 int launch_dense_gershgorin(const DenseOp& op, Workspace* ws, cudaStream_t st);
