@@ -291,7 +291,10 @@ def _roofline_for(cfg, scheme, st, peaks, fp64_peak_tflops):
     nbytes = algorithmic_bytes_per_iteration(cfg, scheme)
     ms = leja_s / mv * 1e3
     achieved = nbytes / (ms * 1e-3) / 1e9
-    kernel = "dense_leja_iter_kernel" if cfg.kind == "dense" else "csr_leja_iter_rowblock_kernel"
+    kernel = "dense_leja_iter_kernel" if cfg.kind == "dense" else (
+        "csr_leja_iter_rowblock_kernel" if cfg.n >= 32768 else
+        "csr_leja_sweep_small_kernel (whole sweep in one launch; L1/L2-resident, latency bound: the HBM fraction is not meaningful)"
+        if cfg.n <= 4096 else "csr_leja_iter_generic")
     return {"kernel": kernel, "bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
             "frac": achieved / peaks["hbm_gbs"], "traffic": None, "peak_source": peaks["source"],
             "bytes_per_launch": nbytes, "ms_per_launch": ms,
