@@ -459,3 +459,37 @@ def test_m2_cf43_vs_oracle(M, oracle, scheme, name, size, nsteps):
     assert np.array_equal(st["iters"], riters)
     assert relerr(psi, ref) <= 1e-9
     assert abs(np.linalg.norm(psi) - 1) < 1e-10
+
+
+# ------------------------------------------------------------------ the paper's own workloads
+@pytest.mark.parametrize("scheme", ["cf4", "m4", "cf4:3"])
+def test_paper_example2_local_heisenberg(M, oracle, scheme):
+    """Example 2: Jx, Jy, Jz = 1, 2, 3, z-field sin t, CSR with n + 1 entries per row, tau = 1e-3 as in the
+    paper's runs, plus a larger step.  H1 is diagonal here, so H0 and H1 OVERLAP on the diagonal."""
+    from workloads import paper_examples as pe
+    n = 10
+    H0, H1 = pe.example2_csr(n)
+    psi0 = pe.initial_value(n)
+    o0, o1 = oracle.CsrHost.of(H0), oracle.CsrHost.of(H1)
+    for t_end, nsteps in ((0.005, 5), (0.3, 6)):
+        ref, riters = oracle.magnus_integrate(o0, o1, pe.f_sin_t, scheme, 0.0, t_end, nsteps, psi0.numpy(), 1e-12)
+        psi = psi0.to(DEV).clone()
+        with M.magnus_create(H0.to(DEV), H1.to(DEV), pe.f_sin_t, scheme) as h:
+            st = h.integrate(0.0, t_end, nsteps, psi)
+        assert np.array_equal(st["iters"], riters)
+        assert relerr(host(psi), ref) <= 1e-9
+
+
+@pytest.mark.parametrize("scheme", ["cf4", "m4"])
+def test_paper_example1_nonlocal_heisenberg(M, oracle, scheme):
+    """Example 1: J_ij = 1/|i-j|, x-field sin t, stored dense (N = 2^8)."""
+    from workloads import paper_examples as pe
+    n = 8
+    H0, H1 = pe.example1_dense(n)
+    psi0 = pe.initial_value(n)
+    ref, riters = oracle.magnus_integrate(H0.numpy(), H1.numpy(), pe.f_sin_t, scheme, 0.0, 0.2, 4, psi0.numpy(), 1e-12)
+    psi = psi0.to(DEV).clone()
+    with M.magnus_create(H0.to(DEV), H1.to(DEV), pe.f_sin_t, scheme) as h:
+        st = h.integrate(0.0, 0.2, 4, psi)
+    assert np.array_equal(st["iters"], riters)
+    assert relerr(host(psi), ref) <= 1e-9

@@ -127,3 +127,47 @@ def test_random_unit_vector_and_configs():
     s = W.scaled(c["cfg3"], 8, nsteps=3)
     assert s.n == 256 and math.isclose(s.tau, 0.05) and s.nsteps == 3
     assert xxz.f_cos2t(0.3) == math.cos(0.6) and dense.f_sin3t(0.3) == math.sin(3 * 0.3)
+
+
+# ------------------------------------------------------------------ the paper's own Examples 1 and 2
+@pytest.mark.parametrize("n", [3, 4, 5])
+def test_paper_example1_matches_kronecker_definition(n):
+    from workloads import paper_examples as pe
+    H0k = np.zeros((1 << n, 1 << n), dtype=complex)
+    H1k = np.zeros_like(H0k)
+    for i in range(1, n + 1):
+        for j in range(1, n + 1):
+            if i != j:
+                H0k -= (1.0 / abs(i - j)) * site_op(SZ, i, n) @ site_op(SZ, j, n)
+        H1k -= site_op(SX, i, n)
+    H0, H1 = pe.example1_dense(n)
+    assert np.allclose(H0.numpy(), H0k, atol=1e-14) and np.array_equal(H1.numpy(), H1k)
+
+
+@pytest.mark.parametrize("n", [3, 4, 5, 6])
+def test_paper_example2_matches_kronecker_definition(n):
+    from workloads import paper_examples as pe
+    jx, jy, jz = 1.0, 2.0, 3.0
+    H0k = np.zeros((1 << n, 1 << n), dtype=complex)
+    H1k = np.zeros_like(H0k)
+    for j in range(1, n + 1):
+        k = j % n + 1                       # periodic reading of sigma_{n+1}
+        H0k -= 0.5 * (jx * site_op(SX, j, n) @ site_op(SX, k, n) + jy * site_op(SY, j, n) @ site_op(SY, k, n)
+                      + jz * site_op(SZ, j, n) @ site_op(SZ, k, n))
+        H1k -= 0.5 * site_op(SZ, j, n)
+    H0, H1 = pe.example2_csr(n)
+    assert np.allclose(H0.to_scipy().toarray(), H0k, atol=1e-14)
+    assert np.array_equal(H1.to_scipy().toarray(), H1k)
+    assert H0.nnz == (1 << n) * (n + 1)                     # exactly n + 1 stored entries per row
+    ci = H0.col_idx.view(1 << n, n + 1)
+    assert bool((ci[:, 1:] > ci[:, :-1]).all())             # ascending, no duplicates
+
+
+def test_paper_initial_value():
+    from workloads import paper_examples as pe
+    n = 6
+    psi = pe.initial_value(n).numpy()
+    assert abs(np.linalg.norm(psi) - 1) < 1e-14
+    sz1 = site_op(SZ, 1, n)
+    sz2 = site_op(SZ, 2, n)
+    assert abs(np.vdot(psi, sz1 @ psi) - 1) < 1e-14 and abs(np.vdot(psi, sz2 @ psi) + 1) < 1e-14   # up, down
