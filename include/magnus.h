@@ -78,7 +78,8 @@ typedef struct magnus_options {
   int32_t m_max;       /* maximal interpolation degree per sub-step (c6); default and maximum 128 */
   int32_t check_hermitian; /* 1: sampled check in magnus_create (costs a device pass); default 0 */
   void* stream;        /* cudaStream_t; NULL = legacy default stream */
-  int32_t csr_kernel;  /* 0 auto, 1 force the generic row-per-subwarp kernel, 2 force the row-block kernel */
+  int32_t csr_kernel;  /* 0 auto (n <= 4096: whole sweep in one launch; n >= 32768: row-block kernel; else generic),
+                          1 force the generic per-iteration kernel, 2 force the row-block per-iteration kernel */
   int32_t reserved;
 } magnus_options;
 
@@ -117,7 +118,10 @@ typedef struct magnus_context* magnus_handle;
  *           (kept alive and unmodified by the caller).
  *   f,user  the scalar drive; called on the host.
  *   scheme  MAGNUS_CF4 / MAGNUS_M4 / MAGNUS_M2 / MAGNUS_CF4_3.
- * Allocates every workspace once (w ping-pong, p, partial-norm buffers; dense: the
+ * Allocates every workspace once (w ping-pong, p, partial-norm buffers; CSR: per-term row
+ * statistics for the Gershgorin bounds, 24 n bytes per term, and a test whether the terms'
+ * patterns overlap -- c4 takes the modulus of the SUMMED entry, which separates only if
+ * they do not; dense: the
  * assembled matrix, and for M4 the node matrices A1, A2 and the product P; CSR
  * M4: computes and owns the sparse commutator C = [H0, H1] -- row S0 of the
  * scope table -- so that a step only rescales it, since

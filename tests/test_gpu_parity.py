@@ -493,3 +493,31 @@ def test_paper_example1_nonlocal_heisenberg(M, oracle, scheme):
         st = h.integrate(0.0, 0.2, 4, psi)
     assert np.array_equal(st["iters"], riters)
     assert relerr(host(psi), ref) <= 1e-9
+
+
+def test_small_csr_sweep_paths(M, oracle):
+    """The single-launch sweep (n <= 4096): non-convergence is reported and leaves the vector untouched;
+    sub-steps chain sweeps; forcing the per-iteration kernels (csr_kernel=1) gives the same counts and result."""
+    N = 9
+    n = 1 << N
+    S = (xxz.xxz_h0(N).to_scipy() + 0.4 * xxz.xxz_h1(N).to_scipy()).tocsr(); S.sort_indices()
+    Hd = csr_from_scipy(S)
+    v = torch.from_numpy(rand_vec(n, 21)).to(DEV)
+    keep = v.clone()
+    with pytest.raises(M.MagnusError) as e:
+        M.leja_expmv(Hd, v, v, 1.5, 1e-300)                  # in place: must not be overwritten on failure
+    assert e.value.code == -4 and torch.equal(v, keep)
+    Mh = oracle.CsrHost(n, S.indptr.astype(np.int32), S.indices.astype(np.int32), S.data.astype(complex))
+    ref, rinfo = oracle.leja_expmv(Mh, host(keep), 2.0, 1e-25)   # two sub-steps, long sweeps (the oracle's
+    out = torch.empty_like(v)                                    # __float128 table is exact to about 1e-32)
+    info = M.leja_expmv(Hd, v, out, 2.0, 1e-25)
+    assert info["substeps"] == rinfo["substeps"] == 2
+    assert info["iters"] == rinfo["iters"] and relerr(host(out), ref) <= 1e-12
+    H0, H1 = xxz.xxz_h0(N).to(DEV), xxz.xxz_h1(N).to(DEV)
+    res = {}
+    for ck in (0, 1):
+        psi = keep.clone()
+        with M.magnus_create(H0, H1, xxz.f_cos2t, "cf4", csr_kernel=ck) as h:
+            st = h.integrate(0.0, 0.2, 4, psi)
+        res[ck] = (st["iters"], host(psi))
+    assert np.array_equal(res[0][0], res[1][0]) and relerr(res[0][1], res[1][1]) <= 1e-13
