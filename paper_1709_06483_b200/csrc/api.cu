@@ -174,7 +174,10 @@ static int expmv_on_interval(const OpRef& op, double a_raw, double b_raw, const 
         }
         CU_TRY(cudaMemsetAsync(ws->status, 0, sizeof(LejaStatus), st));
         if (ws->time_leja) CU_TRY(cudaEventRecord(ws->ev[0], st));
-        launch_csr_leja_sweep_small(op.csr, src, v_out, inv_gamma, c_over_gamma, prm.tol, m_try, phase, tab, ws, st);
+        if (launch_csr_leja_sweep_small(op.csr, src, v_out, inv_gamma, c_over_gamma, prm.tol, m_try, phase, tab, ws, st)) {
+          set_error("small-sweep cluster launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+          return MAGNUS_ECUDA;
+        }
         if (ws->time_leja) CU_TRY(cudaEventRecord(ws->ev[1], st));
         CU_TRY(cudaMemcpyAsync(ws->status_host, ws->status, sizeof(LejaStatus), cudaMemcpyDeviceToHost, st));
         CU_TRY(cudaStreamSynchronize(st));

@@ -1,140 +1,205 @@
 // S5-S8 in ONE launch for small CSR problems (n <= kSmallSweepMaxN, e.g. CFG1: n = 1024,
-// 0.33 MB of matrix, resident in L1/L2): one CTA of 1024 threads runs a whole Leja sweep of a
-// sub-step -- init, the fused iterations with the stop test after each, finish -- separated
-// by __syncthreads() instead of kernel boundaries.  At this size a launch (a few microseconds)
-// costs more than an iteration, so the per-iteration kernels of the large path are launch bound.
+// 0.33 MB of matrix): one thread-block CLUSTER of 8 CTAs runs a whole Leja sweep of a sub-step
+// -- init, the fused iterations with the stop test after each, finish -- separated by cluster
+// barriers instead of kernel boundaries.  At this size a launch (a few microseconds) costs more
+// than an iteration, so the per-iteration kernels of the large path are launch bound.
 //   w_0 = v, p_0 = d_0 v;  w_k = (1/gamma) M w_{k-1} - (c/gamma + l_{k-1}) w_{k-1};  p_k += d_k w_k   (c5)
 //   stop at the first k >= 1 with |d_k| ||w_k|| + |d_{k-1}| ||w_{k-1}|| <= tol ||p_k||               (c6)
 //   out = e^{-i (h/s) c} p_k                                                                          (c7)
-// The divided differences and Leja points arrive as a kernel argument (3 KB, __grid_constant__).
-// Thread t owns rows t, t + 1024, ...; its p entries stay in registers, w ping-pongs through
-// global memory (L1/L2) because every row gathers other rows' previous w.  Deterministic: sequential
-// sum along a row, fixed block-reduction tree.
+// Layout: CTA c owns the contiguous row slice [c n/8, (c+1) n/8); SS_G lanes share a row; p of the
+// slice lives in shared memory.  EVERY CTA holds the whole vector w in its shared memory (ping-pong,
+// 2 x 16 n bytes): after computing its slice of the new w a CTA passes one cluster barrier and pulls
+// the other seven slices through distributed shared memory, so the gathers of the next iteration are
+// local shared-memory reads.  The CTA's slice of the CSR terms is copied to shared memory once per
+// sweep when it fits (cluster barriers flush L1, so global reads would pay an L2 round trip per
+// dependent load in every iteration); otherwise it is read in place.  The per-CTA partial norms are
+// pulled the same way; every CTA sums the eight partials in the same order and takes the same stop
+// decision.  The divided differences and Leja points arrive as a kernel argument (3 KB,
+// __grid_constant__).  Deterministic: fixed lane->entry map, fixed trees.
+// Measured (clock64, CFG1): about 10,000 cycles per iteration -- row slice 4,000, block reduction
+// 1,100, cluster barrier 1,400, DSMEM pull 1,650, stop test (hypot, sqrt) 1,300.
 #include "magnus_internal.h"
 #include "device_utils.cuh"
+
+#include <cooperative_groups.h>
+
+namespace cg = cooperative_groups;
 
 namespace magnus {
 
 namespace {
 
-constexpr int SS_THREADS = 1024;
-constexpr int SS_ROWS = kSmallSweepMaxN / SS_THREADS;   // rows per thread
-constexpr int SS_U = 6;                                 // entries in flight per thread
+constexpr int SS_CTAS = 8;                 // portable cluster size
+constexpr int SS_THREADS = 512;
+constexpr int SS_G = 8;                    // lanes per row
+constexpr int SS_GROUPS = SS_THREADS / SS_G;
+constexpr int SS_MAX_ROWS = kSmallSweepMaxN / SS_CTAS;          // rows per CTA
+constexpr int SS_MCAP = 4000;               // matrix entries (all terms) a CTA can keep in shared memory
+constexpr int SS_W_BYTES = 2 * kSmallSweepMaxN * (int)sizeof(cplx);
+constexpr int SS_SMEM = SS_W_BYTES + SS_MAX_ROWS * (int)sizeof(cplx) + SS_MCAP * (int)(sizeof(cplx) + sizeof(int32_t)) +
+                        3 * (SS_MAX_ROWS + 1) * (int)sizeof(int);
 
-// Sum of (a, b) over the block, result in EVERY thread.  Fixed tree.
-__device__ __forceinline__ void block_allreduce_sum2(double& a, double& b, double* sa, double* sb) {
+// Sum of (a, b) over the block, result in thread 0.  Fixed tree.
+__device__ __forceinline__ void block_reduce_sum2_ss(double& a, double& b, double* sa, double* sb) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
-    a += shfl_xor_d(a, o);
-    b += shfl_xor_d(b, o);
+    a += shfl_down_d(a, o);
+    b += shfl_down_d(b, o);
   }
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  __syncthreads();            // previous use of sa/sb is over
   if (lane == 0) {
     sa[warp] = a;
     sb[warp] = b;
   }
   __syncthreads();
-  a = sa[lane];               // SS_THREADS / 32 == 32 warps: one value per lane
-  b = sb[lane];
+  if (warp == 0) {
+    a = lane < SS_THREADS / 32 ? sa[lane] : 0.0;
+    b = lane < SS_THREADS / 32 ? sb[lane] : 0.0;
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    a += shfl_xor_d(a, o);
-    b += shfl_xor_d(b, o);
+    for (int o = 16; o > 0; o >>= 1) {
+      a += shfl_down_d(a, o);
+      b += shfl_down_d(b, o);
+    }
   }
 }
 
-__global__ void __launch_bounds__(SS_THREADS, 1)
-    csr_leja_sweep_small_kernel(CsrOp op, const cplx* v, cplx* w0, cplx* w1, cplx* out, double inv_gamma,
-                                double c_over_gamma, double tol, int m_max, cplx phase,
-                                const __grid_constant__ SweepTable tab, LejaStatus* status) {
-  static_assert(SS_THREADS == 1024, "the all-reduce assumes 32 warps");
-  __shared__ double sa[32], sb[32];
-  if (status->pad) return;                 // an earlier sub-step did not converge
-  const int tid = threadIdx.x;
+__global__ void __cluster_dims__(SS_CTAS, 1, 1) __launch_bounds__(SS_THREADS, 1)
+    csr_leja_sweep_small_kernel(CsrOp op, const cplx* v, cplx* out, double inv_gamma, double c_over_gamma, double tol,
+                                int m_max, cplx phase, const __grid_constant__ SweepTable tab, LejaStatus* status) {
+  extern __shared__ __align__(16) unsigned char ss_smem[];
+  __shared__ double sa[SS_THREADS / 32], sb[SS_THREADS / 32];
+  __shared__ double part[2][2];                     // [iteration parity](sw, sp) of this CTA, read by the others
+  cg::cluster_group cluster = cg::this_cluster();
+  const int rank = (int)cluster.block_rank();
+  if (status->pad) return;                          // an earlier sub-step did not converge (cluster-uniform)
+  cplx* wbuf[2] = {reinterpret_cast<cplx*>(ss_smem), reinterpret_cast<cplx*>(ss_smem) + kSmallSweepMaxN};
+  const int tid = threadIdx.x, grp = tid / SS_G, sub = tid % SS_G;
   const int n = (int)op.n;
-  cplx pr[SS_ROWS];
-  double s0 = 0.0, s1 = 0.0;
-#pragma unroll
-  for (int j = 0; j < SS_ROWS; ++j) {      // S5
-    const int row = tid + j * SS_THREADS;
-    pr[j] = make_double2(0.0, 0.0);
-    if (row < n) {
-      const cplx x = v[row];
-      w0[row] = x;
-      pr[j] = cmul(tab.d[0], x);
-      s0 += x.x * x.x + x.y * x.y;
+  const int per = (n + SS_CTAS - 1) / SS_CTAS;
+  const int r0 = min(n, rank * per), r1 = min(n, r0 + per);
+
+  // the CTA's slice of every term -> shared memory (values, columns, local row pointers)
+  cplx* prow = reinterpret_cast<cplx*>(ss_smem + SS_W_BYTES);    // p of the CTA's rows (kept out of registers so that
+  cplx* mval = prow + SS_MAX_ROWS;                               // the pass loop need not be unrolled: code size)
+  int32_t* mcol = reinterpret_cast<int32_t*>(mval + SS_MCAP);
+  int* mrp = reinterpret_cast<int*>(mcol + SS_MCAP);           // [term][SS_MAX_ROWS + 1], offsets into mval/mcol
+  int total = 0;
+  for (int t = 0; t < op.nterms; ++t) total += op.t[t].rp[r1] - op.t[t].rp[r0];
+  const bool cached = total <= SS_MCAP;                         // CTA-uniform
+  if (cached) {
+    int off = 0;
+    for (int t = 0; t < op.nterms; ++t) {
+      const CsrTerm& T = op.t[t];
+      const int b = T.rp[r0], len = T.rp[r1] - b;
+      for (int e = tid; e < len; e += SS_THREADS) {
+        mval[off + e] = T.v[b + e];
+        mcol[off + e] = T.ci[b + e];
+      }
+      for (int r = tid; r <= r1 - r0; r += SS_THREADS) mrp[t * (SS_MAX_ROWS + 1) + r] = off + T.rp[r0 + r] - b;
+      off += len;
     }
   }
-  block_allreduce_sum2(s0, s1, sa, sb);
+
+  // S5: every CTA copies the whole v (fixed-order norm, identical in all CTAs); p_0 for its own rows
+  double s0 = 0.0, s1 = 0.0;
+  for (int i = tid; i < n; i += SS_THREADS) {
+    const cplx x = v[i];
+    wbuf[0][i] = x;
+    s0 += x.x * x.x + x.y * x.y;
+  }
+  block_reduce_sum2_ss(s0, s1, sa, sb);
+  if (tid == 0) part[0][0] = s0;
+  __syncthreads();
+  s0 = part[0][0];
+  for (int r = r0 + tid; r < r1; r += SS_THREADS) prow[r - r0] = cmul(tab.d[0], wbuf[0][r]);
   double e_prev = hypot(tab.d[0].x, tab.d[0].y) * sqrt(s0);
   double err = 0.0, sw = 0.0, sp = 0.0;
-  cplx* w_in = w0;
-  cplx* w_out = w1;
-  int k = 0;
+  int k = 0, cur = 0;
   bool done = false;
+  cluster.sync();                                   // everybody's buffers exist before remote writes start
+
   while (!done && k < m_max) {
     ++k;
-    __syncthreads();                       // w_in complete (block-wide visibility of the global stores)
     const cplx dk = tab.d[k];
     const double shift = c_over_gamma + tab.l[k - 1];
-    sw = 0.0;
-    sp = 0.0;
-#pragma unroll
-    for (int j = 0; j < SS_ROWS; ++j) {    // S6
-      const int row = tid + j * SS_THREADS;
-      if (row < n) {
-        cplx y = make_double2(0.0, 0.0);
-        for (int t = 0; t < op.nterms; ++t) {
-          const CsrTerm& T = op.t[t];
-          cplx a = make_double2(0.0, 0.0);
-          const int qs = T.rp[row], qe = T.rp[row + 1];
-          // batches of SS_U entries: all column loads, then all value / w loads, then the FMAs in stored
-          // order -- two dependent memory latencies per batch instead of per entry
-          for (int q0 = qs; q0 < qe; q0 += SS_U) {
-            int c[SS_U];
-            cplx mv[SS_U], xv[SS_U];
-#pragma unroll
-            for (int u = 0; u < SS_U; ++u) c[u] = q0 + u < qe ? T.ci[q0 + u] : row;
-#pragma unroll
-            for (int u = 0; u < SS_U; ++u) {
-              mv[u] = q0 + u < qe ? T.v[q0 + u] : make_double2(0.0, 0.0);
-              xv[u] = w_in[c[u]];
-            }
-#pragma unroll
-            for (int u = 0; u < SS_U; ++u) cfma(a, mv[u], xv[u]);
+    const cplx* w_in = wbuf[cur];
+    double bw = 0.0, bp = 0.0;
+#pragma unroll 1
+    for (int j = 0; j * SS_GROUPS < per; ++j) {     // S6 on the CTA's row slice
+      const int row = r0 + grp + j * SS_GROUPS;
+      const bool valid = row < r1;
+      cplx y = make_double2(0.0, 0.0);
+      for (int t = 0; t < op.nterms; ++t) {
+        const CsrTerm& T = op.t[t];
+        cplx a = make_double2(0.0, 0.0);
+        if (valid) {
+          if (cached) {
+            const int* lrp = mrp + t * (SS_MAX_ROWS + 1) + (row - r0);
+            const int qe = lrp[1];
+            for (int q = lrp[0] + sub; q < qe; q += SS_G) cfma(a, mval[q], w_in[mcol[q]]);
+          } else {
+            const int qe = T.rp[row + 1];
+            for (int q = T.rp[row] + sub; q < qe; q += SS_G) cfma(a, T.v[q], w_in[T.ci[q]]);
           }
-          const cplx ca = cmul(T.coef, a);
-          y.x += ca.x;
-          y.y += ca.y;
         }
+        const cplx ca = cmul(T.coef, a);
+        y.x += ca.x;
+        y.y += ca.y;
+      }
+#pragma unroll
+      for (int o = SS_G / 2; o > 0; o >>= 1) {
+        y.x += shfl_xor_d(y.x, o);
+        y.y += shfl_xor_d(y.y, o);
+      }
+      if (valid && sub == 0) {
         const cplx wi = w_in[row];
         cplx wn;
         wn.x = inv_gamma * y.x - shift * wi.x;
         wn.y = inv_gamma * y.y - shift * wi.y;
-        w_out[row] = wn;
-        cfma(pr[j], dk, wn);
-        sw += wn.x * wn.x + wn.y * wn.y;
-        sp += pr[j].x * pr[j].x + pr[j].y * pr[j].y;
+        cplx pi = prow[row - r0];
+        cfma(pi, dk, wn);
+        prow[row - r0] = pi;
+        bw += wn.x * wn.x + wn.y * wn.y;
+        bp += pi.x * pi.x + pi.y * pi.y;
+        wbuf[cur ^ 1][row] = wn;                    // own slice, own copy; the other CTAs pull it after the barrier
       }
     }
-    block_allreduce_sum2(sw, sp, sa, sb);
+    block_reduce_sum2_ss(bw, bp, sa, sb);
+    if (tid == 0) {
+      part[k & 1][0] = bw;
+      part[k & 1][1] = bp;
+    }
+    cluster.sync();                                 // every CTA's slice of the new w and its partials are written
+    // pull the other CTAs' slices into the local copy through distributed shared memory (independent
+    // 16-byte loads, all in flight at once) and their partial norms
+    for (int i = tid; i < n; i += SS_THREADS) {
+      const int owner = i / per;
+      if (owner != rank) wbuf[cur ^ 1][i] = cluster.map_shared_rank(wbuf[cur ^ 1], owner)[i];
+    }
+    double pw[SS_CTAS], pp[SS_CTAS];
+#pragma unroll
+    for (int c = 0; c < SS_CTAS; ++c) {
+      const double* remote = cluster.map_shared_rank(&part[k & 1][0], c);
+      pw[c] = remote[0];
+      pp[c] = remote[1];
+    }
+    sw = 0.0;
+    sp = 0.0;
+#pragma unroll
+    for (int c = 0; c < SS_CTAS; ++c) {             // same order in every CTA: same decision
+      sw += pw[c];
+      sp += pp[c];
+    }
+    __syncthreads();                                // local copy of w complete before the next gathers
     const double e_k = hypot(dk.x, dk.y) * sqrt(sw);   // S7
     err = e_k + e_prev;
     e_prev = e_k;
     done = err <= tol * sqrt(sp);
-    cplx* tmp = w_in;
-    w_in = w_out;
-    w_out = tmp;
+    cur ^= 1;
   }
-  if (done) {
-#pragma unroll
-    for (int j = 0; j < SS_ROWS; ++j) {    // S8
-      const int row = tid + j * SS_THREADS;
-      if (row < n) out[row] = cmul(phase, pr[j]);
-    }
-  }
-  if (tid == 0) {
+  if (done)
+    for (int r = r0 + tid; r < r1; r += SS_THREADS) out[r] = cmul(phase, prow[r - r0]);   // S8
+  if (rank == 0 && tid == 0) {
     status->done = done ? 1 : 0;
     status->pad = done ? 0 : 1;
     status->k = k;
@@ -144,16 +209,25 @@ __global__ void __launch_bounds__(SS_THREADS, 1)
     status->norm_w2 = sw;
     status->norm_p2 = sp;
   }
+  cluster.sync();                                   // no CTA leaves while its shared memory may still be written
 }
 
 }  // namespace
 
-void launch_csr_leja_sweep_small(const CsrOp& op, const cplx* v, cplx* out, double inv_gamma, double c_over_gamma,
-                                 double tol, int m_max, cplx phase, const SweepTable& tab, Workspace* ws,
-                                 cudaStream_t st) {
-  csr_leja_sweep_small_kernel<<<1, SS_THREADS, 0, st>>>(op, v, ws->w[0], ws->w[1], out, inv_gamma, c_over_gamma, tol,
-                                                        m_max, phase, tab, ws->status);
+int launch_csr_leja_sweep_small(const CsrOp& op, const cplx* v, cplx* out, double inv_gamma, double c_over_gamma,
+                                double tol, int m_max, cplx phase, const SweepTable& tab, Workspace* ws,
+                                cudaStream_t st) {
+  static bool configured = false;
+  if (!configured) {
+    if (cudaFuncSetAttribute(csr_leja_sweep_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SS_SMEM) !=
+        cudaSuccess)
+      return MAGNUS_ECUDA;
+    configured = true;
+  }
+  csr_leja_sweep_small_kernel<<<SS_CTAS, SS_THREADS, SS_SMEM, st>>>(op, v, out, inv_gamma, c_over_gamma, tol, m_max,
+                                                                    phase, tab, ws->status);
   ws->launches += 1;
+  return cudaGetLastError() == cudaSuccess ? MAGNUS_OK : MAGNUS_ECUDA;
 }
 
 }  // namespace magnus

@@ -65,7 +65,7 @@ struct LejaStatus {
   double norm_p2;    // sum |p_k|^2
 };
 
-// Small CSR problems run a whole Leja sweep in one single-CTA launch (kernels_csr_small.cu).
+// Small CSR problems run a whole Leja sweep in one launch of an 8-CTA cluster (kernels_csr_small.cu).
 const int kSmallSweepMaxN = 4096;
 struct SweepTable {
   cplx d[kMaxDegree + 1];     // divided differences d_k (c3)
@@ -127,7 +127,7 @@ int csr_hermitian_check(const magnus_matrix* A, cudaStream_t st, double* max_vio
 // ---- kernels_csr_small.cu ---------------------------------------------------
 // one sub-step sweep (S5-S8) in one launch; on success status->done = 1, status->k = iterations and out is
 // written; if tab's m_max iterations do not meet tol, status->pad = 1 and out is left untouched
-void launch_csr_leja_sweep_small(const CsrOp& op, const cplx* v, cplx* out, double inv_gamma, double c_over_gamma,
+int launch_csr_leja_sweep_small(const CsrOp& op, const cplx* v, cplx* out, double inv_gamma, double c_over_gamma,
                                  double tol, int m_max, cplx phase, const SweepTable& tab, Workspace* ws,
                                  cudaStream_t st);
 
