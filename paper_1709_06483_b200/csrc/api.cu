@@ -282,6 +282,7 @@ struct magnus_context {
   cplx* gs_diag[3] = {nullptr, nullptr, nullptr};
   bool gs_disjoint2 = false;   // H0, H1 share no (row, column)
   bool gs_disjoint3 = false;   // H0, H1, C share none either
+  int unit_cap2 = 0, unit_cap3 = 0;   // stream kernel: largest 32-row unit of (H0, H1) and of (H0, H1, C)
   cudaEvent_t ev_comm[2] = {nullptr, nullptr};
   double comm_ms = 0.0;
   bool time_comm = false;
@@ -317,6 +318,7 @@ static int csr_cache_rowstats(magnus_context* h) {
   }
   CsrOp op;
   op.n = n;
+  op.unit_cap = 0;
   for (int t = 0; t < 3; ++t) op.t[t] = T[t < nterms ? t : 0];
   op.nterms = 2;
   launch_csr_overlap(op, flags, h->stream);
@@ -331,6 +333,12 @@ static int csr_cache_rowstats(magnus_context* h) {
   if (e != cudaSuccess || cudaGetLastError() != cudaSuccess) { set_error("row-statistics kernels failed"); return MAGNUS_ECUDA; }
   h->gs_disjoint2 = hf[0] == 0;
   h->gs_disjoint3 = nterms == 3 && hf[1] == 0;
+  {
+    op.nterms = 2;
+    if (csr_unit_cap(op, h->stream, &h->unit_cap2) != MAGNUS_OK) h->unit_cap2 = 0;
+    op.nterms = 3;
+    if (nterms == 3 && csr_unit_cap(op, h->stream, &h->unit_cap3) != MAGNUS_OK) h->unit_cap3 = 0;
+  }
   return MAGNUS_OK;
 }
 
@@ -512,6 +520,7 @@ int magnus_step(magnus_handle h, double t, double tau, void* psi_, magnus_step_i
         op.csr.t[1] = csr_term(&h->H1, coef[e], 0.0);
         op.csr.t[2] = op.csr.t[1];
       }
+      op.csr.unit_cap = op.csr.nterms == 3 ? h->unit_cap3 : h->unit_cap2;
       if ((op.csr.nterms == 2 && h->gs_disjoint2) || (op.csr.nterms == 3 && h->gs_disjoint3)) {     // S3
         const int nblk = launch_csr_gershgorin_cached(op.csr, h->gs_r, h->gs_diag, ws, st);
         rc = read_interval(nblk, ws, st, &a, &b);
@@ -609,6 +618,8 @@ int leja_expmv(const magnus_matrix* H, const void* v_in, void* v_out, double h, 
     op.csr.nterms = 1;
     op.csr.t[0] = csr_term(H, 1.0, 0.0);
     op.csr.t[1] = op.csr.t[2] = op.csr.t[0];
+    op.csr.unit_cap = 0;
+    if (csr_unit_cap(op.csr, st, &op.csr.unit_cap) != MAGNUS_OK) op.csr.unit_cap = 0;
   } else {
     op.dense = true;
     op.dns.n = H->n;
@@ -703,6 +714,8 @@ static int build_op(const magnus_matrix* H0, const magnus_matrix* H1, double g, 
     op->csr.t[0] = csr_term(H0, 1.0, 0.0);
     op->csr.t[1] = H1 ? csr_term(H1, g, 0.0) : op->csr.t[0];
     op->csr.t[2] = op->csr.t[0];
+    op->csr.unit_cap = 0;
+    if (csr_unit_cap(op->csr, st, &op->csr.unit_cap) != MAGNUS_OK) op->csr.unit_cap = 0;
   } else {
     op->dense = true;
     op->dns.n = H0->n;
@@ -774,8 +787,11 @@ int magnus_leja_iteration(const magnus_matrix* H0, const magnus_matrix* H1, doub
       launch_iter(op, (const cplx*)w_in, (cplx*)w_out, (cplx*)p, inv_gamma, shift, make_double2(d_re, d_im), 1.0, 0.0, &ws, st);
     cudaEventRecord(ws.ev[1], st);
     cudaMemcpyAsync(ws.status_host, ws.status, sizeof(LejaStatus), cudaMemcpyDeviceToHost, st);
-    if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) {
-      set_error("magnus_leja_iteration: kernel failed");
+    cudaError_t ke = cudaStreamSynchronize(st);
+    if (ke == cudaSuccess) ke = cudaGetLastError();
+    if (ke != cudaSuccess) {
+      set_error("magnus_leja_iteration: kernel failed: %s", cudaGetErrorString(ke));
+      cudaGetLastError();
       rc = MAGNUS_ECUDA;
     } else {
       float ms = 0.f;

@@ -61,6 +61,21 @@ __device__ __forceinline__ void ld_stream256(const cplx* p, cplx& a, cplx& b) {
                : "=d"(a.x), "=d"(a.y), "=d"(b.x), "=d"(b.y)
                : "l"(p));
 }
+// 128-bit load / store carrying an L2 cache-policy descriptor (createpolicy), coherent path.
+__device__ __forceinline__ cplx ld_hint(const cplx* p, uint64_t pol) {
+  cplx r;
+  asm volatile("ld.global.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(r.x), "=d"(r.y) : "l"(p), "l"(pol) : "memory");
+  return r;
+}
+__device__ __forceinline__ void st_hint(cplx* p, cplx v, uint64_t pol) {
+  asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;" ::"l"(p), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
+}
+// gather load that does not allocate an L1 line (read-only path)
+__device__ __forceinline__ cplx ld_gather_na(const cplx* p) {
+  cplx r;
+  asm volatile("ld.global.nc.L1::no_allocate.v2.f64 {%0, %1}, [%2];" : "=d"(r.x), "=d"(r.y) : "l"(p));
+  return r;
+}
 // Streaming store (written once, re-read only by the next launch).
 __device__ __forceinline__ void st_stream(cplx* p, cplx v) {
   asm volatile("st.global.cs.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(v.x), "d"(v.y) : "memory");

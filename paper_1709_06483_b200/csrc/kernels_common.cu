@@ -37,10 +37,22 @@ __global__ void __launch_bounds__(256) scale_copy_kernel(const cplx* __restrict_
     out[i] = cmul(phase, in[i]);
 }
 
+int device_sm_count() {
+  static int cached[64] = {0};
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 148;
+  if (cached[dev] == 0) {
+    int v = 0;
+    if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || v <= 0) v = 148;
+    cached[dev] = v;
+  }
+  return cached[dev];
+}
+
 static int vec_grid(int64_t n) {
   int64_t g = (n + 256 * 4 - 1) / (256 * 4);
   if (g < 1) g = 1;
-  if (g > 148 * 8) g = 148 * 8;
+  if (g > (int64_t)device_sm_count() * 8) g = (int64_t)device_sm_count() * 8;
   return (int)g;
 }
 
@@ -79,6 +91,7 @@ int workspace_alloc(Workspace* ws, int64_t n) {
 }
 
 void workspace_free(Workspace* ws) {
+  stream_maps_free(ws);
   cudaFree(ws->w[0]);
   cudaFree(ws->w[1]);
   cudaFree(ws->p);

@@ -157,17 +157,15 @@ __global__ void __launch_bounds__(GS_WARPS * 32, 1) csr_gershgorin_staged_kernel
 
 int launch_csr_gershgorin(const CsrOp& op, Workspace* ws, cudaStream_t st) {
   if (op.n >= 32768) {
-    static bool configured = false;
-    if (!configured) {
-      cudaFuncSetAttribute(csr_gershgorin_staged_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GS_SMEM);
-      configured = true;
-    }
-    csr_gershgorin_staged_kernel<<<148, GS_WARPS * 32, GS_SMEM, st>>>(op, ws->gersh, ws->tickets + 1);
+    // per launch (cheap): the attribute is per device, a process-wide flag would miss a second GPU
+    cudaFuncSetAttribute(csr_gershgorin_staged_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GS_SMEM);
+    const int sms = device_sm_count();
+    csr_gershgorin_staged_kernel<<<sms, GS_WARPS * 32, GS_SMEM, st>>>(op, ws->gersh, ws->tickets + 1);
     ws->launches += 1;
-    return 148;
+    return sms;
   }
   int64_t g = (op.n + 255) / 256;
-  if (g > 148 * 8) g = 148 * 8;
+  if (g > (int64_t)device_sm_count() * 8) g = (int64_t)device_sm_count() * 8;
   csr_gershgorin_kernel<<<(int)g, 256, 0, st>>>(op, ws->gersh, ws->tickets + 1);
   ws->launches += 1;
   return (int)g;
@@ -261,7 +259,7 @@ __global__ void __launch_bounds__(256) csr_gershgorin_cached_kernel(RowStats S, 
 
 static int row_grid256(int64_t n) {
   int64_t g = (n + 255) / 256;
-  if (g > 148 * 8) g = 148 * 8;
+  if (g > (int64_t)device_sm_count() * 8) g = (int64_t)device_sm_count() * 8;
   return (int)g;
 }
 
@@ -366,7 +364,7 @@ static int launch_generic(const CsrOp& op, const cplx* w_in, cplx* w_out, cplx* 
                           cplx dk, double abs_dk, double tol, Workspace* ws, cudaStream_t st) {
   constexpr int ROWS = 256 / G;
   int64_t g = (op.n + ROWS - 1) / ROWS;
-  if (g > 148 * 8) g = 148 * 8;
+  if (g > (int64_t)device_sm_count() * 8) g = (int64_t)device_sm_count() * 8;
   csr_leja_iter_generic<G><<<(int)g, 256, 0, st>>>(op, w_in, w_out, p, inv_gamma, shift, dk, abs_dk, tol,
                                                     ws->status, ws->partials, ws->tickets);
   ws->launches += 1;
@@ -379,7 +377,15 @@ bool csr_rowblock_supported(const CsrOp& op);
 
 int launch_csr_leja_iter(const CsrOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma, double shift,
                          cplx dk, double abs_dk, double tol, Workspace* ws, cudaStream_t st) {
-  if (ws->csr_kernel == 2 || (ws->csr_kernel == 0 && csr_rowblock_supported(op)))
+  if (ws->csr_kernel == 4 && csr_rowtma_supported(op)) {
+    const int g = launch_csr_leja_iter_rowtma(op, w_in, w_out, p, inv_gamma, shift, dk, abs_dk, tol, ws, st);
+    if (g > 0) return g;
+  }
+  if ((ws->csr_kernel == 3 || (ws->csr_kernel >= 20000 && ws->csr_kernel < 30000)) && csr_stream_supported(op)) {
+    const int g = launch_csr_leja_iter_stream(op, w_in, w_out, p, inv_gamma, shift, dk, abs_dk, tol, ws, st);
+    if (g > 0) return g;
+  }
+  if (ws->csr_kernel == 2 || ws->csr_kernel >= 1000 || (ws->csr_kernel == 0 && csr_rowblock_supported(op)))
     return launch_csr_leja_iter_rowblock(op, w_in, w_out, p, inv_gamma, shift, dk, abs_dk, tol, ws, st);
   // lanes per row from the mean stored entries per row and term
   double mean = 0.0;
@@ -535,7 +541,8 @@ int csr_commutator_build(const CsrRaw& A, const CsrRaw& B, int64_t n, int32_t** 
       cudaMalloc(&overflow, sizeof(int)) != cudaSuccess) {
     rc = MAGNUS_ENOMEM;
   }
-  int grid = (int)(n < 148 * 16 ? n : 148 * 16);
+  const int64_t gmax = (int64_t)device_sm_count() * 16;
+  int grid = (int)(n < gmax ? n : gmax);
   int h_over = 0;
   int32_t h_nnz = 0;
   if (rc == MAGNUS_OK) {

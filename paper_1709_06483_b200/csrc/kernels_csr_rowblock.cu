@@ -34,6 +34,12 @@ constexpr int RB_BYTES_PER_WARP = RB_SLOTS * (int)(sizeof(cplx) + sizeof(int32_t
 constexpr int RB_SMEM = RB_WARPS * RB_BYTES_PER_WARP;
 constexpr int RB_UNROLL = 8;
 
+// POL  1: p and w+ move with an L2 evict-first hint (they are streamed once per launch and never gathered), so
+//         that of all the traffic only w competes for L2 residency (n large: w itself exceeds L2)
+// TB    the 32-row blocks are visited in an order that interleaves 2^TB contiguous chunks of the row range:
+//         partners of a row under a flip of one of the top TB index bits are then in flight at the same time
+// PIPE  1: the gathers of the next batch of RB_UNROLL entries are issued before the FMAs of the current one
+template <int POL, int TB, int PIPE>
 __global__ void __launch_bounds__(RB_WARPS * 32, 3)
     csr_leja_iter_rowblock_kernel(CsrOp op, const cplx* __restrict__ w_in, cplx* __restrict__ w_out,
                                   cplx* __restrict__ p, double inv_gamma, double shift, cplx dk,
@@ -47,10 +53,14 @@ __global__ void __launch_bounds__(RB_WARPS * 32, 3)
   const uint64_t pol = policy_evict_first();
   const int64_t n = op.n;
   const int64_t nblocks = (n + 31) >> 5;
+  const int64_t chunk = (nblocks + (1 << TB) - 1) >> TB;      // blocks per interleaved chunk
+  const int64_t nslots = chunk << TB;
   const int64_t total_warps = (int64_t)gridDim.x * RB_WARPS;
   double sw = 0.0, sp = 0.0;
 
-  for (int64_t blk = (int64_t)blockIdx.x * RB_WARPS + warp; blk < nblocks; blk += total_warps) {
+  for (int64_t slot = (int64_t)blockIdx.x * RB_WARPS + warp; slot < nslots; slot += total_warps) {
+    const int64_t blk = TB == 0 ? slot : (slot & ((1 << TB) - 1)) * chunk + (slot >> TB);
+    if (blk >= nblocks) continue;
     const int64_t row = (blk << 5) + lane;
     const bool valid = row < n;
     cplx y = make_double2(0.0, 0.0);
@@ -68,7 +78,7 @@ __global__ void __launch_bounds__(RB_WARPS * 32, 3)
     cplx wi = make_double2(0.0, 0.0), pi = make_double2(0.0, 0.0);
     if (valid) {
       wi = w_in[row];
-      pi = p[row];
+      pi = POL ? ld_hint(p + row, pol) : p[row];
     }
 #pragma unroll
     for (int t = 0; t < 3; ++t) {
@@ -113,18 +123,53 @@ __global__ void __launch_bounds__(RB_WARPS * 32, 3)
         const int qs = rs - base;
         const int mylen = mine ? re - rs : 0;
         const int maxlen = __reduce_max_sync(0xffffffffu, mylen);
-        for (int j = 0; j < maxlen; j += RB_UNROLL) {
-          cplx xv[RB_UNROLL], mv[RB_UNROLL];
+        const int64_t safe = valid ? row : 0;
+        if (PIPE) {
+          // two batches in flight: gathers of batch b+1 are requested before batch b is consumed
+          cplx xa[RB_UNROLL], xb[RB_UNROLL];
 #pragma unroll
           for (int u = 0; u < RB_UNROLL; ++u) {
-            const bool ok = j + u < mylen;
-            const int s = ok ? rb_slot(qs + j + u) : 0;
-            mv[u] = ok ? sv[s] : make_double2(0.0, 0.0);
-            const int64_t c = ok ? (int64_t)sc[s] : (valid ? row : 0);
-            xv[u] = w_in[c];
+            const bool ok = u < mylen;
+            xa[u] = w_in[ok ? (int64_t)sc[rb_slot(qs + u)] : safe];
           }
+          for (int j = 0; j < maxlen; j += 2 * RB_UNROLL) {
 #pragma unroll
-          for (int u = 0; u < RB_UNROLL; ++u) cfma(a, mv[u], xv[u]);
+            for (int u = 0; u < RB_UNROLL; ++u) {
+              const bool ok = j + RB_UNROLL + u < mylen;
+              xb[u] = w_in[ok ? (int64_t)sc[rb_slot(qs + j + RB_UNROLL + u)] : safe];
+            }
+#pragma unroll
+            for (int u = 0; u < RB_UNROLL; ++u) {
+              const bool ok = j + u < mylen;
+              const cplx m = ok ? sv[rb_slot(qs + j + u)] : make_double2(0.0, 0.0);
+              cfma(a, m, xa[u]);
+            }
+#pragma unroll
+            for (int u = 0; u < RB_UNROLL; ++u) {
+              const bool ok = j + 2 * RB_UNROLL + u < mylen;
+              xa[u] = w_in[ok ? (int64_t)sc[rb_slot(qs + j + 2 * RB_UNROLL + u)] : safe];
+            }
+#pragma unroll
+            for (int u = 0; u < RB_UNROLL; ++u) {
+              const bool ok = j + RB_UNROLL + u < mylen;
+              const cplx m = ok ? sv[rb_slot(qs + j + RB_UNROLL + u)] : make_double2(0.0, 0.0);
+              cfma(a, m, xb[u]);
+            }
+          }
+        } else {
+          for (int j = 0; j < maxlen; j += RB_UNROLL) {
+            cplx xv[RB_UNROLL], mv[RB_UNROLL];
+#pragma unroll
+            for (int u = 0; u < RB_UNROLL; ++u) {
+              const bool ok = j + u < mylen;
+              const int s = ok ? rb_slot(qs + j + u) : 0;
+              mv[u] = ok ? sv[s] : make_double2(0.0, 0.0);
+              const int64_t c = ok ? (int64_t)sc[s] : safe;
+              xv[u] = w_in[c];
+            }
+#pragma unroll
+            for (int u = 0; u < RB_UNROLL; ++u) cfma(a, mv[u], xv[u]);
+          }
         }
         __syncwarp();   // everyone done reading before the buffer is refilled
         first = last;
@@ -137,9 +182,14 @@ __global__ void __launch_bounds__(RB_WARPS * 32, 3)
       cplx wn;
       wn.x = inv_gamma * y.x - shift * wi.x;
       wn.y = inv_gamma * y.y - shift * wi.y;
-      w_out[row] = wn;
       cfma(pi, dk, wn);
-      p[row] = pi;
+      if (POL) {
+        st_hint(w_out + row, wn, pol);
+        st_hint(p + row, pi, pol);
+      } else {
+        w_out[row] = wn;
+        p[row] = pi;
+      }
       sw += wn.x * wn.x + wn.y * wn.y;
       sp += pi.x * pi.x + pi.y * pi.y;
     }
@@ -152,24 +202,42 @@ __global__ void __launch_bounds__(RB_WARPS * 32, 3)
   if (last_block_ticket(ticket)) leja_finalize_warp0(partials, gridDim.x, abs_dk, tol, false, status);   // S7
 }
 
+template <int POL, int TB, int PIPE>
+int launch_variant(const CsrOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma, double shift, cplx dk,
+                   double abs_dk, double tol, Workspace* ws, cudaStream_t st) {
+  auto kern = csr_leja_iter_rowblock_kernel<POL, TB, PIPE>;
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, RB_SMEM) != cudaSuccess) return -1;
+  const int64_t nblocks = (op.n + 31) >> 5;
+  int64_t g = (nblocks + RB_WARPS - 1) / RB_WARPS;
+  const int64_t cap = (int64_t)device_sm_count() * 3;
+  if (g > cap) g = cap;
+  kern<<<(int)g, RB_WARPS * 32, RB_SMEM, st>>>(op, w_in, w_out, p, inv_gamma, shift, dk, abs_dk, tol, ws->status,
+                                               ws->partials, ws->tickets);
+  ws->launches += 1;
+  return (int)g;
+}
+
 }  // namespace
 
 bool csr_rowblock_supported(const CsrOp& op) { return op.n >= 32768; }
 
 int launch_csr_leja_iter_rowblock(const CsrOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma,
                                   double shift, cplx dk, double abs_dk, double tol, Workspace* ws, cudaStream_t st) {
-  static bool configured = false;
-  if (!configured) {
-    cudaFuncSetAttribute(csr_leja_iter_rowblock_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, RB_SMEM);
-    configured = true;
+#define RB_ARGS op, w_in, w_out, p, inv_gamma, shift, dk, abs_dk, tol, ws, st
+  switch (ws->csr_kernel) {   // experimental variants (round-2 sweep): 1000 + 100 POL + 10 TB + PIPE
+    case 1001: return launch_variant<0, 0, 1>(RB_ARGS);
+    case 1100: return launch_variant<1, 0, 0>(RB_ARGS);
+    case 1101: return launch_variant<1, 0, 1>(RB_ARGS);
+    case 1020: return launch_variant<0, 2, 0>(RB_ARGS);
+    case 1120: return launch_variant<1, 2, 0>(RB_ARGS);
+    case 1130: return launch_variant<1, 3, 0>(RB_ARGS);
+    case 1140: return launch_variant<1, 4, 0>(RB_ARGS);
+    case 1121: return launch_variant<1, 2, 1>(RB_ARGS);
+    case 1131: return launch_variant<1, 3, 1>(RB_ARGS);
+    case 1141: return launch_variant<1, 4, 1>(RB_ARGS);
+    default: return launch_variant<0, 0, 0>(RB_ARGS);
   }
-  const int64_t nblocks = (op.n + 31) >> 5;
-  int64_t g = (nblocks + RB_WARPS - 1) / RB_WARPS;
-  if (g > 148 * 3) g = 148 * 3;
-  csr_leja_iter_rowblock_kernel<<<(int)g, RB_WARPS * 32, RB_SMEM, st>>>(
-      op, w_in, w_out, p, inv_gamma, shift, dk, abs_dk, tol, ws->status, ws->partials, ws->tickets);
-  ws->launches += 1;
-  return (int)g;
+#undef RB_ARGS
 }
 
 }  // namespace magnus

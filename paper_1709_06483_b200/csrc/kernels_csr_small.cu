@@ -217,13 +217,10 @@ __global__ void __cluster_dims__(SS_CTAS, 1, 1) __launch_bounds__(SS_THREADS, 1)
 int launch_csr_leja_sweep_small(const CsrOp& op, const cplx* v, cplx* out, double inv_gamma, double c_over_gamma,
                                 double tol, int m_max, cplx phase, const SweepTable& tab, Workspace* ws,
                                 cudaStream_t st) {
-  static bool configured = false;
-  if (!configured) {
-    if (cudaFuncSetAttribute(csr_leja_sweep_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SS_SMEM) !=
-        cudaSuccess)
-      return MAGNUS_ECUDA;
-    configured = true;
-  }
+  // per launch (cheap): the attribute is per device, a process-wide flag would miss a second GPU
+  if (cudaFuncSetAttribute(csr_leja_sweep_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SS_SMEM) !=
+      cudaSuccess)
+    return MAGNUS_ECUDA;
   csr_leja_sweep_small_kernel<<<SS_CTAS, SS_THREADS, SS_SMEM, st>>>(op, v, out, inv_gamma, c_over_gamma, tol, m_max,
                                                                     phase, tab, ws->status);
   ws->launches += 1;

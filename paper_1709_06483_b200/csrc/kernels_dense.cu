@@ -259,7 +259,7 @@ int launch_dense_assemble(int64_t n, const cplx* A, int64_t lda, const cplx* B, 
 void launch_dense_assemble2(int64_t n, const cplx* H0, int64_t ld0, const cplx* H1, int64_t ld1, double f1, double f2,
                             cplx* A1, cplx* A2, Workspace* ws, cudaStream_t st) {
   int64_t g = (n * n + 255) / 256;
-  if (g > 148 * 16) g = 148 * 16;
+  if (g > (int64_t)device_sm_count() * 16) g = (int64_t)device_sm_count() * 16;
   dense_assemble2_kernel<<<(int)g, 256, 0, st>>>(n, H0, ld0, H1, ld1, f1, f2, A1, A2);
   ws->launches += 1;
 }

@@ -42,6 +42,7 @@ struct CsrTerm {
 struct CsrOp {
   int64_t n;
   int nterms;
+  int unit_cap;   // max over 32-row units and terms of one term's stored entries in one unit (0 = unknown): stream kernel
   CsrTerm t[3];
 };
 
@@ -89,7 +90,11 @@ struct Workspace {
   int64_t launches = 0;
   double leja_ms = 0.0;
   bool time_leja = false;
+  void* stream_maps = nullptr;       // stream kernel: cached TMA tensor maps of the operator's terms (host)
 };
+
+// cudaDevAttrMultiProcessorCount of the current device (cached per device; 148 on B200)
+int device_sm_count();
 
 int workspace_alloc(Workspace* ws, int64_t n);
 void workspace_free(Workspace* ws);
@@ -123,6 +128,18 @@ int csr_commutator(const magnus_matrix* A, const magnus_matrix* B, int64_t cap, 
 int csr_commutator_owned(const magnus_matrix* A, const magnus_matrix* B, int32_t** rp, int32_t** ci, cplx** v,
                          int64_t* nnz, cudaStream_t st);
 int csr_hermitian_check(const magnus_matrix* A, cudaStream_t st, double* max_violation);
+
+// ---- kernels_csr_stream.cu --------------------------------------------------
+// warp-specialised kernel for large n: bulk-copy (TMA) ring + mbarriers, see the file header
+int csr_unit_cap(const CsrOp& op, cudaStream_t st, int* cap_out);      // synchronises the stream
+bool csr_stream_supported(const CsrOp& op);
+void stream_maps_free(Workspace* ws);
+// row-block structure (a private buffer per warp) with TMA staging
+bool csr_rowtma_supported(const CsrOp& op);
+int launch_csr_leja_iter_rowtma(const CsrOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma,
+                                double shift, cplx dk, double abs_dk, double tol, Workspace* ws, cudaStream_t st);
+int launch_csr_leja_iter_stream(const CsrOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma,
+                                double shift, cplx dk, double abs_dk, double tol, Workspace* ws, cudaStream_t st);
 
 // ---- kernels_csr_small.cu ---------------------------------------------------
 // one sub-step sweep (S5-S8) in one launch; on success status->done = 1, status->k = iterations and out is

@@ -184,13 +184,9 @@ __global__ void __launch_bounds__(256) dfma_peak_kernel(int iters, double* __res
 
 int launch_zgemm(int64_t n, const cplx* A, int64_t lda, const cplx* B, int64_t ldb, cplx* C, int64_t ldc,
                  cudaStream_t st) {
-  static bool configured = false;
-  if (!configured) {
-    if (cudaFuncSetAttribute(zgemm_dmma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ZGEMM_SMEM) !=
-        cudaSuccess)
-      return MAGNUS_ECUDA;
-    configured = true;
-  }
+  // per launch (cheap): the attribute is per device, a process-wide flag would miss a second GPU
+  if (cudaFuncSetAttribute(zgemm_dmma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ZGEMM_SMEM) != cudaSuccess)
+    return MAGNUS_ECUDA;
   const int tiles_m = (int)((n + BM - 1) / BM), tiles_n = (int)((n + BN - 1) / BN);
   zgemm_dmma_kernel<<<tiles_m * tiles_n, 256, ZGEMM_SMEM, st>>>(n, A, lda, B, ldb, C, ldc, tiles_m, tiles_n);
   return cudaGetLastError() == cudaSuccess ? MAGNUS_OK : MAGNUS_ECUDA;
@@ -202,7 +198,7 @@ int fp64_peaks(double* dmma_tflops, double* dfma_tflops, cudaStream_t st) {
   cudaEvent_t e0, e1;
   cudaEventCreate(&e0);
   cudaEventCreate(&e1);
-  const int blocks = 148 * 8, iters = 4096;
+  const int blocks = device_sm_count() * 8, iters = 4096;
   float ms = 0.f;
   double best_mma = 0.0, best_fma = 0.0;
   for (int rep = 0; rep < 4; ++rep) {

@@ -126,7 +126,7 @@ def expected_iteration(oracle, Mh, w, p, inv_gamma, shift, d):
     return wn, pn
 
 
-@pytest.mark.parametrize("N,kernel", [(8, 1), (12, 1), (12, 2), (15, 2), (16, 0)])
+@pytest.mark.parametrize("N,kernel", [(8, 1), (12, 1), (12, 2), (15, 2), (16, 0), (8, 3), (12, 3), (16, 3), (16, 24001), (16, 27081), (16, 22040), (8, 4), (12, 4), (16, 4)])
 def test_fused_iteration_csr_xxz(M, oracle, N, kernel):
     n = 1 << N
     H0, H1 = xxz.xxz_h0(N), xxz.xxz_h1(N)
@@ -146,11 +146,13 @@ def test_fused_iteration_csr_xxz(M, oracle, N, kernel):
     assert math.isclose(sp, np.sum(np.abs(pn) ** 2), rel_tol=1e-12)
 
 
-@pytest.mark.parametrize("kernel", [1, 2])
-def test_fused_iteration_csr_general_ragged(M, oracle, kernel):
-    """Non-power-of-two n, empty rows, one row longer than the row-block staging buffer."""
+@pytest.mark.parametrize("kernel,long_len", [(1, 1900), (2, 1900), (3, 1900), (3, 2990), (27001, 2990), (22030, 700), (23000, 40), (4, 1900), (4, 40)])
+def test_fused_iteration_csr_general_ragged(M, oracle, kernel, long_len):
+    """Non-power-of-two n, empty rows, one row longer than the row-block staging buffer / than a ring stage of
+    the stream kernel (kernel 3 and its 2000+ variants: that unit is read straight from global memory), rows
+    longer than 32 entries, an index array whose length is not a multiple of four (unaligned tail unit)."""
     n = 3001
-    S = random_sparse_hermitian(n, 0.004, 5, long_row=(17, 1900))
+    S = random_sparse_hermitian(n, 0.004, 5, long_row=(17, long_len))
     Mh = oracle.CsrHost(n, S.indptr.astype(np.int32), S.indices.astype(np.int32), S.data.astype(complex))
     w, p = rand_vec(n, 3), rand_vec(n, 4)
     inv_gamma, shift, d = 0.05, 0.7, -0.11 + 0.4j

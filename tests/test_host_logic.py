@@ -14,6 +14,8 @@ import mpmath
 import numpy as np
 import pytest
 
+import leja_check
+
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
@@ -73,6 +75,8 @@ def test_leja_points_defining_property(M):
         if k <= 32:
             logp = np.sum(np.log(np.abs(grid[:, None] - prev[None, :]) + 1e-300), axis=1)
             assert np.sum(np.log(np.abs(l[k] - prev))) >= logp.max() - 1e-9, k
+    # all k <= 128: the winning gap and its maximiser, by a route independent of the library's Newton iteration
+    assert leja_check.check_sequence(l) > 1e-4
 
 
 def test_leja_points_agree_with_oracle(M, oracle):

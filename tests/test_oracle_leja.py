@@ -12,6 +12,7 @@ import mpmath
 import numpy as np
 import pytest
 
+import leja_check
 import workloads as W
 from workloads import xxz
 
@@ -53,6 +54,21 @@ def test_leja_points_closed_form_and_extremal_property(oracle):
             logp = np.sum(np.log(np.abs(grid[:, None] - prev[None, :]) + 1e-300), axis=1)
             mine = np.sum(np.log(np.abs(l[k] - prev)))
             assert mine >= logp.max() - 1e-9, k
+    # every k up to m_max = 128: l_k is the maximiser of the WINNING gap (per-gap golden section + 40-digit polish,
+    # tests/leja_check.py -- a route independent of the oracle's bisection), and no other gap comes within 1e-7
+    # in log: a wrong gap choice anywhere in the sequence fails here
+    worst = leja_check.check_sequence(l)
+    assert worst > 1e-4
+
+
+def test_leja_check_rejects_a_wrong_gap(oracle):
+    """Negative control for the pin above: the runner-up gap's stationary point is refused."""
+    l = oracle.leja_points(60).copy()
+    x, fx = leja_check.gap_maxima(l[:50])
+    order = np.argsort(fx)
+    l[50] = x[order[-2]]          # stationary, interior, distinct -- but not the global maximum
+    with pytest.raises(AssertionError):
+        leja_check.check_sequence(l[:51], first=50)
 
 
 # ------------------------------------------------------------------ c-P1
