@@ -16,7 +16,10 @@ flush is needed between timed steps).  Rank 0 prints ONE JSON line.
   roofline   fused Leja iteration kernel (dense: the GEMV variant; with --scheme m4 on dense H the
              DMMA commutator): algorithmic bytes (flops) per launch / mean launch time measured
              live with CUDA events inside the timed region, against MEASURED_PEAKS.json
-  cpu_baseline  the oracle (oracle/, test infrastructure) timed on this box's host cores on a bounded sample
+  cpu_baseline  the oracle (oracle/, test infrastructure) timed on this box's host cores on a bounded sample:
+             ONE Magnus step of the SAME workload at full size (N = 24 for cfg5; about 45 s)
+  extra      (default run only) two short secondary measurements so that the record carries all three parts of
+             the metric: cfg4 CF4 (dense GEMV GB/s) and cfg4 M4 (DMMA commutator TFLOP/s)
 
 Multi-GPU: the path does not shard ("replicas only"); --gpus N runs N
 independent replicas, one process per GPU, no data-path collective, scaling "weak".
@@ -42,6 +45,11 @@ UNIT = "steps/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` captures (profiles/r1_csr_rowblock_ncu.md, profiles/r1_dense_gemv_ncu.md); None = not captured.
 NCU_TRAFFIC_BYTES = {("cfg5", "cf4"): 15.093e9, ("cfg4", "cf4"): 4.299e9}
+NCU_TRAFFIC_SOURCE = {("cfg5", "cf4"): "ncu --set full capture of csr_leja_iter_rowblock_kernel, round 1 (commit 6319c2a, "
+                                       "profiles/r1_csr_rowblock_ncu.md); the default instantiation of the kernel is "
+                                       "unchanged since (round 2 re-capture: profiles/r2_csr_rowblock_ncu.md)",
+                      ("cfg4", "cf4"): "ncu --set full capture of dense_leja_iter_kernel, round 1 (profiles/r1_dense_gemv_ncu.md); "
+                                       "kernel unchanged since"}
 
 
 # ----------------------------------------------------------------------------- helpers
@@ -141,17 +149,15 @@ def algorithmic_bytes_per_iteration(cfg, scheme):
 
 # ----------------------------------------------------------------------------- reference arm (CPU oracle)
 def oracle_sample(cfg, scheme, max_size=None):
-    """The bounded sample the oracle is timed on: ONE Magnus step of the workload's recipe.  The sparse
-    configs and the dense CF4 run at full size where that is tens of seconds; dense M4 by the plain
-    definition (two n^3 products) and the 2^24 chain are reduced, and the sample says so."""
+    """The bounded sample the oracle is timed on: ONE Magnus step of the workload's recipe at FULL size (same
+    config as the GPU arm).  Only dense M4 by the plain definition (two n^3 products per step: hours at
+    n = 16384) is reduced, to n = 4096, and the sample says so."""
     import workloads as W
     size = cfg.size
     if max_size is not None:
         size = min(size, max_size)
-    elif cfg.kind == "dense":
-        size = min(size, 2048 if scheme == "m4" else 8192)
-    else:
-        size = min(size, 22)
+    elif cfg.kind == "dense" and scheme == "m4":
+        size = min(size, 4096)
     return W.scaled(cfg, size, 1)
 
 
@@ -188,18 +194,24 @@ def time_oracle(cfg, scheme, steps, warmup, max_size=None):
 
 
 def run_reference(args):
+    """The reference arm is the CPU oracle (the tier has no reference code).  It times ONE Magnus step of the same
+    workload at full size, without warm-up (a step is tens of seconds of host time; `--steps K` would not end
+    within minutes), and reports the steps it actually timed."""
     rank, _, world = dist_env()
     if rank != 0:
         return
     import workloads as W
     cfg = W.CONFIGS[args.workload]
     scheme = args.scheme or cfg.schemes[0]
-    base = time_oracle(cfg, scheme, max(1, min(args.steps, 3)), min(args.warmup, 1), args.oracle_max_size)
-    line = {"impl": "reference", "metric": METRIC, "value": base["value"], "unit": UNIT, "n_gpus": args.gpus,
-            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 / base["value"], "higher_is_better": True,
+    timed = 1 if args.oracle_steps is None else max(1, args.oracle_steps)
+    base = time_oracle(cfg, scheme, timed, 0, args.oracle_max_size)
+    line = {"impl": "reference", "metric": METRIC, "value": base["value"], "unit": UNIT, "n_gpus": max(1, world),
+            "steps": timed, "warmup": 0, "ms_per_step": 1e3 / base["value"], "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "complex128 (f64)", "data": "synthetic",
             "config": {"workload": workload_description(cfg, scheme), "scheme": scheme,
-                       "note": "CPU oracle (oracle/), rank 0 only; each timed step is one Magnus step of the bounded sample"},
+                       "note": "CPU oracle (oracle/), rank 0 only; timed steps = 'steps' (requested: "
+                               f"--steps {args.steps} --warmup {args.warmup}); each step is one Magnus step of the sample",
+                       "same_size_as_gpu_arm": base["sample_size"] == base["full_size"]},
             "cpu_baseline": {k: base[k] for k in ("value", "unit", "cores", "kind", "sample")},
             "e2e": {"value": base["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -264,15 +276,18 @@ def measure_e2e(M, torch, cfg, scheme, steps, inputs):
     torch.cuda.synchronize()
     sec = time.perf_counter() - t0
     return {"value": steps / sec, "unit": UNIT, "h2d_bytes_per_step": h2d / steps, "d2h_bytes_per_step": d2h / steps,
-            "seconds": sec, "matvecs": st["total_matvecs"],
+            "seconds": sec, "seconds_integrate": st["seconds_device"], "seconds_h2d_create_d2h": sec - st["seconds_device"],
+            "steps": steps, "matvecs": st["total_matvecs"],
             "region": "one magnus_integrate_host call: H2D of H0, H1, psi0 from pinned host memory (inputs go to the "
-                      "device once per integration, PAPER.md l.209), magnus_create, K steps, D2H of psi"}
+                      "device ONCE per integration, PAPER.md l.209), magnus_create, K steps, D2H of psi; the one-off "
+                      "part (seconds_h2d_create_d2h) is amortised over the K steps of the call, so `value` depends on K"}
 
 
 def roofline_for(cfg, scheme, st, peaks, fp64_peak_tflops):
     r = _roofline_for(cfg, scheme, st, peaks, fp64_peak_tflops)
     if r["bound"] == "hbm":
         r["traffic"] = NCU_TRAFFIC_BYTES.get((cfg.name, scheme))
+        r["traffic_source"] = NCU_TRAFFIC_SOURCE.get((cfg.name, scheme))
     return r
 
 
@@ -303,24 +318,71 @@ def _roofline_for(cfg, scheme, st, peaks, fp64_peak_tflops):
             "frac_of_nominal_8TBs": achieved / 8000.0}
 
 
+def max_over_ranks(seconds: float, dist=None, device="cpu") -> float:
+    """The timed region of the job is the slowest rank's: MAX over ranks of the per-rank seconds (every rank gets
+    the result).  `dist` is torch.distributed when a process group is up, else None (single process)."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return float(seconds)
+    import torch
+    t = torch.tensor([seconds], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(steps: int, seconds_per_rank: float, dist=None, device="cpu"):
+    """(value, seconds): steps/s summed over all replicas = world * steps / max-over-ranks seconds."""
+    world = dist.get_world_size() if dist is not None and dist.is_initialized() else 1
+    sec = max_over_ranks(seconds_per_rank, dist, device)
+    return world * steps / sec, sec
+
+
+def respawn_under_torchrun(args) -> int:
+    """`python bench.py --gpus N` without a launcher: start N replicas, one process per GPU, over NCCL."""
+    port = 29500 + (os.getpid() % 2000)
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
+def measure_extra(M, W, torch, dev, peaks, dmma_tf):
+    """Short secondary measurements for the default line: cfg4 CF4 (2 steps, dense GEMV) and cfg4 M4 (1 step, DMMA)."""
+    out = {}
+    cfg = W.CONFIGS["cfg4"]
+    for scheme, steps in (("cf4", 2), ("m4", 1)):
+        sampler = ClockSampler(torch.cuda.current_device())
+        res = measure_workload(M, W, torch, cfg, scheme, steps, 1, dev, lambda: None, sampler)
+        st = res["stats"]
+        roof = roofline_for(cfg, scheme, st, peaks, dmma_tf)
+        out[f"cfg4_{scheme}"] = {"workload": workload_description(cfg, scheme), "steps": steps, "warmup": 1,
+                                 "value": steps / res["seconds"], "unit": UNIT, "ms_per_step": res["seconds"] / steps * 1e3,
+                                 "matvecs": st["total_matvecs"], "seconds_leja": st["seconds_leja"],
+                                 "seconds_commutator": st["seconds_commutator"], "gpu_launches": st["kernel_launches"],
+                                 "clocks": res["clocks"], "roofline": roof, "psi_norm_after": res["norm"]}
+        res["inputs"] = None
+        del res
+        torch.cuda.empty_cache()
+    return out
+
+
 def run_ours(args):
     import torch
     rank, local_rank, world = dist_env()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback "
                          "(use --impl reference for the oracle)")
+    if world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}: launch with torchrun --nproc-per-node "
+                         f"{args.gpus} (or without a launcher: bench.py starts the replicas itself)")
     torch.cuda.set_device(local_rank)
     dev = f"cuda:{local_rank}"
-    use_dist = world > 1
-    if use_dist:
+    dist = None
+    if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device(dev))
 
-        def barrier():
+    def barrier():
+        if dist is not None:
             dist.barrier()
-    else:
-        def barrier():
-            pass
 
     import paper_1709_06483_b200 as M     # raises if the CUDA library is missing
     import workloads as W
@@ -332,27 +394,19 @@ def run_ours(args):
 
     sampler = ClockSampler(local_rank) if rank == 0 else None
     res = measure_workload(M, W, torch, cfg, scheme, args.steps, args.warmup, dev, barrier, sampler)
-    sec = res["seconds"]
-    if use_dist:
-        t = torch.tensor([sec], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        sec = float(t.item())
+    value, sec = whole_job_value(args.steps, res["seconds"], dist, dev)
     st = res["stats"]
 
     e2e = None
     if not args.no_e2e:
         e2e = measure_e2e(M, torch, cfg, scheme, args.steps, res["inputs"])
-        if use_dist:
-            t = torch.tensor([e2e["seconds"]], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            e2e["seconds"] = float(t.item())
-            e2e["value"] = world * args.steps / e2e["seconds"]
+        e2e["value"], e2e["seconds"] = whole_job_value(args.steps, e2e["seconds"], dist, dev)
     res["inputs"] = None
     torch.cuda.empty_cache()
 
     if rank == 0:
         roof = roofline_for(cfg, scheme, st, peaks, dmma_tf)
-        line = {"metric": METRIC, "value": world * args.steps / sec, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": sec / args.steps * 1e3, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "complex128 (f64)", "data": "synthetic",
                 "config": {"workload": workload_description(cfg, scheme), "scheme": scheme,
@@ -365,12 +419,15 @@ def run_ours(args):
                 "clocks": res["clocks"], "gpu_launches": st["kernel_launches"], "roofline": roof,
                 "fp64_peaks_measured_tflops": {"dmma": dmma_tf, "dfma": dfma_tf}}
         if e2e:
-            line["e2e"] = {k: e2e[k] for k in ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step", "region")}
+            line["e2e"] = {k: e2e[k] for k in ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step", "steps",
+                                               "seconds", "seconds_integrate", "seconds_h2d_create_d2h", "region")}
+        if world == 1 and args.workload == "cfg5" and not args.no_extra:
+            line["extra"] = measure_extra(M, W, torch, dev, peaks, dmma_tf)
         if world == 1 and not args.no_cpu_baseline:
             base = time_oracle(cfg, scheme, 1, 0, args.oracle_max_size)
             line["cpu_baseline"] = {k: base[k] for k in ("value", "unit", "cores", "kind", "sample")}
         print(json.dumps(line), flush=True)
-    if use_dist:
+    if dist is not None:
         dist.barrier()
         dist.destroy_process_group()
 
@@ -391,12 +448,17 @@ def main():
     ap.add_argument("--scheme", default=None, choices=["cf4", "m4"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extra", action="store_true", help="skip the cfg4 secondary measurements of the default run")
+    ap.add_argument("--oracle-steps", type=int, default=None,
+                    help="reference arm: Magnus steps of the oracle to time (default 1: a step is tens of seconds)")
     ap.add_argument("--oracle-max-size", type=int, default=None,
                     help="cap N (xxz) or n (dense) of the oracle's bounded sample")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
     else:
+        if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+            raise SystemExit(respawn_under_torchrun(args))
         if args.warmup < 3:
             sys.stderr.write("bench.py: note: fewer than 3 warm-up steps\n")
         run_ours(args)

@@ -79,7 +79,10 @@ typedef struct magnus_options {
   int32_t check_hermitian; /* 1: sampled check in magnus_create (costs a device pass); default 0 */
   void* stream;        /* cudaStream_t; NULL = legacy default stream */
   int32_t csr_kernel;  /* 0 auto (n <= 4096: whole sweep in one launch; n >= 32768: row-block kernel; else generic),
-                          1 force the generic per-iteration kernel, 2 force the row-block per-iteration kernel */
+                          1 force the generic per-iteration kernel, 2 force the row-block per-iteration kernel,
+                          3 the warp-specialised TMA-ring kernel, 4 the row-block kernel with TMA staging (both need
+                          16-byte aligned value and index arrays, else the row-block kernel runs); values >= 1000
+                          select tuning variants of these kernels (see the kernel sources) */
   int32_t reserved;
 } magnus_options;
 
@@ -196,6 +199,16 @@ int magnus_zgemm(int64_t n, const void* A, int64_t lda, const void* B, int64_t l
  * work: device scratch of n*n complex128. */
 int magnus_commutator_dense(int64_t n, const void* A, const void* B, void* K, void* work,
                             void* stream);
+
+/* Omega_H of one M4 step on dense H (rows S2, D3, D4, S3 of the scope table; P:99, P:262 l.3-9 with A = -iH; c1):
+ *   A1 = H0 + f1 H1, A2 = H0 + f2 H1, P = A2 A1 (FP64 tensor-core GEMM),
+ *   Omega = (A1 + A2)/2 - i (sqrt(3) tau / 12) (P - P^H),
+ * exactly the launches magnus_step makes, exposed so that the assembled matrix can be compared entry by entry with
+ * the plain definition.  H0, H1 device, row-major, leading dimensions ld0, ld1 (0 = n), Hermitian.  Omega, work_a2,
+ * work_p: device, n*n complex128 each, pairwise distinct; Omega receives the result.  ab_host (nullable): raw
+ * Gershgorin interval of Omega.  Errors: EINVAL, ENOMEM, ECUDA. */
+int magnus_omega_dense(int64_t n, const void* H0, int64_t ld0, const void* H1, int64_t ld1, double f1, double f2,
+                       double tau, void* Omega, void* work_a2, void* work_p, void* stream, double* ab_host);
 
 /* C = A B - B A for CSR A, B (device), exact zeros dropped.  Two-call protocol:
  * with cap_nnz == 0 only *nnz_out is written; otherwise row_ptr_out[n+1],

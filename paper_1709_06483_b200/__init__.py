@@ -10,5 +10,5 @@ from .binding import (  # noqa: F401
     magnus_commutator_dense, magnus_create, magnus_destroy, magnus_fp64_peaks, magnus_gershgorin,
     magnus_host_divided_differences, magnus_host_leja_points, magnus_host_snap_interval,
     magnus_host_step_coefficients, magnus_integrate, magnus_integrate_host, magnus_leja_iteration, magnus_step,
-    magnus_version, magnus_zgemm,
+    magnus_omega_dense, magnus_version, magnus_zgemm,
 )

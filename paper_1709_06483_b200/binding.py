@@ -61,7 +61,7 @@ DRIVE = C.CFUNCTYPE(C.c_double, C.c_double, C.c_void_p)
 
 EXPORTS = [
     "magnus_create", "magnus_destroy", "leja_expmv", "magnus_step", "magnus_integrate", "magnus_integrate_host",
-    "magnus_gershgorin", "magnus_leja_iteration", "magnus_zgemm", "magnus_commutator_dense", "magnus_commutator_csr",
+    "magnus_gershgorin", "magnus_leja_iteration", "magnus_zgemm", "magnus_commutator_dense", "magnus_commutator_csr", "magnus_omega_dense",
     "magnus_fp64_peaks", "magnus_host_leja_points", "magnus_host_divided_differences", "magnus_host_snap_interval",
     "magnus_host_step_coefficients", "magnus_strerror", "magnus_last_error", "magnus_version",
 ]
@@ -102,6 +102,9 @@ def lib():
         L.magnus_commutator_dense.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.magnus_commutator_csr.argtypes = [C.POINTER(MatrixStruct), C.POINTER(MatrixStruct), C.c_int64,
                                             C.POINTER(C.c_int64), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.magnus_omega_dense.argtypes = [C.c_int64, C.c_void_p, C.c_int64, C.c_void_p, C.c_int64, C.c_double, C.c_double,
+                                         C.c_double, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                         C.POINTER(C.c_double)]
         L.magnus_fp64_peaks.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_void_p]
         L.magnus_host_leja_points.argtypes = [C.c_int, C.c_void_p]
         L.magnus_host_divided_differences.argtypes = [C.c_double, C.c_int, C.c_void_p]
@@ -307,6 +310,14 @@ def magnus_zgemm(A, B, Cout, stream=None) -> float:
 
 def magnus_commutator_dense(A, B, K, work, stream=None) -> None:
     _check(lib().magnus_commutator_dense(int(A.shape[0]), _ptr(A), _ptr(B), _ptr(K), _ptr(work), _stream_ptr(stream)))
+
+
+def magnus_omega_dense(H0, H1, f1: float, f2: float, tau: float, Omega, work_a2, work_p, stream=None) -> Tuple[float, float]:
+    """Omega_H of one dense M4 step into `Omega`; returns its raw Gershgorin interval."""
+    ab = (C.c_double * 2)()
+    _check(lib().magnus_omega_dense(int(H0.shape[0]), _ptr(H0), int(H0.stride(0)), _ptr(H1), int(H1.stride(0)), f1, f2,
+                                    tau, _ptr(Omega), _ptr(work_a2), _ptr(work_p), _stream_ptr(stream), ab))
+    return ab[0], ab[1]
 
 
 def magnus_commutator_csr(A, B, stream=None):

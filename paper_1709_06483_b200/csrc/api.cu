@@ -850,6 +850,41 @@ int magnus_commutator_dense(int64_t n, const void* A, const void* B, void* K, vo
   return MAGNUS_OK;
 }
 
+int magnus_omega_dense(int64_t n, const void* H0, int64_t ld0, const void* H1, int64_t ld1, double f1, double f2,
+                       double tau, void* Omega, void* work_a2, void* work_p, void* stream, double* ab_host) {
+  if (n <= 0 || !H0 || !H1 || !Omega || !work_a2 || !work_p || Omega == work_a2 || Omega == work_p ||
+      work_a2 == work_p || Omega == H0 || Omega == H1) {
+    set_error("magnus_omega_dense: bad arguments");
+    return MAGNUS_EINVAL;
+  }
+  if (ld0 == 0) ld0 = n;
+  if (ld1 == 0) ld1 = n;
+  int rc = require_device();
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  Workspace ws;
+  rc = workspace_alloc(&ws, 1);
+  if (rc) { workspace_free(&ws); return rc; }
+  // the same three launches magnus_step makes for M4 on dense H: S2 (A1, A2), D3 (P = A2 A1), D4 + S3
+  launch_dense_assemble2(n, (const cplx*)H0, ld0, (const cplx*)H1, ld1, f1, f2, (cplx*)Omega, (cplx*)work_a2, &ws, st);
+  rc = launch_zgemm(n, (const cplx*)work_a2, n, (const cplx*)Omega, n, (cplx*)work_p, n, st);
+  if (rc == MAGNUS_OK) {
+    const int nblk = launch_dense_omega(n, (cplx*)Omega, (const cplx*)work_a2, (const cplx*)work_p,
+                                        std::sqrt(3.0) * tau / 12.0, &ws, st);
+    double a = 0.0, b = 0.0;
+    rc = read_interval(nblk, &ws, st, &a, &b);
+    if (rc == MAGNUS_OK && ab_host) {
+      ab_host[0] = a;
+      ab_host[1] = b;
+    }
+    if (rc == MAGNUS_OK && cudaGetLastError() != cudaSuccess) rc = MAGNUS_ECUDA;
+  } else {
+    set_error("magnus_omega_dense: zgemm launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+  }
+  workspace_free(&ws);
+  return rc;
+}
+
 int magnus_commutator_csr(const magnus_matrix* A, const magnus_matrix* B, int64_t cap_nnz, int64_t* nnz_out,
                           int32_t* row_ptr_out, int32_t* col_idx_out, void* values_out, void* stream) {
   int rc = check_matrix(A, "A");

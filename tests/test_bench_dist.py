@@ -14,16 +14,15 @@ import pytest
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 WORKER = r"""
-import os, sys, torch, torch.distributed as dist
+import os, sys, torch.distributed as dist
+sys.path.insert(0, os.environ["BENCH_ROOT"])
+import bench                                    # bench.py's own reduction code, not a copy of it
 dist.init_process_group("gloo")
-rank, world = dist.get_rank(), dist.get_world_size()
-# what bench.py does with the per-rank seconds of the timed region
-t = torch.tensor([1.0 + rank], dtype=torch.float64)
+rank = dist.get_rank()
 dist.barrier()
-dist.all_reduce(t, op=dist.ReduceOp.MAX)
-steps = 5
+value, sec = bench.whole_job_value(5, 1.0 + rank, dist, "cpu")     # per-rank seconds of the timed region: 1.0, 2.0
 if rank == 0:
-    print("VALUE", world * steps / float(t.item()))
+    print("VALUE", value, sec)
 dist.barrier()
 dist.destroy_process_group()
 """
@@ -40,11 +39,30 @@ def _torchrun(args, env_extra=None, timeout=300):
 def test_max_over_ranks_and_whole_job_value(tmp_path):
     script = tmp_path / "worker.py"
     script.write_text(WORKER)
-    res = _torchrun([str(script)])
+    res = _torchrun([str(script)], env_extra={"BENCH_ROOT": ROOT})
     assert res.returncode == 0, res.stderr[-2000:]
     lines = [ln for ln in res.stdout.splitlines() if ln.startswith("VALUE")]
     assert len(lines) == 1                                   # rank 0 alone prints
     assert abs(float(lines[0].split()[1]) - 2 * 5 / 2.0) < 1e-12   # N*K / max(1.0, 2.0)
+    assert abs(float(lines[0].split()[2]) - 2.0) < 1e-12           # the slowest rank's seconds
+
+
+def test_single_process_reduction_is_identity():
+    sys.path.insert(0, ROOT)
+    import bench
+    assert bench.max_over_ranks(1.25) == 1.25
+    assert bench.whole_job_value(4, 2.0) == (2.0, 2.0)
+
+
+def test_gpus_flag_must_match_world_size():
+    """`--gpus 2` inside a 1-process environment that claims WORLD_SIZE=1 is refused, not silently run on one GPU."""
+    import torch
+    env = dict(os.environ, WORLD_SIZE="1", RANK="0", LOCAL_RANK="0")
+    res = subprocess.run([sys.executable, "bench.py", "--gpus", "2", "--steps", "1", "--warmup", "0"], cwd=ROOT, env=env,
+                         capture_output=True, text=True, timeout=300)
+    assert res.returncode != 0
+    msg = res.stderr + res.stdout
+    assert ("no CUDA device" in msg) if not torch.cuda.is_available() else ("WORLD_SIZE=1" in msg)
 
 
 def test_reference_arm_rank0_only():
