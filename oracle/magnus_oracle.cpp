@@ -14,6 +14,7 @@
 //
 //   Scheme M4   P:97-101 (Method 2), P:260-264 (pseudocode)        -> step_m4
 //   Scheme Cf4  P:130-134 (Method 4)                                -> step_cf4
+//   Scheme M6   P:103-114 (Method 3; reading m6: the coefficient of B3)  -> m6_omega_dense / m6_omega_csr
 //   Leja/Newton P:169-186 (formula and code fragment)               -> leja_expmv
 //   early stop  P:188, P:229-231 (reading c6)                       -> leja_expmv
 //   spectrum    P:190 (estimate "from the matrix"; Gershgorin, c4)  -> gershgorin_*
@@ -364,8 +365,9 @@ const double kC2 = 0.5 + std::sqrt(3.0) / 6.0;
 const double kAlpha1 = (3.0 - 2.0 * std::sqrt(3.0)) / 12.0;
 const double kAlpha2 = (3.0 + 2.0 * std::sqrt(3.0)) / 12.0;
 
-// Scheme codes: 0 = Cf4, 1 = M4, 2 = M2, 3 = Cf4:3, 101 = M4 with the commutator sign flipped
-// (a NEGATIVE CONTROL for the order test only: it must drop to order 2).
+// Scheme codes: 0 = Cf4, 1 = M4, 2 = M2, 3 = Cf4:3, 4 = M6, 101 = M4 with the commutator sign flipped
+// (a NEGATIVE CONTROL for the order test only: it must drop to order 2), 104 = M6 with the coefficient of B3
+// exactly as PAPER.md prints it (1/2; NEGATIVE CONTROL: see m6_c3).
 double m4_kappa(int scheme, double tau) {
   double kappa = std::sqrt(3.0) * tau / 12.0;
   return scheme == 101 ? -kappa : kappa;
@@ -413,6 +415,88 @@ int cf_exponentials(int scheme, drive_fn f, void* user, double t, double tau, do
 
 int exponentials_per_step(int scheme) { return scheme == 0 ? 2 : scheme == 3 ? 3 : 1; }
 
+// ---------------------------------------------------------------------------
+// M6 (Method 3).  With A_j = A(t + c_j tau) = -i H(t_j), c = 1/2 - sqrt(15)/10, 1/2, 1/2 + sqrt(15)/10:
+//   B1 = tau A2,  B2 = (sqrt(15)/3) tau (A3 - A1),  B3 = (10/3) tau (A3 - 2 A2 + A1),
+//   Omega = B1 + c3 B3 + (1/240) [ -20 B1 - B3 + [B1, B2],  B2 - (1/60) [B1, 2 B3 + [B1, B2]] ],
+//   psi <- exp(Omega) psi = exp(-i tau Omega_H) psi,  Omega_H = (i / tau) Omega  (Hermitian).
+// Reading m6: PAPER.md l.105 prints the coefficient of B3 as 1/2.  For A(t) = a0 + a1 s + a2 s^2 (s measured from
+// the midpoint) B1 = tau a0 and B3 = tau^3 a2 exactly, while the first Magnus term is int A = tau a0 + tau^3 a2 / 12:
+// the coefficient must be c3 = 1/12 for the scheme to be consistent beyond order 2 (the extracted formula lost a
+// digit).  tests/test_oracle_magnus.py shows order 6 with 1/12 and order 2 with the printed 1/2 (scheme 104).
+// Every commutator is formed by its plain definition X Y - Y X (two products).
+// ---------------------------------------------------------------------------
+double m6_c3(int scheme) { return scheme == 104 ? 0.5 : 1.0 / 12.0; }
+
+void m6_nodes(drive_fn f, void* user, double t, double tau, double* fn) {
+  const double r15 = std::sqrt(15.0);
+  fn[0] = f(t + (0.5 - r15 / 10.0) * tau, user);
+  fn[1] = f(t + 0.5 * tau, user);
+  fn[2] = f(t + (0.5 + r15 / 10.0) * tau, user);
+}
+
+void dense_comm(int64_t n, const cplx* X, const cplx* Y, cplx* K) {
+  std::vector<cplx> xy(n * n), yx(n * n);
+  dense_mul(n, X, Y, xy.data());
+  dense_mul(n, Y, X, yx.data());
+#pragma omp parallel for schedule(static)
+  for (int64_t q = 0; q < n * n; ++q) K[q] = xy[q] - yx[q];
+}
+
+// Omega_H of one M6 step, dense.
+void m6_omega_dense(int64_t n, const cplx* H0, const cplx* H1, const double* fn, double tau, double c3, cplx* OmH) {
+  const int64_t nn = n * n;
+  const cplx mi(0.0, -1.0);
+  const double r15 = std::sqrt(15.0);
+  std::vector<cplx> B1(nn), B2(nn), B3(nn), C1(nn), T(nn), C2(nn), L(nn), R(nn), K(nn);
+#pragma omp parallel for schedule(static)
+  for (int64_t q = 0; q < nn; ++q) {
+    const cplx A1 = mi * (H0[q] + fn[0] * H1[q]), A2 = mi * (H0[q] + fn[1] * H1[q]), A3 = mi * (H0[q] + fn[2] * H1[q]);
+    B1[q] = tau * A2;
+    B2[q] = (r15 / 3.0) * tau * (A3 - A1);
+    B3[q] = (10.0 / 3.0) * tau * (A3 - 2.0 * A2 + A1);
+  }
+  dense_comm(n, B1.data(), B2.data(), C1.data());                    // [B1, B2]
+#pragma omp parallel for schedule(static)
+  for (int64_t q = 0; q < nn; ++q) T[q] = 2.0 * B3[q] + C1[q];
+  dense_comm(n, B1.data(), T.data(), C2.data());                     // [B1, 2 B3 + [B1, B2]]
+#pragma omp parallel for schedule(static)
+  for (int64_t q = 0; q < nn; ++q) {
+    L[q] = -20.0 * B1[q] - B3[q] + C1[q];
+    R[q] = B2[q] - C2[q] / 60.0;
+  }
+  dense_comm(n, L.data(), R.data(), K.data());
+  const cplx i_over_tau(0.0, 1.0 / tau);
+#pragma omp parallel for schedule(static)
+  for (int64_t q = 0; q < nn; ++q) OmH[q] = i_over_tau * (B1[q] + c3 * B3[q] + K[q] / 240.0);
+}
+
+SpMat sp_comm(const CsrView& X, const CsrView& Y) {
+  SpMat xy = sp_mul(X, Y), yx = sp_mul(Y, X);
+  return sp_axpby(1.0, xy.view(), -1.0, yx.view());
+}
+
+// Omega_H of one M6 step, CSR (same formulas on sparse matrices).
+SpMat m6_omega_csr(const CsrView& H0, const CsrView& H1, const double* fn, double tau, double c3) {
+  const cplx mi(0.0, -1.0);
+  const double r15 = std::sqrt(15.0);
+  SpMat A1 = sp_axpby(mi, H0, mi * fn[0], H1), A2 = sp_axpby(mi, H0, mi * fn[1], H1), A3 = sp_axpby(mi, H0, mi * fn[2], H1);
+  SpMat B1 = sp_axpby(tau, A2.view(), 0.0, A2.view());
+  SpMat B2 = sp_axpby((r15 / 3.0) * tau, A3.view(), -(r15 / 3.0) * tau, A1.view());
+  SpMat S13 = sp_axpby(1.0, A3.view(), 1.0, A1.view());
+  SpMat B3 = sp_axpby((10.0 / 3.0) * tau, S13.view(), -(20.0 / 3.0) * tau, A2.view());
+  SpMat C1 = sp_comm(B1.view(), B2.view());
+  SpMat T = sp_axpby(2.0, B3.view(), 1.0, C1.view());
+  SpMat C2 = sp_comm(B1.view(), T.view());
+  SpMat L0 = sp_axpby(-20.0, B1.view(), -1.0, B3.view());
+  SpMat L = sp_axpby(1.0, L0.view(), 1.0, C1.view());
+  SpMat R = sp_axpby(1.0, B2.view(), -1.0 / 60.0, C2.view());
+  SpMat K = sp_comm(L.view(), R.view());
+  SpMat O1 = sp_axpby(1.0, B1.view(), c3, B3.view());
+  const cplx i_over_tau(0.0, 1.0 / tau);
+  return sp_axpby(i_over_tau, O1.view(), i_over_tau / 240.0, K.view());
+}
+
 // One step on dense H0, H1.  Cf4: P:132-134 with A = -iH (c1): first
 // exp(-i tau/2 (H0 + g_a H1)), g_a = 2(alpha2 f1 + alpha1 f2), then
 // exp(-i tau/2 (H0 + g_b H1)), g_b = 2(alpha1 f1 + alpha2 f2).
@@ -432,6 +516,13 @@ int step_dense(int64_t n, const cplx* H0, const cplx* H1, drive_fn f, void* user
       if (rc) return rc;
     }
     return 0;
+  }
+  if (scheme == 4 || scheme == 104) {
+    double fn[3];
+    m6_nodes(f, user, t, tau, fn);
+    std::vector<cplx> OmH(nn);
+    m6_omega_dense(n, H0, H1, fn, tau, m6_c3(scheme), OmH.data());
+    return leja_expmv(DenseView(n, OmH.data()), psi, psi, tau, tol, infos);
   }
   const double f1 = f(t + kC1 * tau, user), f2 = f(t + kC2 * tau, user);
   std::vector<cplx> A1(nn), A2(nn), P21(nn), P12(nn), Om(nn);
@@ -456,6 +547,12 @@ int step_csr(const CsrView& H0, const CsrView& H1, drive_fn f, void* user, int s
       if (rc) return rc;
     }
     return 0;
+  }
+  if (scheme == 4 || scheme == 104) {
+    double fn[3];
+    m6_nodes(f, user, t, tau, fn);
+    SpMat OmH = m6_omega_csr(H0, H1, fn, tau, m6_c3(scheme));
+    return leja_expmv(OmH.view(), psi, psi, tau, tol, infos);
   }
   const double f1 = f(t + kC1 * tau, user), f2 = f(t + kC2 * tau, user);
   SpMat A1 = sp_axpby(1.0, H0, f1, H1), A2 = sp_axpby(1.0, H0, f2, H1);
@@ -570,6 +667,12 @@ int oracle_commutator_csr(int64_t n, const int32_t* arp, const int32_t* aci, con
 }
 
 // One step t -> t + tau.  infos: room for 3 entries (Cf4:3 uses all, Cf4 two, M4 and M2 the first).
+// Omega_H of one M6 step (dense) at the three node values fn[0..2] of f: exposed so that its structure can be pinned.
+void oracle_m6_omega_dense(int64_t n, const double* H0, const double* H1, const double* fn, double tau, double* out) {
+  m6_omega_dense(n, reinterpret_cast<const cplx*>(H0), reinterpret_cast<const cplx*>(H1), fn, tau, m6_c3(4),
+                 reinterpret_cast<cplx*>(out));
+}
+
 int oracle_magnus_step_dense(int64_t n, const double* H0, const double* H1, drive_fn f, void* user,
                              int scheme, double t, double tau, double* psi, double tol,
                              oracle_expmv_info* infos) {

@@ -13,9 +13,10 @@ import numpy as np
 
 from . import build as _build
 
-CF4, M4, M2, CF4_3, M4_WRONG_SIGN = 0, 1, 2, 3, 101
-SCHEMES = {"cf4": CF4, "m4": M4, "m2": M2, "cf4:3": CF4_3, "m4_wrong_sign": M4_WRONG_SIGN}
-N_EXP = {CF4: 2, M4: 1, M2: 1, CF4_3: 3, M4_WRONG_SIGN: 1}
+CF4, M4, M2, CF4_3, M6, M4_WRONG_SIGN, M6_AS_PRINTED = 0, 1, 2, 3, 4, 101, 104
+SCHEMES = {"cf4": CF4, "m4": M4, "m2": M2, "cf4:3": CF4_3, "m6": M6, "m4_wrong_sign": M4_WRONG_SIGN,
+           "m6_as_printed": M6_AS_PRINTED}
+N_EXP = {CF4: 2, M4: 1, M2: 1, CF4_3: 3, M6: 1, M4_WRONG_SIGN: 1, M6_AS_PRINTED: 1}
 
 DRIVE = C.CFUNCTYPE(C.c_double, C.c_double, C.c_void_p)
 
@@ -155,6 +156,15 @@ def commutator(A, B):
     K = np.empty_like(A)
     lib().oracle_commutator_dense(C.c_int64(A.shape[0]), _p(A), _p(B), _p(K))
     return K
+
+
+def m6_omega(H0, H1, fn, tau: float) -> np.ndarray:
+    """Omega_H of one M6 step on dense H0, H1 at the node values fn = (f(t1), f(t2), f(t3))."""
+    H0 = _c(H0, np.complex128); H1 = _c(H1, np.complex128)
+    fn = _c(fn, np.float64)
+    out = np.empty_like(H0)
+    lib().oracle_m6_omega_dense(C.c_int64(H0.shape[0]), _p(H0), _p(H1), _p(fn), C.c_double(tau), _p(out))
+    return out
 
 
 def _drive(f: Callable[[float], float]):

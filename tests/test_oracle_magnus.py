@@ -315,3 +315,100 @@ def test_m2_cf43_time_independent_and_reversal(oracle, scheme):
     a, _ = oracle.magnus_step(H0, H1, f, scheme, 0.2, 0.1, psi0, 1e-13)
     b, _ = oracle.magnus_step(H0, H1, f, scheme, 0.3, -0.1, a, 1e-13)
     assert np.linalg.norm(b - psi0) < 1e-11
+
+
+# ------------------------------------------------------------------ M6 (Method 3)
+def _herm_pair(n, seed):
+    r = np.random.default_rng(seed)
+    def herm():
+        G = r.normal(size=(n, n)) + 1j * r.normal(size=(n, n))
+        return (G + G.conj().T) / 2
+    H0, H1 = herm(), herm()
+    psi0 = r.normal(size=n) + 1j * r.normal(size=n)
+    return H0, H1, psi0 / np.linalg.norm(psi0)
+
+
+def test_m6_order_six_and_printed_coefficient_is_order_two(oracle):
+    """P:103 "the following scheme of order six": step-halving slope 6 against a brute-force propagator that does not
+    use the oracle.  Reading m6: with the coefficient of B3 as PAPER.md l.105 prints it (1/2) the same test gives
+    order 2 -- the first Magnus term int A = tau a0 + tau^3 a2/12 needs 1/12."""
+    n = 10
+    H0, H1, psi0 = _herm_pair(n, 11)
+    H0, H1 = 0.6 * H0, 0.6 * H1
+    f = lambda t: math.sin(3 * t) + 0.3 * t
+    T = 0.6
+    # reference: the oracle-independent exact-exponential midpoint rule, Richardson-extrapolated twice (errors
+    # O(dt^2), O(dt^4) removed) so that it is good to ~1e-13, below the order-6 errors measured here
+    U1 = _exact_propagator_reference(H0, H1, f, 0.0, T, fine=1500) @ psi0
+    U2 = _exact_propagator_reference(H0, H1, f, 0.0, T, fine=3000) @ psi0
+    U4 = _exact_propagator_reference(H0, H1, f, 0.0, T, fine=6000) @ psi0
+    R1, R2 = (4 * U2 - U1) / 3, (4 * U4 - U2) / 3
+    exact = (16 * R2 - R1) / 15
+    assert np.linalg.norm(R2 - exact) < 1e-11
+    errs = []
+    for ns in (2, 4, 8):
+        psi, _ = oracle.magnus_integrate(H0, H1, f, "m6", 0.0, T, ns, psi0, 1e-15)
+        errs.append(np.linalg.norm(psi - exact))
+    slopes = [math.log2(errs[i] / errs[i + 1]) for i in range(2)]
+    assert errs[-1] > 3e-12, errs                         # still above the reference's own accuracy
+    assert all(5.5 < s < 6.6 for s in slopes), (errs, slopes)
+    bad = []
+    for ns in (4, 8, 16):
+        psi, _ = oracle.magnus_integrate(H0, H1, f, "m6_as_printed", 0.0, T, ns, psi0, 1e-14)
+        bad.append(np.linalg.norm(psi - exact))
+    bslopes = [math.log2(bad[i] / bad[i + 1]) for i in range(2)]
+    assert all(1.7 < s < 2.3 for s in bslopes), (bad, bslopes)
+    # and M6 beats the fourth-order schemes at the same step (P:156, Figure 1)
+    p4, _ = oracle.magnus_integrate(H0, H1, f, "m4", 0.0, T, 8, psi0, 1e-15)
+    assert errs[-1] < 0.05 * np.linalg.norm(p4 - exact)
+
+
+def test_m6_time_independent_commuting_and_reversal(oracle):
+    n = 14
+    H0, H1, psi0 = _herm_pair(n, 12)
+    # f = const: B2 = B3 = 0, Omega = tau A: exact exponential
+    psi, iters = oracle.magnus_integrate(H0, H1, lambda t: -0.4, "m6", 0.0, 0.7, 3, psi0, 1e-13)
+    lam, V = np.linalg.eigh(H0 - 0.4 * H1)
+    assert np.linalg.norm(psi - V @ (np.exp(-0.7j * lam) * (V.conj().T @ psi0))) < 1e-11 and len(iters) == 3
+    # time reversal: step(t, tau) then step(t + tau, -tau) is the identity (the scheme is self-adjoint)
+    f = lambda t: math.cos(2 * t) + t * t
+    a, _ = oracle.magnus_step(H0, H1, f, "m6", 0.1, 0.2, psi0, 1e-13)
+    b, _ = oracle.magnus_step(H0, H1, f, "m6", 0.3, -0.2, a, 1e-13)
+    assert np.linalg.norm(b - psi0) < 1e-11 and np.linalg.norm(a - psi0) > 1e-2
+    # commuting H0, H1: every commutator vanishes, Omega_H = H0 + Q3 H1 with Q3 the three-point Gauss rule of f
+    U = np.linalg.qr(H0)[0]
+    r = np.random.default_rng(13)
+    D0 = (U * r.normal(size=n)) @ U.conj().T; D0 = (D0 + D0.conj().T) / 2
+    D1 = (U * r.normal(size=n)) @ U.conj().T; D1 = (D1 + D1.conj().T) / 2
+    t, tau = 0.3, 0.25
+    s15 = math.sqrt(15) / 10
+    fn = [f(t + (0.5 - s15) * tau), f(t + 0.5 * tau), f(t + (0.5 + s15) * tau)]
+    Om = oracle.m6_omega(D0, D1, fn, tau)
+    Q3 = (5 * fn[0] + 8 * fn[1] + 5 * fn[2]) / 18
+    assert np.abs(Om - (D0 + Q3 * D1)).max() < 1e-13
+
+
+def test_m6_omega_structure_and_csr_agrees_with_dense(oracle):
+    """Omega_H is Hermitian; its leading terms are the ones the formula prints: H0 + Q3 H1 + (commutator terms of
+    relative size tau); and the CSR implementation of the same formulas gives the same step as the dense one."""
+    N = 6
+    H0s, H1s = xxz.xxz_h0(N), xxz.xxz_h1(N)
+    H0d, H1d = H0s.to_scipy().toarray(), H1s.to_scipy().toarray()
+    f = xxz.f_cos2t
+    t, tau = 0.4, 0.05
+    s15 = math.sqrt(15) / 10
+    fn = [f(t + (0.5 - s15) * tau), f(t + 0.5 * tau), f(t + (0.5 + s15) * tau)]
+    Om = oracle.m6_omega(H0d, H1d, fn, tau)
+    assert np.abs(Om - Om.conj().T).max() < 1e-13
+    Q3 = (5 * fn[0] + 8 * fn[1] + 5 * fn[2]) / 18
+    C = H0d @ H1d - H1d @ H0d
+    # leading commutator term: (1/240)[-20 B1, B2] = -(1/12)[B1, B2], and with A = -iH
+    # [B1, B2] = -(sqrt(15)/3) tau^2 (f3 - f1) [H0, H1], so
+    # Omega_H = (i/tau) Omega = H0 + Q3 H1 + i (sqrt(15)/36) tau (f3 - f1) [H0, H1] + O(tau^3)
+    # (the counterpart of M4's -i (sqrt(3) tau/12)(f1 - f2)[H0, H1], P:99, on the three-point nodes)
+    lead = H0d + Q3 * H1d + 1j * (math.sqrt(15) / 36) * tau * (fn[2] - fn[0]) * C
+    assert np.abs(Om - lead).max() < 5e-3 * tau and np.abs(Om - (H0d + Q3 * H1d)).max() > 1e-4
+    psi0 = rand_vec(1 << N, 7)
+    a, ia = oracle.magnus_step(oracle.CsrHost.of(H0s), oracle.CsrHost.of(H1s), f, "m6", t, tau, psi0)
+    b, ib = oracle.magnus_step(H0d, H1d, f, "m6", t, tau, psi0)
+    assert np.linalg.norm(a - b) < 1e-12 and ia[0]["iters"] == ib[0]["iters"]
