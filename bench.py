@@ -156,8 +156,10 @@ def oracle_sample(cfg, scheme, max_size=None):
     size = cfg.size
     if max_size is not None:
         size = min(size, max_size)
-    elif cfg.kind == "dense" and scheme == "m4":
-        size = min(size, 4096)
+    elif cfg.kind == "dense" and scheme in ("m4", "m6"):
+        size = min(size, 4096 if scheme == "m4" else 2048)
+    elif cfg.kind == "xxz" and scheme == "m6":
+        size = min(size, 12)
     return W.scaled(cfg, size, 1)
 
 
@@ -295,8 +297,9 @@ def _roofline_for(cfg, scheme, st, peaks, fp64_peak_tflops):
     """Dominant kernel of the step: the fused Leja iteration (HBM) or, for M4 on dense H, the DMMA commutator."""
     leja_s, comm_s, mv = st["seconds_leja"], st["seconds_commutator"], max(1, st["total_matvecs"])
     nsteps_exp = max(1, st["n_exp"])
-    if cfg.kind == "dense" and scheme == "m4" and comm_s > leja_s:
-        flops = 8.0 * cfg.n ** 3                       # one complex product P = A2 A1 (K = P - P^H)
+    if cfg.kind == "dense" and scheme in ("m4", "m6") and comm_s > leja_s:
+        # M4: one complex product P = A2 A1 per step (K = P - P^H); M6: three (magnus.h at magnus_step)
+        flops = 8.0 * cfg.n ** 3 * (3 if scheme == "m6" else 1)
         achieved = flops * nsteps_exp / comm_s / 1e12
         return {"kernel": "zgemm_dmma_kernel", "bound": "tensor", "achieved": achieved, "peak": fp64_peak_tflops,
                 "unit": "TFLOP/s", "frac": achieved / fp64_peak_tflops if fp64_peak_tflops else None, "traffic": None,
@@ -445,7 +448,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--workload", default="cfg5", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
-    ap.add_argument("--scheme", default=None, choices=["cf4", "m4"])
+    ap.add_argument("--scheme", default=None, choices=["cf4", "m4", "m2", "cf4:3", "m6"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extra", action="store_true", help="skip the cfg4 secondary measurements of the default run")

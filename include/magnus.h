@@ -49,6 +49,7 @@ extern "C" {
 #define MAGNUS_M4    1            /* classical, one commutator          (Method 2) */
 #define MAGNUS_M2    2            /* exponential midpoint rule          (Method 1) */
 #define MAGNUS_CF4_3 3            /* optimised commutator-free, three exponentials (Method 5) */
+#define MAGNUS_M6    4            /* sixth order, nested commutators     (Method 3; reading m6) */
 
 #define MAGNUS_MAX_EXP_PER_STEP 3
 
@@ -120,7 +121,7 @@ typedef struct magnus_context* magnus_handle;
  *   H0, H1  device matrices of the same format and n; BORROWED until magnus_destroy
  *           (kept alive and unmodified by the caller).
  *   f,user  the scalar drive; called on the host.
- *   scheme  MAGNUS_CF4 / MAGNUS_M4 / MAGNUS_M2 / MAGNUS_CF4_3.
+ *   scheme  MAGNUS_CF4 / MAGNUS_M4 / MAGNUS_M2 / MAGNUS_CF4_3 / MAGNUS_M6.
  * Allocates every workspace once (w ping-pong, p, partial-norm buffers; CSR: per-term row
  * statistics for the Gershgorin bounds, 24 n bytes per term, and a test whether the terms'
  * patterns overlap -- c4 takes the modulus of the SUMMED entry, which separates only if
@@ -129,6 +130,9 @@ typedef struct magnus_context* magnus_handle;
  * M4: computes and owns the sparse commutator C = [H0, H1] -- row S0 of the
  * scope table -- so that a step only rescales it, since
  * [H(t2), H(t1)] = (f1 - f2) [H0, H1]).
+ * M6 runs on dense matrices (three FP64 tensor-core GEMMs per step, see magnus_step); CSR input of n <= 16384 --
+ * the range the paper runs sparse M6 on -- is expanded into handle-owned dense copies, larger CSR
+ * input is refused (EINVAL): the nested commutators fill in.
  * Errors: EINVAL, ENOMEM, ECUDA, ENOTHERMITIAN (only with check_hermitian). */
 int magnus_create(magnus_handle* out, const magnus_matrix* H0, const magnus_matrix* H1,
                   magnus_drive_fn f, void* user, int scheme, const magnus_options* opt);
@@ -150,7 +154,12 @@ int leja_expmv(const magnus_matrix* H, const void* v_in, void* v_out, double h, 
  * n complex128) updated in place.  CF4 (c1): exp(-i tau/2 (H0+g_a H1))
  * then exp(-i tau/2 (H0+g_b H1)).  M4 (c1): one exponential of
  * Omega_H = (H(t1)+H(t2))/2 - i (sqrt(3) tau/12) [H(t2),H(t1)] with h = tau; on dense
- * H the commutator is one FP64 tensor-core complex GEMM per step.  info nullable. */
+ * H the commutator is one FP64 tensor-core complex GEMM per step.  M6 (reading m6): with H2 = H(t2),
+ * b2 = (sqrt(15)/3) tau (f3 - f1), b3 = (10/3) tau (f3 - 2 f2 + f1) and A = -iH every nested commutator reduces to a
+ * product of Hermitian / anti-Hermitian factors, three GEMMs in all:  G = [H2, H1] = P1 - P1^H (P1 = H2 H1),
+ * S = [H2, G] = P2 + P2^H (P2 = H2 G),  L = 20 i tau H2 + i b3 H1 - tau b2 G,
+ * R = -i b2 H1 + (tau b3/30) G - (i tau^2 b2/60) S,  Omega_H = H2 + (b3/(12 tau)) H1 + (i/(240 tau)) (P3 - P3^H),
+ * P3 = L R;  one exponential with h = tau.  info nullable. */
 int magnus_step(magnus_handle h, double t, double tau, void* psi, magnus_step_info* info);
 
 /* magnus_integrate -- nsteps steps of size tau = (t_end - t0)/nsteps from

@@ -18,8 +18,8 @@ LIB_PATH = os.path.join(HERE, "libmagnus_b200.so")
 
 OK, EINVAL, ENOMEM, ECUDA, ENOCONV, ENOTHERMITIAN = 0, -1, -2, -3, -4, -5
 DENSE, CSR = 0, 1
-CF4, M4, M2, CF4_3 = 0, 1, 2, 3
-SCHEMES = {"cf4": CF4, "m4": M4, "m2": M2, "cf4:3": CF4_3}
+CF4, M4, M2, CF4_3, M6 = 0, 1, 2, 3, 4
+SCHEMES = {"cf4": CF4, "m4": M4, "m2": M2, "cf4:3": CF4_3, "m6": M6}
 MAX_EXP_PER_STEP = 3
 
 
@@ -371,7 +371,7 @@ def magnus_host_step_coefficients(scheme, f, t: float, tau: float):
     kappa = C.c_double()
     cb = _drive(f)
     n = _check(lib().magnus_host_step_coefficients(sc, cb, None, t, tau, coef, hs, C.byref(kappa)))
-    m = 2 if sc == M4 else n
+    m = 2 if sc == M4 else (3 if sc == M6 else n)
     return list(coef)[:m], list(hs)[:n], kappa.value
 
 

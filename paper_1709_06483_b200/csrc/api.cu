@@ -13,6 +13,8 @@
 
 namespace magnus {
 
+const int kM6DenseMaxN = 16384;   // CSR input of MAGNUS_M6 is expanded into dense copies up to this n
+
 static thread_local char g_err[512] = "";
 
 void set_error(const char* fmt, ...) {
@@ -268,10 +270,15 @@ struct magnus_context {
   LejaParams prm;
   cudaStream_t stream = 0;
   Workspace ws;
-  // dense: assembled matrix (commutator-free schemes) or A1 (M4; Omega_H overwrites it), A2, P
+  // dense: assembled matrix (commutator-free schemes) or A1 (M4; Omega_H overwrites it), A2, P; M6: two more
   cplx* M = nullptr;
   cplx* A2 = nullptr;
   cplx* P = nullptr;
+  cplx* X4 = nullptr;
+  cplx* X5 = nullptr;
+  // M6 on CSR input (n <= kM6DenseMaxN): handle-owned dense copies of H0, H1
+  cplx* d0 = nullptr;
+  cplx* d1 = nullptr;
   // CSR M4: cached C = [H0, H1] (row S0)
   int32_t* c_rp = nullptr;
   int32_t* c_ci = nullptr;
@@ -392,6 +399,10 @@ int magnus_destroy(magnus_handle h) {
   cudaFree(h->M);
   cudaFree(h->A2);
   cudaFree(h->P);
+  cudaFree(h->X4);
+  cudaFree(h->X5);
+  cudaFree(h->d0);
+  cudaFree(h->d1);
   cudaFree(h->c_rp);
   cudaFree(h->c_ci);
   cudaFree(h->c_v);
@@ -415,7 +426,7 @@ int magnus_create(magnus_handle* out, const magnus_matrix* H0, const magnus_matr
   if (rc) return rc;
   if (H0->format != H1->format || H0->n != H1->n) { set_error("H0 and H1 differ in format or n"); return MAGNUS_EINVAL; }
   if (!f) { set_error("f is NULL"); return MAGNUS_EINVAL; }
-  if (scheme < MAGNUS_CF4 || scheme > MAGNUS_CF4_3) { set_error("unknown scheme %d", scheme); return MAGNUS_EINVAL; }
+  if (scheme < MAGNUS_CF4 || scheme > MAGNUS_M6) { set_error("unknown scheme %d", scheme); return MAGNUS_EINVAL; }
   rc = require_device();
   if (rc) return rc;
 
@@ -453,18 +464,47 @@ int magnus_create(magnus_handle* out, const magnus_matrix* H0, const magnus_matr
     }
   }
 
+  if (scheme == MAGNUS_M6 && h->format == MAGNUS_CSR) {
+    // the nested commutators of M6 fill in: CSR input of the sizes the paper runs (n <= 2^14) is
+    // expanded into dense copies and takes the dense path; larger CSR input is refused
+    if (h->n > kM6DenseMaxN) {
+      set_error("MAGNUS_M6 on CSR input needs n <= %d (the nested commutators fill in; got n=%lld)", kM6DenseMaxN,
+                (long long)h->n);
+      magnus_destroy(h);
+      return MAGNUS_EINVAL;
+    }
+    const size_t bytes = sizeof(cplx) * (size_t)h->n * (size_t)h->n;
+    if (cudaMalloc(&h->d0, bytes) != cudaSuccess || cudaMalloc(&h->d1, bytes) != cudaSuccess) {
+      cudaGetLastError();
+      set_error("dense copies for M6 on CSR input: allocation failed (%zu bytes each)", bytes);
+      magnus_destroy(h);
+      return MAGNUS_ENOMEM;
+    }
+    launch_csr_to_dense(h->n, H0->row_ptr, H0->col_idx, (const cplx*)H0->values, h->d0, h->stream);
+    launch_csr_to_dense(h->n, H1->row_ptr, H1->col_idx, (const cplx*)H1->values, h->d1, h->stream);
+    std::memset(&h->H0, 0, sizeof h->H0);
+    std::memset(&h->H1, 0, sizeof h->H1);
+    h->H0.format = h->H1.format = MAGNUS_DENSE;
+    h->H0.n = h->H1.n = h->n;
+    h->H0.ld = h->H1.ld = h->n;
+    h->H0.values = h->d0;
+    h->H1.values = h->d1;
+    h->format = MAGNUS_DENSE;
+  }
   if (h->format == MAGNUS_DENSE) {
     const size_t bytes = sizeof(cplx) * (size_t)h->n * (size_t)h->n;
     bool ok = cudaMalloc(&h->M, bytes) == cudaSuccess;
-    if (ok && scheme == MAGNUS_M4)
+    if (ok && (scheme == MAGNUS_M4 || scheme == MAGNUS_M6))
       ok = cudaMalloc(&h->A2, bytes) == cudaSuccess && cudaMalloc(&h->P, bytes) == cudaSuccess;
+    if (ok && scheme == MAGNUS_M6)
+      ok = cudaMalloc(&h->X4, bytes) == cudaSuccess && cudaMalloc(&h->X5, bytes) == cudaSuccess;
     if (!ok) {
       cudaGetLastError();
       set_error("dense workspace allocation failed (%zu bytes per matrix)", bytes);
       magnus_destroy(h);
       return MAGNUS_ENOMEM;
     }
-    if (scheme == MAGNUS_M4) {
+    if (scheme == MAGNUS_M4 || scheme == MAGNUS_M6) {
       cudaEventCreate(&h->ev_comm[0]);
       cudaEventCreate(&h->ev_comm[1]);
       h->time_comm = true;
@@ -532,7 +572,38 @@ int magnus_step(magnus_handle h, double t, double tau, void* psi_, magnus_step_i
       const cplx* H0v = (const cplx*)h->H0.values;
       const cplx* H1v = (const cplx*)h->H1.values;
       int nblk = 0;
-      if (h->scheme == MAGNUS_M4) {
+      if (h->scheme == MAGNUS_M6) {
+        // P:103-114 with A = -iH (reading m6); X1 = h->M, X2 = h->A2, X3 = h->P, X4, X5; see magnus.h at magnus_step
+        const int64_t n = h->n;
+        const double f1 = coef[0], f2 = coef[1], f3 = coef[2];
+        const double b2 = (std::sqrt(15.0) / 3.0) * tau * (f3 - f1), b3 = (10.0 / 3.0) * tau * (f3 - 2.0 * f2 + f1);
+        LinComb lc;
+        auto term = [&](int k, const cplx* x, double re, double im) {
+          lc.x[k] = x;
+          lc.c[k] = make_double2(re, im);
+        };
+        term(0, H0v, 1.0, 0.0); term(1, H1v, f2, 0.0); term(2, nullptr, 0.0, 0.0); term(3, nullptr, 0.0, 0.0);
+        if (dense_ld(&h->H0) != n || dense_ld(&h->H1) != n) { set_error("MAGNUS_M6 needs ld == n"); rc = MAGNUS_EINVAL; break; }
+        launch_dense_lincomb(n, h->M, lc, ws, st);                                   // X1 = H2 = H0 + f2 H1
+        if (h->time_comm) cudaEventRecord(h->ev_comm[0], st);
+        rc = launch_zgemm(n, h->M, n, H1v, n, h->A2, n, st);                          // X2 = P1 = H2 H1
+        if (rc) break;
+        launch_dense_antiherm(n, h->A2, h->P, -1.0, st);                              // X3 = G = P1 - P1^H = [H2, H1]
+        rc = launch_zgemm(n, h->M, n, h->P, n, h->A2, n, st);                         // X2 = P2 = H2 G
+        if (rc) break;
+        launch_dense_antiherm(n, h->A2, h->X4, 1.0, st);                              // X4 = S = P2 + P2^H = [H2, G]
+        term(0, h->M, 0.0, 20.0 * tau); term(1, H1v, 0.0, b3); term(2, h->P, -tau * b2, 0.0); term(3, nullptr, 0.0, 0.0);
+        launch_dense_lincomb(n, h->A2, lc, ws, st);                                  // X2 = L
+        term(0, H1v, 0.0, -b2); term(1, h->P, tau * b3 / 30.0, 0.0); term(2, h->X4, 0.0, -tau * tau * b2 / 60.0);
+        term(3, nullptr, 0.0, 0.0);
+        launch_dense_lincomb(n, h->X5, lc, ws, st);                                  // X5 = R
+        rc = launch_zgemm(n, h->A2, n, h->X5, n, h->X4, n, st);                       // X4 = P3 = L R
+        ws->launches += 5;
+        if (h->time_comm) cudaEventRecord(h->ev_comm[1], st);
+        if (rc) break;
+        // Omega_H = H2 + (b3/(12 tau)) H1 + (i/(240 tau)) (P3 - P3^H), over X1, with its Gershgorin bounds
+        nblk = launch_dense_omega(n, h->M, H1v, h->X4, 1.0, b3 / (12.0 * tau), -1.0 / (240.0 * tau), ws, st);
+      } else if (h->scheme == MAGNUS_M4) {
         launch_dense_assemble2(h->n, H0v, dense_ld(&h->H0), H1v, dense_ld(&h->H1), coef[0], coef[1], h->M, h->A2, ws,
                                st);                                                                // S2: A1, A2
         if (h->time_comm) cudaEventRecord(h->ev_comm[0], st);
@@ -540,7 +611,7 @@ int magnus_step(magnus_handle h, double t, double tau, void* psi_, magnus_step_i
         ws->launches += 1;
         if (h->time_comm) cudaEventRecord(h->ev_comm[1], st);
         if (rc) { set_error("zgemm launch failed: %s", cudaGetErrorString(cudaGetLastError())); break; }
-        nblk = launch_dense_omega(h->n, h->M, h->A2, h->P, std::sqrt(3.0) * tau / 12.0, ws, st);    // D4 (+S3)
+        nblk = launch_dense_omega(h->n, h->M, h->A2, h->P, 0.5, 0.5, std::sqrt(3.0) * tau / 12.0, ws, st);   // D4 (+S3)
       } else {
         nblk = launch_dense_assemble(h->n, H0v, dense_ld(&h->H0), H1v, dense_ld(&h->H1), coef[e], h->M, ws, st);
       }
@@ -844,7 +915,7 @@ int magnus_commutator_dense(int64_t n, const void* A, const void* B, void* K, vo
   cudaStream_t st = (cudaStream_t)stream;
   rc = launch_zgemm(n, (const cplx*)A, n, (const cplx*)B, n, (cplx*)work, n, st);   // P = A B
   if (rc) return rc;
-  launch_dense_antiherm(n, (const cplx*)work, (cplx*)K, st);                        // K = P - P^H
+  launch_dense_antiherm(n, (const cplx*)work, (cplx*)K, -1.0, st);                  // K = P - P^H
   CU_TRY(cudaStreamSynchronize(st));
   CU_TRY(cudaGetLastError());
   return MAGNUS_OK;
@@ -869,7 +940,7 @@ int magnus_omega_dense(int64_t n, const void* H0, int64_t ld0, const void* H1, i
   launch_dense_assemble2(n, (const cplx*)H0, ld0, (const cplx*)H1, ld1, f1, f2, (cplx*)Omega, (cplx*)work_a2, &ws, st);
   rc = launch_zgemm(n, (const cplx*)work_a2, n, (const cplx*)Omega, n, (cplx*)work_p, n, st);
   if (rc == MAGNUS_OK) {
-    const int nblk = launch_dense_omega(n, (cplx*)Omega, (const cplx*)work_a2, (const cplx*)work_p,
+    const int nblk = launch_dense_omega(n, (cplx*)Omega, (const cplx*)work_a2, (const cplx*)work_p, 0.5, 0.5,
                                         std::sqrt(3.0) * tau / 12.0, &ws, st);
     double a = 0.0, b = 0.0;
     rc = read_interval(nblk, &ws, st, &a, &b);

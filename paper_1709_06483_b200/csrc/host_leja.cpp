@@ -163,6 +163,13 @@ int step_coefficients(int scheme, magnus_drive_fn f, void* user, double t, doubl
       }
       return 3;
     }
+    case MAGNUS_M6: {    // the three Gauss nodes; the step driver forms b2, b3 and the nested commutators
+      coef_h1[0] = f(t + (0.5 - s15 / 10.0) * tau, user);
+      coef_h1[1] = f(t + 0.5 * tau, user);
+      coef_h1[2] = f(t + (0.5 + s15 / 10.0) * tau, user);
+      h_scale[0] = 1.0;
+      return 1;
+    }
     default:
       return -1;
   }

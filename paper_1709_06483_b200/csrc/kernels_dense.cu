@@ -76,9 +76,11 @@ __global__ void __launch_bounds__(256) dense_assemble2_kernel(int64_t n, const c
 // through a 32x33 shared-memory tile so that both P reads are coalesced.
 // Block = 32 x 8 threads, owns a strip of 32 rows.
 // ---------------------------------------------------------------------------
+// General form Omega = wa A1 + wb A2 - i kappa (P - P^H): M4 has wa = wb = 1/2; M6 uses it with
+// A1 = H(t2), A2 = H1 and P = L R, see magnus_step.
 __global__ void __launch_bounds__(256) dense_omega_kernel(int64_t n, cplx* __restrict__ A1, const cplx* __restrict__ A2,
-                                                           const cplx* __restrict__ P, double kappa, double* out,
-                                                           unsigned* ticket) {
+                                                           const cplx* __restrict__ P, double wa, double wb,
+                                                           double kappa, double* out, unsigned* ticket) {
   __shared__ cplx tile[32][33];
   const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
   double lo = INFINITY, hi = -INFINITY;
@@ -102,8 +104,8 @@ __global__ void __launch_bounds__(256) dense_omega_kernel(int64_t n, cplx* __res
           const double kx = pij.x - pji.x, ky = pij.y + pji.y;      // K = P - P^H
           const cplx a1 = A1[i * n + j], a2 = A2[i * n + j];
           cplx om;
-          om.x = 0.5 * (a1.x + a2.x) + kappa * ky;                   // -i kappa (kx + i ky) = kappa (ky - i kx)
-          om.y = 0.5 * (a1.y + a2.y) - kappa * kx;
+          om.x = wa * a1.x + wb * a2.x + kappa * ky;                 // -i kappa (kx + i ky) = kappa (ky - i kx)
+          om.y = wa * a1.y + wb * a2.y - kappa * kx;
           A1[i * n + j] = om;
           if (i == j) D[k] = om.x; else R[k] += hypot(om.x, om.y);
         }
@@ -132,9 +134,10 @@ __global__ void __launch_bounds__(256) dense_omega_kernel(int64_t n, cplx* __res
   if (last_block_ticket(ticket)) minmax_finalize_warp0(out, gridDim.x, out + 2 * kMaxPartials);
 }
 
-// K = P - P^H (for the standalone dense commutator entry point).
+// K = P + s P^H, s = -1 (K = P - P^H: the commutator of two Hermitian or two anti-Hermitian factors of P) or
+// s = +1 (the commutator of a Hermitian with an anti-Hermitian factor).
 __global__ void __launch_bounds__(256) dense_antiherm_kernel(int64_t n, const cplx* __restrict__ P,
-                                                              cplx* __restrict__ K) {
+                                                              cplx* __restrict__ K, double s) {
   __shared__ cplx tile[32][33];
   const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
   const int64_t ib = blockIdx.y, jb = blockIdx.x;
@@ -150,7 +153,7 @@ __global__ void __launch_bounds__(256) dense_antiherm_kernel(int64_t n, const cp
     if (i < n && j < n) {
       const cplx pij = P[i * n + j];
       const cplx pji = tile[tx][ty + 8 * k];
-      K[i * n + j] = make_double2(pij.x - pji.x, pij.y + pji.y);
+      K[i * n + j] = make_double2(pij.x + s * pji.x, pij.y - s * pji.y);
     }
   }
 }
@@ -215,6 +218,25 @@ __global__ void __launch_bounds__(DW * 32) dense_leja_iter_kernel(DenseOp op, co
   if (last_block_ticket(ticket)) leja_finalize_warp0(partials, gridDim.x, abs_dk, tol, false, status);   // S7
 }
 
+__global__ void __launch_bounds__(256) dense_lincomb_kernel(int64_t total, cplx* __restrict__ out, LinComb lc) {
+  for (int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (int64_t)gridDim.x * blockDim.x) {
+    cplx acc = make_double2(0.0, 0.0);
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+      if (lc.x[k]) cfma(acc, lc.c[k], lc.x[k][q]);
+    out[q] = acc;
+  }
+}
+
+// one warp per row
+__global__ void __launch_bounds__(256) csr_to_dense_kernel(int64_t n, const int32_t* __restrict__ rp,
+                                                            const int32_t* __restrict__ ci, const cplx* __restrict__ v,
+                                                            cplx* __restrict__ A) {
+  const int64_t row = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
+  if (row >= n) return;
+  for (int q = rp[row] + (threadIdx.x & 31); q < rp[row + 1]; q += 32) A[row * n + ci[q]] = v[q];
+}
+
 // Sampled Hermitian check: pseudo-random (i, j) pairs, largest |M_ij - conj(M_ji)|.
 __global__ void dense_hermitian_check_kernel(DenseOp op, int64_t samples, double* __restrict__ worst) {
   double bad = 0.0;
@@ -264,18 +286,33 @@ void launch_dense_assemble2(int64_t n, const cplx* H0, int64_t ld0, const cplx* 
   ws->launches += 1;
 }
 
-int launch_dense_omega(int64_t n, cplx* A1, const cplx* A2, const cplx* P, double kappa, Workspace* ws,
-                       cudaStream_t st) {
+int launch_dense_omega(int64_t n, cplx* A1, const cplx* A2, const cplx* P, double wa, double wb, double kappa,
+                       Workspace* ws, cudaStream_t st) {
   int64_t g = (n + 31) / 32;
   if (g > kMaxPartials) g = kMaxPartials;
-  dense_omega_kernel<<<(int)g, 256, 0, st>>>(n, A1, A2, P, kappa, ws->gersh, ws->tickets + 1);
+  dense_omega_kernel<<<(int)g, 256, 0, st>>>(n, A1, A2, P, wa, wb, kappa, ws->gersh, ws->tickets + 1);
   ws->launches += 1;
   return (int)g;
 }
 
-void launch_dense_antiherm(int64_t n, const cplx* P, cplx* K, cudaStream_t st) {
+void launch_dense_antiherm(int64_t n, const cplx* P, cplx* K, double s, cudaStream_t st) {
   const unsigned t = (unsigned)((n + 31) / 32);
-  dense_antiherm_kernel<<<dim3(t, t), 256, 0, st>>>(n, P, K);
+  dense_antiherm_kernel<<<dim3(t, t), 256, 0, st>>>(n, P, K, s);
+}
+
+// out = c0 X0 + c1 X1 + c2 X2 + c3 X3, elementwise on n x n row-major matrices (null inputs are skipped)
+void launch_dense_lincomb(int64_t n, cplx* out, LinComb lc, Workspace* ws, cudaStream_t st) {
+  int64_t g = (n * n + 255) / 256;
+  if (g > (int64_t)device_sm_count() * 16) g = (int64_t)device_sm_count() * 16;
+  dense_lincomb_kernel<<<(int)g, 256, 0, st>>>(n * n, out, lc);
+  ws->launches += 1;
+}
+
+// A = CSR matrix written out densely (row-major, zero-filled first)
+void launch_csr_to_dense(int64_t n, const int32_t* rp, const int32_t* ci, const cplx* v, cplx* A, cudaStream_t st) {
+  cudaMemsetAsync(A, 0, sizeof(cplx) * (size_t)n * (size_t)n, st);
+  int64_t g = (n + 7) / 8;
+  csr_to_dense_kernel<<<(int)g, 256, 0, st>>>(n, rp, ci, v, A);
 }
 
 int launch_dense_leja_iter(const DenseOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma, double shift,

@@ -156,11 +156,17 @@ int launch_dense_assemble(int64_t n, const cplx* A, int64_t lda, const cplx* B, 
 // A1 = H0 + f1 H1, A2 = H0 + f2 H1 in one pass
 void launch_dense_assemble2(int64_t n, const cplx* H0, int64_t ld0, const cplx* H1, int64_t ld1, double f1, double f2,
                             cplx* A1, cplx* A2, Workspace* ws, cudaStream_t st);
-// Om = (A1 + A2)/2 - i kappa (P - P^H), written over A1, fused with Gershgorin bounds (row D4)
-int launch_dense_omega(int64_t n, cplx* A1, const cplx* A2, const cplx* P, double kappa, Workspace* ws,
-                       cudaStream_t st);
-// K = P - P^H
-void launch_dense_antiherm(int64_t n, const cplx* P, cplx* K, cudaStream_t st);
+// Om = wa A1 + wb A2 - i kappa (P - P^H), written over A1, fused with Gershgorin bounds (row D4; M4: wa = wb = 1/2)
+int launch_dense_omega(int64_t n, cplx* A1, const cplx* A2, const cplx* P, double wa, double wb, double kappa,
+                       Workspace* ws, cudaStream_t st);
+// K = P + s P^H (s = -1: P - P^H)
+void launch_dense_antiherm(int64_t n, const cplx* P, cplx* K, double s, cudaStream_t st);
+struct LinComb {
+  const cplx* x[4];
+  cplx c[4];
+};
+void launch_dense_lincomb(int64_t n, cplx* out, LinComb lc, Workspace* ws, cudaStream_t st);
+void launch_csr_to_dense(int64_t n, const int32_t* rp, const int32_t* ci, const cplx* v, cplx* A, cudaStream_t st);
 int launch_dense_leja_iter(const DenseOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma, double shift,
                            cplx dk, double abs_dk, double tol, Workspace* ws, cudaStream_t st);
 int dense_hermitian_check(const DenseOp& op, cudaStream_t st, double* max_violation);

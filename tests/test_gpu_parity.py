@@ -463,6 +463,41 @@ def test_m2_cf43_vs_oracle(M, oracle, scheme, name, size, nsteps):
     assert abs(np.linalg.norm(psi) - 1) < 1e-10
 
 
+# ------------------------------------------------------------------ M6 against the oracle
+@pytest.mark.parametrize("name,size,nsteps", [("cfg1", 10, 10), ("cfg3", 12, 3), ("cfg2", 515, 4), ("cfg2", 1024, 2)])
+def test_m6_vs_oracle(M, oracle, name, size, nsteps):
+    """The sixth-order scheme: three DMMA products per step built from Hermitian / anti-Hermitian factors
+    (magnus.h at magnus_step) against the oracle's six plain-definition products; CSR input runs on dense copies
+    on the GPU and as sparse matrices in the oracle.  Identical iteration counts, psi within 1e-9."""
+    cfg = W.scaled(W.CONFIGS[name], size, nsteps)
+    psi, st, ref, riters = run_config(M, oracle, cfg, "m6")
+    assert len(riters) == nsteps
+    assert np.array_equal(st["iters"], riters)
+    assert relerr(psi, ref) <= 1e-9
+    assert abs(np.linalg.norm(psi) - 1) < 1e-10
+
+
+def test_m6_is_more_accurate_than_m4_and_refuses_large_csr(M):
+    """Self-convergence at a coarse step: M6 is far closer to a fine-step solution than M4; CSR input beyond
+    the dense-copy limit is refused with EINVAL instead of running out of memory."""
+    cfg = W.scaled(W.CONFIGS["cfg2"], 256, 4)
+    H0, H1, psi0, f = W.build(cfg, device=DEV)
+    def run(scheme, ns):
+        psi = psi0.clone()
+        with M.magnus_create(H0, H1, f, scheme, tol=1e-13) as h:
+            h.integrate(0.0, 0.4, ns, psi)
+        return psi
+    fine = run("m6", 64)
+    e6 = float(torch.linalg.vector_norm(run("m6", 4) - fine))
+    e4 = float(torch.linalg.vector_norm(run("m4", 4) - fine))
+    assert e6 < 0.1 * e4 and e6 < 1e-6, (e6, e4)
+    big = W.scaled(W.CONFIGS["cfg3"], 15, 1)
+    B0, B1, _, fb = W.build(big, device=DEV)
+    with pytest.raises(M.MagnusError) as ei:
+        M.magnus_create(B0, B1, fb, "m6")
+    assert ei.value.code == -1
+
+
 # ------------------------------------------------------------------ the paper's own workloads (SURVEY 8f-3)
 @pytest.mark.parametrize("scheme", ["cf4", "m4", "cf4:3"])
 def test_paper_example2_local_heisenberg(M, oracle, scheme):
