@@ -84,8 +84,15 @@ typedef struct magnus_options {
                           3 the warp-specialised TMA-ring kernel, 4 the row-block kernel with TMA staging (both need
                           16-byte aligned value and index arrays, else the row-block kernel runs); values >= 1000
                           select tuning variants of these kernels (see the kernel sources) */
-  int32_t reserved;
+  int32_t shortcuts;   /* bit mask of beyond-paper shortcuts, default 0 = the mandated path only:
+                          MAGNUS_SHORTCUT_CACHED_COMMUTATOR (dense M4) */
 } magnus_options;
+
+/* Shortcut (reported separately from the mandated path): for H(t) = H0 + f(t) H1 the commutator of
+ * an M4 step is [H(t2), H(t1)] = (f1 - f2) [H0, H1], so on dense H the product P0 = H0 H1 is formed ONCE in
+ * magnus_create and a step assembles Omega_H = H0 + fbar H1 - i kappa (P0 - P0^H) without any GEMM (the paper
+ * recomputes A2 A1 and A1 A2 every step, P:262 l.6-7; the CSR path always caches [H0, H1], row S0). */
+#define MAGNUS_SHORTCUT_CACHED_COMMUTATOR 1
 
 /* What one exponential did (reading c4-c7). */
 typedef struct magnus_expmv_info {

@@ -36,7 +36,7 @@ class MatrixStruct(C.Structure):
 
 class Options(C.Structure):
     _fields_ = [("tol", C.c_double), ("theta_max", C.c_double), ("m_max", C.c_int32), ("check_hermitian", C.c_int32),
-                ("stream", C.c_void_p), ("csr_kernel", C.c_int32), ("reserved", C.c_int32)]
+                ("stream", C.c_void_p), ("csr_kernel", C.c_int32), ("shortcuts", C.c_int32)]
 
 
 class ExpmvInfo(C.Structure):
@@ -177,7 +177,11 @@ def _drive(f: Callable[[float], float]):
     return DRIVE(lambda t, _user: float(f(t)))
 
 
-def _options(tol=None, theta_max=None, m_max=None, check_hermitian=False, stream=None, csr_kernel=0) -> Options:
+SHORTCUT_CACHED_COMMUTATOR = 1
+
+
+def _options(tol=None, theta_max=None, m_max=None, check_hermitian=False, stream=None, csr_kernel=0,
+             shortcuts=0) -> Options:
     o = Options()
     o.tol = tol or 0.0
     o.theta_max = theta_max or 0.0
@@ -185,6 +189,7 @@ def _options(tol=None, theta_max=None, m_max=None, check_hermitian=False, stream
     o.check_hermitian = 1 if check_hermitian else 0
     o.stream = _stream_ptr(stream)
     o.csr_kernel = csr_kernel
+    o.shortcuts = shortcuts
     return o
 
 

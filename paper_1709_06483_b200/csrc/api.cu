@@ -248,7 +248,9 @@ static int expmv_on_interval(const OpRef& op, double a_raw, double b_raw, const 
   return MAGNUS_OK;
 }
 
-static void default_params(const magnus_options* opt, LejaParams* prm, cudaStream_t* st, int* csr_kernel) {
+static void default_params(const magnus_options* opt, LejaParams* prm, cudaStream_t* st, int* csr_kernel,
+                           int* shortcuts) {
+  *shortcuts = opt ? opt->shortcuts : 0;
   prm->tol = (opt && opt->tol > 0.0) ? opt->tol : 1e-12;
   prm->theta_max = (opt && opt->theta_max > 0.0) ? opt->theta_max : 16.0;
   prm->m_max = (opt && opt->m_max > 0 && opt->m_max <= kMaxDegree) ? opt->m_max : kMaxDegree;
@@ -263,6 +265,8 @@ using namespace magnus;
 struct magnus_context {
   int scheme = 0;
   int format = 0;
+  int shortcuts = 0;
+  bool cached_p0 = false;      // dense M4 shortcut: h->P holds P0 = H0 H1
   int64_t n = 0;
   magnus_matrix H0, H1;
   magnus_drive_fn f = nullptr;
@@ -439,7 +443,7 @@ int magnus_create(magnus_handle* out, const magnus_matrix* H0, const magnus_matr
   h->H1 = *H1;
   h->f = f;
   h->user = user;
-  default_params(opt, &h->prm, &h->stream, &h->ws.csr_kernel);
+  default_params(opt, &h->prm, &h->stream, &h->ws.csr_kernel, &h->shortcuts);
   const int csr_kernel = h->ws.csr_kernel;
   rc = workspace_alloc(&h->ws, h->n);
   h->ws.csr_kernel = csr_kernel;
@@ -508,6 +512,17 @@ int magnus_create(magnus_handle* out, const magnus_matrix* H0, const magnus_matr
       cudaEventCreate(&h->ev_comm[0]);
       cudaEventCreate(&h->ev_comm[1]);
       h->time_comm = true;
+    }
+    if (scheme == MAGNUS_M4 && (h->shortcuts & MAGNUS_SHORTCUT_CACHED_COMMUTATOR)) {
+      if (dense_ld(H0) != h->n || dense_ld(H1) != h->n) {
+        set_error("MAGNUS_SHORTCUT_CACHED_COMMUTATOR needs ld == n");
+        magnus_destroy(h);
+        return MAGNUS_EINVAL;
+      }
+      rc = launch_zgemm(h->n, (const cplx*)H0->values, h->n, (const cplx*)H1->values, h->n, h->P, h->n, h->stream);
+      if (rc) { set_error("zgemm launch failed: %s", cudaGetErrorString(cudaGetLastError())); magnus_destroy(h); return rc; }
+      h->cached_p0 = true;
+      h->time_comm = false;
     }
   } else if (scheme == MAGNUS_M4) {
     int64_t nnz = 0;
@@ -603,6 +618,14 @@ int magnus_step(magnus_handle h, double t, double tau, void* psi_, magnus_step_i
         if (rc) break;
         // Omega_H = H2 + (b3/(12 tau)) H1 + (i/(240 tau)) (P3 - P3^H), over X1, with its Gershgorin bounds
         nblk = launch_dense_omega(n, h->M, H1v, h->X4, 1.0, b3 / (12.0 * tau), -1.0 / (240.0 * tau), ws, st);
+      } else if (h->scheme == MAGNUS_M4 && h->cached_p0) {
+        // shortcut: Omega_H = H0 + fbar H1 - i kappa (P0 - P0^H), kappa = (sqrt(3) tau/12)(f1 - f2), no GEMM
+        LinComb lc;
+        lc.x[0] = H0v; lc.c[0] = make_double2(1.0, 0.0);
+        lc.x[1] = H1v; lc.c[1] = make_double2(0.5 * (coef[0] + coef[1]), 0.0);
+        lc.x[2] = lc.x[3] = nullptr; lc.c[2] = lc.c[3] = make_double2(0.0, 0.0);
+        launch_dense_lincomb(h->n, h->M, lc, ws, st);
+        nblk = launch_dense_omega(h->n, h->M, H1v, h->P, 1.0, 0.0, kappa, ws, st);
       } else if (h->scheme == MAGNUS_M4) {
         launch_dense_assemble2(h->n, H0v, dense_ld(&h->H0), H1v, dense_ld(&h->H1), coef[0], coef[1], h->M, h->A2, ws,
                                st);                                                                // S2: A1, A2

@@ -498,6 +498,28 @@ def test_m6_is_more_accurate_than_m4_and_refuses_large_csr(M):
     assert ei.value.code == -1
 
 
+# ------------------------------------------------------------------ shortcut: cached dense commutator
+@pytest.mark.parametrize("n,nsteps", [(200, 5), (515, 3), (2048, 2)])
+def test_shortcut_cached_dense_commutator_vs_oracle(M, oracle, n, nsteps):
+    """Dense M4 with P0 = H0 H1 formed once at create ([H(t2), H(t1)] = (f1 - f2)[H0, H1]) against the oracle's
+    per-step plain-definition commutator: identical counts and interval, psi within 1e-9; and it agrees with the
+    mandated per-step-GEMM path of the library to rounding."""
+    cfg = W.scaled(W.CONFIGS["cfg2"], n, nsteps)
+    H0, H1, psi0, f = W.build(cfg)
+    ref, riters = oracle.magnus_integrate(H0.numpy(), H1.numpy(), f, "m4", cfg.t0, cfg.t_end, nsteps, psi0.numpy(), cfg.tol)
+    d0, d1 = H0.to(DEV), H1.to(DEV)
+    out = {}
+    for sc in (0, M.SHORTCUT_CACHED_COMMUTATOR):
+        psi = psi0.to(DEV).clone()
+        with M.magnus_create(d0, d1, f, "m4", tol=cfg.tol, shortcuts=sc) as h:
+            st = h.integrate(cfg.t0, cfg.t_end, nsteps, psi)
+        assert np.array_equal(st["iters"], riters)
+        assert relerr(host(psi), ref) <= 1e-9
+        out[sc] = (host(psi), st)
+    assert relerr(out[1][0], out[0][0]) <= 1e-12
+    assert out[1][1]["seconds_commutator"] == 0.0 and out[0][1]["seconds_commutator"] > 0.0
+
+
 # ------------------------------------------------------------------ the paper's own workloads (SURVEY 8f-3)
 @pytest.mark.parametrize("scheme", ["cf4", "m4", "cf4:3"])
 def test_paper_example2_local_heisenberg(M, oracle, scheme):
