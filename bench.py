@@ -439,6 +439,25 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_sweep(args):
+    """The paper's sweeps (paper_1709_06483_b200/sweeps.py) with the oracle timed beside the sizes it affords."""
+    from paper_1709_06483_b200 import sweeps
+    from oracle import oracle as O
+
+    def cpu_timer(example, N, H0, H1, psi0, f, tau, tol):
+        o0 = H0.cpu().numpy() if example == 1 else O.CsrHost.of(H0)
+        o1 = H1.cpu().numpy() if example == 1 else O.CsrHost.of(H1)
+        if N <= 10:   # untimed first call: the OpenMP team starts up
+            O.magnus_step(o0, o1, f, "cf4", 0.0, tau, psi0.cpu().numpy(), tol)
+        t0 = time.perf_counter()
+        O.magnus_step(o0, o1, f, "cf4", 0.0, tau, psi0.cpu().numpy(), tol)
+        return time.perf_counter() - t0
+
+    cmd = f"python bench.py --sweep {args.sweep}{' --sweep-quick' if args.sweep_quick else ''}"
+    lines = sweeps.run_all(args.sweep, cpu_timer, args.sweep_quick, cmd + f" (oracle: {O.num_threads()} host threads)")
+    print("\n".join(lines))
+
+
 def matrix_bytes_cfg(cfg):
     if cfg.kind == "xxz":
         return 20 * (1 << cfg.size) * (3 * cfg.size + 2) // 2
@@ -456,12 +475,18 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extra", action="store_true", help="skip the cfg4 secondary measurements of the default run")
+    ap.add_argument("--sweep", default=None, metavar="FILE.md",
+                    help="instead of the benchmark line: re-run the paper's cost-vs-size and accuracy-vs-cost sweeps "
+                         "(PAPER.md section 4) and write the tables to FILE.md")
+    ap.add_argument("--sweep-quick", action="store_true")
     ap.add_argument("--oracle-steps", type=int, default=None,
                     help="reference arm: Magnus steps of the oracle to time (default 1: a step is tens of seconds)")
     ap.add_argument("--oracle-max-size", type=int, default=None,
                     help="cap N (xxz) or n (dense) of the oracle's bounded sample")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.sweep:
+        run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
