@@ -291,6 +291,7 @@ struct magnus_context {
   // CSR: cached per-term row statistics for the Gershgorin bounds (valid while the terms' patterns are disjoint)
   double* gs_r[3] = {nullptr, nullptr, nullptr};
   cplx* gs_diag[3] = {nullptr, nullptr, nullptr};
+  SliceLayout slice;           // CSR: slice-major copy of (H0, H1[, C]) for the slice kernel (csr_kernel 5)
   bool gs_disjoint2 = false;   // H0, H1 share no (row, column)
   bool gs_disjoint3 = false;   // H0, H1, C share none either
   int unit_cap2 = 0, unit_cap3 = 0;   // stream kernel: largest 32-row unit of (H0, H1) and of (H0, H1, C)
@@ -400,6 +401,7 @@ int magnus_host_step_coefficients(int scheme, magnus_drive_fn f, void* user, dou
 int magnus_destroy(magnus_handle h) {
   if (!h) return MAGNUS_OK;
   workspace_free(&h->ws);
+  slice_layout_free(&h->slice);
   cudaFree(h->M);
   cudaFree(h->A2);
   cudaFree(h->P);
@@ -533,6 +535,22 @@ int magnus_create(magnus_handle* out, const magnus_matrix* H0, const magnus_matr
   if (h->format == MAGNUS_CSR) {
     rc = csr_cache_rowstats(h);
     if (rc) { magnus_destroy(h); return rc; }
+    if (csr_kernel == 5 || (csr_kernel >= 5000 && csr_kernel < 6000)) {
+      CsrOp op;
+      op.n = h->n;
+      op.unit_cap = 0;
+      op.nterms = (scheme == MAGNUS_M4 && h->c_nnz > 0) ? 3 : 2;
+      op.t[0] = csr_term(&h->H0, 1.0, 0.0);
+      op.t[1] = csr_term(&h->H1, 1.0, 0.0);
+      op.t[2] = op.t[1];
+      if (op.nterms == 3) {
+        op.t[2].rp = h->c_rp;
+        op.t[2].ci = h->c_ci;
+        op.t[2].v = h->c_v;
+        op.t[2].nnz = h->c_nnz;
+      }
+      slice_layout_build(op, &h->slice, h->stream);   // on failure the CSR kernels run
+    }
   }
   if (cudaStreamSynchronize(h->stream) != cudaSuccess) { magnus_destroy(h); return MAGNUS_ECUDA; }
   *out = h;
@@ -576,6 +594,7 @@ int magnus_step(magnus_handle h, double t, double tau, void* psi_, magnus_step_i
         op.csr.t[2] = op.csr.t[1];
       }
       op.csr.unit_cap = op.csr.nterms == 3 ? h->unit_cap3 : h->unit_cap2;
+      op.csr.slice = h->slice.meta ? &h->slice : nullptr;
       if ((op.csr.nterms == 2 && h->gs_disjoint2) || (op.csr.nterms == 3 && h->gs_disjoint3)) {     // S3
         const int nblk = launch_csr_gershgorin_cached(op.csr, h->gs_r, h->gs_diag, ws, st);
         rc = read_interval(nblk, ws, st, &a, &b);
@@ -798,7 +817,7 @@ int magnus_integrate_host(const magnus_matrix* H0_host, const magnus_matrix* H1_
 
 // ---- single kernels -----------------------------------------------------------------
 static int build_op(const magnus_matrix* H0, const magnus_matrix* H1, double g, OpRef* op, cplx** tmpM, Workspace* ws,
-                    cudaStream_t st, int* assemble_blocks) {
+                    cudaStream_t st, int* assemble_blocks, SliceLayout* tmpS = nullptr) {
   *tmpM = nullptr;
   *assemble_blocks = -1;
   if (H0->format == MAGNUS_CSR) {
@@ -810,6 +829,7 @@ static int build_op(const magnus_matrix* H0, const magnus_matrix* H1, double g, 
     op->csr.t[2] = op->csr.t[0];
     op->csr.unit_cap = 0;
     if (csr_unit_cap(op->csr, st, &op->csr.unit_cap) != MAGNUS_OK) op->csr.unit_cap = 0;
+    if (tmpS && (ws->csr_kernel == 5 || (ws->csr_kernel >= 5000 && ws->csr_kernel < 6000)) && slice_layout_build(op->csr, tmpS, st) == MAGNUS_OK) op->csr.slice = tmpS;
   } else {
     op->dense = true;
     op->dns.n = H0->n;
@@ -872,8 +892,9 @@ int magnus_leja_iteration(const magnus_matrix* H0, const magnus_matrix* H1, doub
   ws.csr_kernel = csr_kernel;
   OpRef op;
   cplx* tmp = nullptr;
+  SliceLayout tmp_slice;
   int ab = -1;
-  rc = build_op(H0, H1, g, &op, &tmp, &ws, st, &ab);
+  rc = build_op(H0, H1, g, &op, &tmp, &ws, st, &ab, &tmp_slice);
   if (rc == MAGNUS_OK) {
     cudaMemsetAsync(ws.status, 0, sizeof(LejaStatus), st);
     cudaEventRecord(ws.ev[0], st);
@@ -898,6 +919,7 @@ int magnus_leja_iteration(const magnus_matrix* H0, const magnus_matrix* H1, doub
     }
   }
   cudaFree(tmp);
+  slice_layout_free(&tmp_slice);
   workspace_free(&ws);
   return rc;
 }

@@ -1,0 +1,452 @@
+// S6 -- fused Leja iteration on a SLICE-MAJOR copy of the CSR operator (csr_kernel = 5).
+//
+// The row-block kernel (kernels_csr_rowblock.cu) streams the CSR range of 32 rows into shared
+// memory so that a lane can walk "its" row while the warp's global reads stay coalesced; ncu shows
+// it limited by what fits into shared memory between request and last use (profiles/
+// r2_csr_kernel_study.md).  Here the handle owns a re-ordered copy of the operator, built once
+// in magnus_create, in which the coalesced order IS the storage order, so the kernel needs no
+// staging at all and the register file holds what is in flight:
+//
+//   * a SLICE is 32 consecutive rows; the entries of all terms (H0, H1 and, for M4, C = [H0,H1])
+//     of a slice are stored together, term after term;
+//   * inside a term the entries of a slice are grouped into SLOTS.  A slot holds at most one
+//     entry per row, all with the same diagonal offset (column - row): the slots of a slice are
+//     found by a 32-way merge of its rows on that key.  A slot is stored as a 32-bit row mask
+//     plus its entries packed in row order, values and columns in two parallel arrays -- no
+//     padding, 20 bytes per stored entry exactly as in CSR;
+//   * lane l of the warp that owns the slice is row l.  For a slot with mask m it reads entry
+//     popc(m & lanes below l): active lanes read consecutive addresses (128-bit values, 32-bit
+//     columns), and because all entries of a slot share col - row, the gather of w touches one
+//     contiguous piece of w (on the spin chains col = row XOR mask: col - row is +-mask).
+//
+// The warp runs a software pipeline over the slots of its slices, eight at a time: the column
+// indices of batch b+1 are requested while the values and the w-gathers of batch b are in
+// flight, across term and slice boundaries (the next 32 slot masks are prefetched too).
+// Per-iteration HBM traffic: 20 B per stored entry + 64 B per row (w, w+, p) + 4 B per slot and
+// 24 B per slice of bookkeeping (instead of CSR's 4 B per row and term of row pointers).
+// Deterministic: fixed row -> lane map, per-row sums in slot order (ascending col - row inside a
+// term), fixed reduction trees.  The summation order differs from CSR order by a permutation
+// inside a row, so results agree with the other kernels to rounding, not bit for bit.
+#include "magnus_internal.h"
+#include "device_utils.cuh"
+#include "leja_finalize.cuh"
+
+#include <climits>
+
+namespace magnus {
+
+namespace {
+
+constexpr int SL_WARPS = 4;     // warps per CTA
+constexpr int SL_PAD = 8;       // the slots of every term of a slice are padded (zero masks) to a multiple of this
+constexpr int SL_CAP = 512;     // slots of one slice the per-warp mask buffer holds; a layout with a larger slice is refused
+
+struct SliceView {
+  int64_t n, nslices;
+  const int4* meta;            // per slice: {first slot (global), slots, first slot of term 1, of term 2 (slice-relative)}
+  const int64_t* ent_ptr;      // [nslices + 1] first entry of the slice in ci / v
+  const unsigned* slot_mask;
+  const int32_t* ci;
+  const cplx* v;
+  cplx coef[3];
+};
+
+// Predicated loads whose destination is preset inside the asm block: the compiler sees one producer, so the
+// load stays asynchronous (a C++ "x = ok ? load : 0" becomes load + select and the select waits for the load).
+// No L2 cache-policy operand: it has to sit in a uniform register and cost two R2UR per load (ncu), and the
+// evict-first hint made no difference on this workload (profiles/r2_csr_kernel_study.md).
+__device__ __forceinline__ cplx ld_stream_if(const cplx* p, unsigned ok) {
+  cplx r;
+  asm("{\n .reg .pred q;\n setp.ne.b32 q, %3, 0;\n mov.f64 %0, 0d0000000000000000;\n mov.f64 %1, 0d0000000000000000;\n"
+      " @q ld.global.nc.L1::no_allocate.v2.f64 {%0, %1}, [%2];\n}"
+      : "=d"(r.x), "=d"(r.y)
+      : "l"(p), "r"(ok));
+  return r;
+}
+// column index, or `other` (the lane's own row: a harmless gather target) for a lane without an entry in the slot
+__device__ __forceinline__ int ld_stream_i32_if(const int32_t* p, unsigned ok, int other) {
+  int r;
+  asm("{\n .reg .pred q;\n setp.ne.b32 q, %2, 0;\n mov.b32 %0, %3;\n"
+      " @q ld.global.nc.L1::no_allocate.s32 %0, [%1];\n}"
+      : "=r"(r)
+      : "l"(p), "r"(ok), "r"(other));
+  return r;
+}
+
+struct SliceDesc {
+  unsigned eb;  // first entry of the slice (the layout is refused beyond 2^32 stored entries)
+  int sb;       // first slot of the slice in slot_mask
+  int ns;       // slots (padded: a multiple of SL_PAD, at least SL_PAD)
+  int b1, b2;   // first slot of term 1 / of term 2
+};
+
+// per-warp buffer of a slice's slots: .x = row mask (arrives by cp.async), .y = entries of the slice before the slot
+__device__ __forceinline__ void stage_masks(const SliceView& L, const SliceDesc& D, uint2* buf, int lane) {
+  const unsigned* __restrict__ src = L.slot_mask + D.sb;
+#pragma unroll 1
+  for (int k = lane; k < D.ns; k += 32) {
+    const unsigned dst = (unsigned)__cvta_generic_to_shared(&buf[k].x);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst), "l"(src + k) : "memory");
+  }
+}
+// after the masks have landed: running entry offsets, 32 slots per warp scan
+__device__ __forceinline__ void scan_masks(uint2* buf, int ns, int lane) {
+  int run = 0;
+  for (int k0 = 0; k0 < ns; k0 += 32) {
+    const int k = k0 + lane;
+    const int cnt = k < ns ? __popc(buf[k].x) : 0;
+    int inc = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int up = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= o) inc += up;
+    }
+    if (k < ns) buf[k].y = (unsigned)(run + inc - cnt);
+    run += __shfl_sync(0xffffffffu, inc, 31);
+  }
+  __syncwarp();
+}
+
+// C stage: column indices of the SL_U slots whose masks start at mk; run = entries of the slice before them
+template <int SL_U>
+__device__ __forceinline__ void issue_cols(const int32_t* __restrict__ ci, unsigned eb, const uint2* mk, unsigned lbit,
+                                           unsigned lt, int row, int (&cn)[SL_U]) {
+#pragma unroll
+  for (int u = 0; u < SL_U; u += 2) {
+    const uint4 q = *reinterpret_cast<const uint4*>(mk + u);   // two slots: {mask, start, mask, start}
+    cn[u] = ld_stream_i32_if(ci + (eb + q.y + __popc(q.x & lt)), q.x & lbit, row);
+    cn[u + 1] = ld_stream_i32_if(ci + (eb + q.w + __popc(q.z & lt)), q.z & lbit, row);
+  }
+}
+
+// SL_U slots per batch, MINB resident CTAs per SM (register budget 65536 / (128 MINB) per thread)
+template <int SL_U, int MINB>
+__global__ void __launch_bounds__(SL_WARPS * 32, MINB)
+    csr_leja_iter_slice_kernel(SliceView L, const cplx* __restrict__ w_in, cplx* __restrict__ w_out,
+                               cplx* __restrict__ p, double inv_gamma, double shift, cplx dk, double abs_dk,
+                               double tol, LejaStatus* status, double* partials, unsigned* ticket) {
+  if (status->done) return;
+  __shared__ __align__(16) uint2 s_mask[SL_WARPS][2][SL_CAP];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const unsigned lbit = 1u << lane, lt = lbit - 1u;
+  const int stride = (int)gridDim.x * SL_WARPS, nslices = (int)L.nslices;
+  double sw = 0.0, sp = 0.0;
+
+  int s0 = (int)blockIdx.x * SL_WARPS + warp;   // slice in the V stage
+  if (s0 < nslices) {
+    auto load_desc = [&](int s, SliceDesc& D) {
+      const int4 m = __ldg(L.meta + s);
+      D.eb = (unsigned)__ldg(L.ent_ptr + s);
+      D.sb = m.x;
+      D.ns = m.y;
+      D.b1 = m.z;
+      D.b2 = m.w;
+    };
+    auto own_row = [&](int s) { return (int)min(((int64_t)s << 5) + lane, L.n - 1); };
+    SliceDesc D0, D1, D2;   // current slice, next, the one after (its masks are not staged yet)
+    int cb = 0;             // D0's masks are in s_mask[warp][cb], D1's in the other buffer
+    load_desc(s0, D0);
+    stage_masks(L, D0, s_mask[warp][0], lane);
+    bool have1 = s0 + stride < nslices, have2 = s0 + 2 * stride < nslices;
+    D1 = D0;
+    D2 = D0;
+    if (have1) {
+      load_desc(s0 + stride, D1);
+      stage_masks(L, D1, s_mask[warp][1], lane);
+    }
+    if (have2) load_desc(s0 + 2 * stride, D2);
+    cp_async_wait_all();
+    __syncwarp();
+    scan_masks(s_mask[warp][0], D0.ns, lane);
+    if (have1) scan_masks(s_mask[warp][1], D1.ns, lane);
+
+    int cn[SL_U];
+    int j = 0;
+    bool fresh1 = have1;   // D1's buffer is already scanned (only before the first slice switch)
+    issue_cols<SL_U>(L.ci, D0.eb, s_mask[warp][0], lbit, lt, own_row(s0), cn);
+    cplx a = make_double2(0.0, 0.0), y = a, wi = a, pi = a;
+    int term = 0;
+    {
+      const int64_t row = ((int64_t)s0 << 5) + lane;
+      if (row < L.n) {
+        wi = w_in[row];
+        pi = p[row];
+      }
+    }
+    while (true) {
+      // ---- V stage: values and w-gathers of slots j .. j+U-1 of D0
+      const uint2* mv = s_mask[warp][cb] + j;
+      cplx v[SL_U], x[SL_U];
+#pragma unroll
+      for (int u = 0; u < SL_U; u += 2) {
+        const uint4 q = *reinterpret_cast<const uint4*>(mv + u);
+        v[u] = ld_stream_if(L.v + (D0.eb + q.y + __popc(q.x & lt)), q.x & lbit);
+        x[u] = w_in[cn[u]];   // a lane without an entry gathers its own row's w against v = 0
+        v[u + 1] = ld_stream_if(L.v + (D0.eb + q.w + __popc(q.z & lt)), q.z & lbit);
+        x[u + 1] = w_in[cn[u + 1]];
+      }
+      // ---- C stage: columns of the next batch (same slice, or the first batch of the next one)
+      const int jn = j + SL_U;
+      const bool last = jn >= D0.ns;
+      if (!last) {
+        issue_cols<SL_U>(L.ci, D0.eb, s_mask[warp][cb] + jn, lbit, lt, own_row(s0), cn);
+      } else if (have1) {
+        if (!fresh1) {           // D1's masks were requested a slice ago
+          cp_async_wait_all();
+          __syncwarp();
+          scan_masks(s_mask[warp][cb ^ 1], D1.ns, lane);
+        }
+        fresh1 = false;
+        issue_cols<SL_U>(L.ci, D1.eb, s_mask[warp][cb ^ 1], lbit, lt, own_row(s0 + stride), cn);
+      }
+      // ---- the batch belongs to one term (terms are padded to whole batches)
+      const int tnow = (j >= D0.b1) + (j >= D0.b2);
+      if (tnow != term) {
+        cfma(y, L.coef[term], a);
+        a = make_double2(0.0, 0.0);
+        term = tnow;
+      }
+#pragma unroll
+      for (int u = 0; u < SL_U; ++u) cfma(a, v[u], x[u]);
+      j = jn;
+      if (last) {
+        // finish the rows of the slice
+        cfma(y, L.coef[term], a);
+        const int64_t row = ((int64_t)s0 << 5) + lane;
+        if (row < L.n) {
+          cplx wn;
+          wn.x = inv_gamma * y.x - shift * wi.x;
+          wn.y = inv_gamma * y.y - shift * wi.y;
+          cfma(pi, dk, wn);
+          w_out[row] = wn;
+          p[row] = pi;
+          sw += wn.x * wn.x + wn.y * wn.y;
+          sp += pi.x * pi.x + pi.y * pi.y;
+        }
+        if (!have1) break;
+        s0 += stride;
+        D0 = D1;
+        D1 = D2;
+        have1 = have2;
+        have2 = s0 + 2 * stride < nslices;
+        __syncwarp();   // every lane is done with the old D0's masks
+        if (have1) stage_masks(L, D1, s_mask[warp][cb], lane);
+        cb ^= 1;
+        if (have2) load_desc(s0 + 2 * stride, D2);
+        j = 0;
+        term = 0;
+        a = make_double2(0.0, 0.0);
+        y = a;
+        const int64_t nrow = ((int64_t)s0 << 5) + lane;
+        if (nrow < L.n) {
+          wi = w_in[nrow];
+          pi = p[nrow];
+        }
+      }
+    }
+  }
+  block_reduce_sum2<SL_WARPS * 32>(sw, sp);
+  if (threadIdx.x == 0) {
+    partials[2 * blockIdx.x] = sw;
+    partials[2 * blockIdx.x + 1] = sp;
+  }
+  if (last_block_ticket(ticket)) leja_finalize_warp0(partials, gridDim.x, abs_dk, tol, false, status);   // S7
+}
+
+// ---- building the layout (once per handle) ------------------------------------------------
+// 32-way merge of the rows of a slice on key = column - row (ascending inside a CSR row).
+// FILL = false: count slots and entries per slice; FILL = true: write masks and packed entries.
+template <bool FILL>
+__global__ void __launch_bounds__(128)
+    slice_merge_kernel(CsrOp op, int64_t nslices, int4* meta, int64_t* ent_ptr, unsigned* slot_mask, int32_t* ci_out,
+                       cplx* v_out) {
+  const int lane = threadIdx.x & 31;
+  const unsigned lt = (1u << lane) - 1u;
+  const int64_t s = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (s >= nslices) return;
+  const int64_t row = (s << 5) + lane;
+  const bool valid = row < op.n;
+  int nslots = 0, b[3] = {0, 0, 0};
+  int64_t ents = 0;
+  int sb = 0;
+  int64_t eb = 0;
+  if (FILL) {
+    sb = meta[s].x;
+    eb = ent_ptr[s];
+  }
+#pragma unroll
+  for (int t = 0; t < 3; ++t) {
+    b[t] = nslots;
+    if (t >= op.nterms) continue;
+    const int32_t* __restrict__ ci = op.t[t].ci;
+    const cplx* __restrict__ vv = op.t[t].v;
+    int cur = valid ? op.t[t].rp[row] : 0;
+    const int end = valid ? op.t[t].rp[row + 1] : 0;
+    int col = cur < end ? ci[cur] : 0;
+    int key = cur < end ? col - (int)row : INT_MAX;
+    while (true) {
+      const int kmin = __reduce_min_sync(0xffffffffu, key);
+      if (kmin == INT_MAX) break;
+      const bool hit = key == kmin;
+      const unsigned m = __ballot_sync(0xffffffffu, hit);
+      if (FILL) {
+        if (lane == 0) slot_mask[sb + nslots] = m;
+        if (hit) {
+          const int64_t q = eb + ents + __popc(m & lt);
+          ci_out[q] = col;
+          v_out[q] = vv[cur];
+        }
+      }
+      ents += __popc(m);
+      nslots += 1;
+      if (hit) {
+        cur += 1;
+        col = cur < end ? ci[cur] : 0;
+        key = cur < end ? col - (int)row : INT_MAX;
+      }
+    }
+    nslots = (nslots + SL_PAD - 1) / SL_PAD * SL_PAD;   // whole batches per term; the padding masks stay zero
+  }
+  if (nslots == 0) nslots = SL_PAD;
+  if (!FILL && lane == 0) {
+    meta[s] = make_int4(0, nslots, op.nterms > 1 ? b[1] : nslots, op.nterms > 2 ? b[2] : nslots);
+    ent_ptr[s] = ents;
+  }
+}
+
+// exclusive prefix sums of the slot and entry counts (one CTA; nslices is at most a few million)
+__global__ void __launch_bounds__(1024) slice_scan_kernel(int64_t nslices, int4* meta, int64_t* ent_ptr, int64_t* totals) {
+  __shared__ int64_t s_slots[1024], s_ents[1024];
+  __shared__ int s_max[1024];
+  const int tid = threadIdx.x;
+  const int64_t per = (nslices + 1023) / 1024;
+  const int64_t lo = min(nslices, (int64_t)tid * per), hi = min(nslices, lo + per);
+  int64_t ns = 0, ne = 0;
+  int mx = 0;
+  for (int64_t s = lo; s < hi; ++s) {
+    ns += meta[s].y;
+    mx = max(mx, meta[s].y);
+    ne += ent_ptr[s];
+  }
+  s_slots[tid] = ns;
+  s_ents[tid] = ne;
+  s_max[tid] = mx;
+  __syncthreads();
+  if (tid == 0) {
+    int64_t as = 0, ae = 0;
+    for (int i = 0; i < 1024; ++i) {
+      const int64_t cs = s_slots[i], ce = s_ents[i];
+      s_slots[i] = as;
+      s_ents[i] = ae;
+      as += cs;
+      ae += ce;
+      mx = max(mx, s_max[i]);
+    }
+    totals[0] = as;
+    totals[1] = ae;
+    totals[2] = mx;
+    ent_ptr[nslices] = ae;
+  }
+  __syncthreads();
+  ns = s_slots[tid];
+  ne = s_ents[tid];
+  for (int64_t s = lo; s < hi; ++s) {
+    const int cnt = meta[s].y;
+    const int64_t ce = ent_ptr[s];
+    meta[s].x = (int)ns;
+    ent_ptr[s] = ne;
+    ns += cnt;
+    ne += ce;
+  }
+}
+
+}  // namespace
+
+void slice_layout_free(SliceLayout* L) {
+  if (!L) return;
+  cudaFree(L->meta);
+  cudaFree(L->ent_ptr);
+  cudaFree(L->slot_mask);
+  cudaFree(L->ci);
+  cudaFree(L->v);
+  *L = SliceLayout();
+}
+
+// Returns MAGNUS_OK and a filled layout, or an error code with *out left empty (callers fall back to
+// the CSR kernels: the layout is an optimisation, never a requirement).  Synchronises the stream once.
+int slice_layout_build(const CsrOp& op, SliceLayout* out, cudaStream_t st) {
+  *out = SliceLayout();
+  SliceLayout L;
+  L.n = op.n;
+  L.nslices = (op.n + 31) >> 5;
+  L.nterms = op.nterms;
+  int64_t* totals = nullptr;
+  int64_t host_totals[3] = {0, 0, 0};
+  bool ok = cudaMalloc(&L.meta, sizeof(int4) * (size_t)L.nslices) == cudaSuccess &&
+            cudaMalloc(&L.ent_ptr, sizeof(int64_t) * (size_t)(L.nslices + 1)) == cudaSuccess &&
+            cudaMalloc(&totals, 3 * sizeof(int64_t)) == cudaSuccess;
+  if (ok) {
+    const int64_t blocks = (L.nslices * 32 + 127) / 128;
+    slice_merge_kernel<false><<<(unsigned)blocks, 128, 0, st>>>(op, L.nslices, L.meta, L.ent_ptr, nullptr, nullptr, nullptr);
+    slice_scan_kernel<<<1, 1024, 0, st>>>(L.nslices, L.meta, L.ent_ptr, totals);
+    ok = cudaMemcpyAsync(host_totals, totals, sizeof host_totals, cudaMemcpyDeviceToHost, st) == cudaSuccess &&
+         cudaStreamSynchronize(st) == cudaSuccess;
+  }
+  if (ok) ok = host_totals[0] < ((int64_t)1 << 31) && host_totals[2] <= SL_CAP && host_totals[1] < ((int64_t)1 << 32);
+  if (ok) {
+    L.nslots = host_totals[0];
+    L.nent = host_totals[1];
+    ok = cudaMalloc(&L.slot_mask, sizeof(unsigned) * (size_t)(L.nslots > 0 ? L.nslots : 1)) == cudaSuccess &&
+         cudaMalloc(&L.ci, sizeof(int32_t) * (size_t)(L.nent > 0 ? L.nent : 1)) == cudaSuccess &&
+         cudaMalloc(&L.v, sizeof(cplx) * (size_t)(L.nent > 0 ? L.nent : 1)) == cudaSuccess;
+  }
+  if (ok) ok = cudaMemsetAsync(L.slot_mask, 0, sizeof(unsigned) * (size_t)(L.nslots > 0 ? L.nslots : 1), st) == cudaSuccess;
+  if (ok) {
+    const int64_t blocks = (L.nslices * 32 + 127) / 128;
+    slice_merge_kernel<true><<<(unsigned)blocks, 128, 0, st>>>(op, L.nslices, L.meta, L.ent_ptr, L.slot_mask, L.ci, L.v);
+    ok = cudaGetLastError() == cudaSuccess;
+  }
+  cudaFree(totals);
+  if (!ok) {
+    cudaGetLastError();
+    slice_layout_free(&L);
+    return MAGNUS_ENOMEM;
+  }
+  *out = L;
+  return MAGNUS_OK;
+}
+
+int launch_csr_leja_iter_slice(const CsrOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma, double shift,
+                               cplx dk, double abs_dk, double tol, Workspace* ws, cudaStream_t st) {
+  const SliceLayout& S = *op.slice;
+  SliceView L;
+  L.n = S.n;
+  L.nslices = S.nslices;
+  L.meta = S.meta;
+  L.ent_ptr = S.ent_ptr;
+  L.slot_mask = S.slot_mask;
+  L.ci = S.ci;
+  L.v = S.v;
+  for (int t = 0; t < 3; ++t) L.coef[t] = t < op.nterms ? op.t[t].coef : make_double2(0.0, 0.0);
+  int code = ws->csr_kernel >= 5000 && ws->csr_kernel < 6000 ? ws->csr_kernel - 5000 : 84;   // 10 U + MINB
+#define SL_LAUNCH(U, MINB)                                                                                         \
+  if (code == 10 * U + MINB) {                                                                                     \
+    int64_t g = (S.nslices + SL_WARPS - 1) / SL_WARPS;                                                             \
+    const int64_t cap = (int64_t)device_sm_count() * MINB;                                                         \
+    if (g > cap) g = cap;                                                                                          \
+    csr_leja_iter_slice_kernel<U, MINB><<<(int)g, SL_WARPS * 32, 0, st>>>(L, w_in, w_out, p, inv_gamma, shift, dk,  \
+                                                                         abs_dk, tol, ws->status, ws->partials,   \
+                                                                         ws->tickets);                            \
+    ws->launches += 1;                                                                                             \
+    return (int)g;                                                                                                 \
+  }
+  SL_LAUNCH(8, 4)
+  SL_LAUNCH(8, 3)
+  SL_LAUNCH(4, 5)
+  SL_LAUNCH(4, 6)
+  SL_LAUNCH(4, 8)
+#undef SL_LAUNCH
+  return -1;
+}
+
+}  // namespace magnus

@@ -39,11 +39,22 @@ struct CsrTerm {
   cplx coef;
   int64_t nnz;
 };
+// Slice-major copy of a CSR operator, all terms merged (kernels_csr_slice.cu); owned by a handle or a single call.
+struct SliceLayout {
+  int64_t n = 0, nslices = 0, nslots = 0, nent = 0;
+  int nterms = 0;
+  int4* meta = nullptr;          // per 32-row slice: {first slot, slots, first slot of term 1, of term 2}
+  int64_t* ent_ptr = nullptr;    // [nslices + 1]
+  unsigned* slot_mask = nullptr; // [nslots] rows of the slice with an entry in the slot
+  int32_t* ci = nullptr;         // [nent] columns, slot-major
+  cplx* v = nullptr;             // [nent] values, same order
+};
 struct CsrOp {
   int64_t n;
   int nterms;
   int unit_cap;   // max over 32-row units and terms of one term's stored entries in one unit (0 = unknown): stream kernel
   CsrTerm t[3];
+  const SliceLayout* slice = nullptr;   // host pointer; set: the slice kernel may run (its terms = t[0..] in order)
 };
 
 struct DenseOp {
@@ -140,6 +151,13 @@ int launch_csr_leja_iter_rowtma(const CsrOp& op, const cplx* w_in, cplx* w_out, 
                                 double shift, cplx dk, double abs_dk, double tol, Workspace* ws, cudaStream_t st);
 int launch_csr_leja_iter_stream(const CsrOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma,
                                 double shift, cplx dk, double abs_dk, double tol, Workspace* ws, cudaStream_t st);
+
+// ---- kernels_csr_slice.cu ---------------------------------------------------
+// slice-major copy of op's terms (coefficients ignored); an error leaves *out empty and callers keep the CSR kernels
+int slice_layout_build(const CsrOp& op, SliceLayout* out, cudaStream_t st);
+void slice_layout_free(SliceLayout* L);
+int launch_csr_leja_iter_slice(const CsrOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma, double shift,
+                               cplx dk, double abs_dk, double tol, Workspace* ws, cudaStream_t st);
 
 // ---- kernels_csr_small.cu ---------------------------------------------------
 // one sub-step sweep (S5-S8) in one launch; on success status->done = 1, status->k = iterations and out is
