@@ -44,12 +44,18 @@ UNIT = "steps/s"
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` captures (profiles/r1_csr_rowblock_ncu.md, profiles/r1_dense_gemv_ncu.md); None = not captured.
-NCU_TRAFFIC_BYTES = {("cfg5", "cf4"): 15.093e9, ("cfg4", "cf4"): 4.299e9}
-NCU_TRAFFIC_SOURCE = {("cfg5", "cf4"): "ncu --set full capture of csr_leja_iter_rowblock_kernel, round 1 (commit 6319c2a, "
-                                       "profiles/r1_csr_rowblock_ncu.md); the default instantiation of the kernel is "
-                                       "unchanged since (round 2 re-capture: profiles/r2_csr_rowblock_ncu.md)",
-                      ("cfg4", "cf4"): "ncu --set full capture of dense_leja_iter_kernel, round 1 (profiles/r1_dense_gemv_ncu.md); "
-                                       "kernel unchanged since"}
+# Keyed by (config, scheme, kernel): a capture only describes the kernel it was taken on.
+NCU_TRAFFIC_BYTES = {("cfg5", "cf4", "csr_leja_iter_sliceoff_kernel"): 12.737e9,
+                     ("cfg5", "cf4", "csr_leja_iter_rowblock_kernel"): 15.093e9,
+                     ("cfg4", "cf4", "dense_leja_iter_kernel"): 4.299e9}
+NCU_TRAFFIC_SOURCE = {
+    ("cfg5", "cf4", "csr_leja_iter_sliceoff_kernel"):
+        "ncu --set full capture of csr_leja_iter_sliceoff_kernel<8,4,0> at N=24, 2026-11-04, round 2 "
+        "(profiles/r2_csr_sliceoff_ncu.md): dram read 12.207 GB + write 0.530 GB in 2.218 ms",
+    ("cfg5", "cf4", "csr_leja_iter_rowblock_kernel"):
+        "ncu --set full capture of csr_leja_iter_rowblock_kernel, round 1 (commit 6319c2a, profiles/r1_csr_rowblock_ncu.md)",
+    ("cfg4", "cf4", "dense_leja_iter_kernel"):
+        "ncu --set full capture of dense_leja_iter_kernel, round 1 (profiles/r1_dense_gemv_ncu.md); kernel unchanged since"}
 
 
 # ----------------------------------------------------------------------------- helpers
@@ -244,6 +250,7 @@ def measure_workload(M, W, torch, cfg, scheme, steps, warmup, dev, barrier, samp
         out["clocks"] = sampler.stop() if sampler else None
         out["seconds"] = e0.elapsed_time(e1) * 1e-3
         out["stats"] = st
+        out["path"] = h.describe()
         out["norm"] = float(torch.linalg.vector_norm(psi))
     out["inputs"] = (H0, H1, psi0, f)
     return out
@@ -285,15 +292,16 @@ def measure_e2e(M, torch, cfg, scheme, steps, inputs):
                       "part (seconds_h2d_create_d2h) is amortised over the K steps of the call, so `value` depends on K"}
 
 
-def roofline_for(cfg, scheme, st, peaks, fp64_peak_tflops):
-    r = _roofline_for(cfg, scheme, st, peaks, fp64_peak_tflops)
+def roofline_for(cfg, scheme, st, peaks, fp64_peak_tflops, path=None):
+    r = _roofline_for(cfg, scheme, st, peaks, fp64_peak_tflops, path)
     if r["bound"] == "hbm":
-        r["traffic"] = NCU_TRAFFIC_BYTES.get((cfg.name, scheme))
-        r["traffic_source"] = NCU_TRAFFIC_SOURCE.get((cfg.name, scheme))
+        key = (cfg.name, scheme, r["kernel"].split(" ")[0])
+        r["traffic"] = NCU_TRAFFIC_BYTES.get(key)
+        r["traffic_source"] = NCU_TRAFFIC_SOURCE.get(key)
     return r
 
 
-def _roofline_for(cfg, scheme, st, peaks, fp64_peak_tflops):
+def _roofline_for(cfg, scheme, st, peaks, fp64_peak_tflops, path=None):
     """Dominant kernel of the step: the fused Leja iteration (HBM) or, for M4 on dense H, the DMMA commutator."""
     leja_s, comm_s, mv = st["seconds_leja"], st["seconds_commutator"], max(1, st["total_matvecs"])
     nsteps_exp = max(1, st["n_exp"])
@@ -306,19 +314,33 @@ def _roofline_for(cfg, scheme, st, peaks, fp64_peak_tflops):
                 "peak_source": "FP64 DMMA m8n8k4 register-resident micro-benchmark (magnus_fp64_peaks) run in this process; "
                                "MEASURED_PEAKS.json has no FP64 figure and the guide gives no bf16->fp64 ratio",
                 "flops_per_launch": flops}
-    nbytes = algorithmic_bytes_per_iteration(cfg, scheme)
+    # bytes of the variant the library actually runs (magnus_describe): "never count bytes a variant does not
+    # move"; the plain-CSR figure of SURVEY 8(d) is reported beside it as csr_equivalent
+    csr_bytes = algorithmic_bytes_per_iteration(cfg, scheme)
+    nbytes = path["bytes_per_iteration"] if path and path.get("bytes_per_iteration") else csr_bytes
+    kernel = path["leja_kernel"] if path else ("dense_leja_iter_kernel" if cfg.kind == "dense" else "csr")
+    if path and path.get("csr_bytes_per_iteration"):
+        assert path["csr_bytes_per_iteration"] == csr_bytes, (path, csr_bytes)
     ms = leja_s / mv * 1e3
     achieved = nbytes / (ms * 1e-3) / 1e9
-    kernel = "dense_leja_iter_kernel" if cfg.kind == "dense" else (
-        "csr_leja_iter_rowblock_kernel" if cfg.n >= 32768 else
-        "csr_leja_sweep_small_kernel (whole sweep in one launch; L1/L2-resident, latency bound: the HBM fraction is not meaningful)"
-        if cfg.n <= 4096 else "csr_leja_iter_generic")
-    return {"kernel": kernel, "bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-            "frac": achieved / peaks["hbm_gbs"], "traffic": None, "peak_source": peaks["source"],
-            "bytes_per_launch": nbytes, "ms_per_launch": ms,
-            "how": "CUDA events around every Leja sweep (init .. stop) inside the timed region / matvecs: an upper "
-                   "bound on the kernel time (it includes the init, stop-test and early-exit launches)",
-            "frac_of_nominal_8TBs": achieved / 8000.0}
+    if kernel.startswith("csr_leja_sweep_small") or (cfg.kind == "dense" and cfg.n <= 4096):
+        kernel += " (L1/L2-resident working set, latency bound: the HBM fraction is not meaningful)"
+    r = {"kernel": kernel, "bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+         "frac": achieved / peaks["hbm_gbs"], "traffic": None, "peak_source": peaks["source"],
+         "bytes_per_launch": nbytes, "ms_per_launch": ms,
+         "how": "CUDA events around every Leja sweep (init .. stop) inside the timed region / matvecs: an upper "
+                "bound on the kernel time (it includes the init, stop-test and early-exit launches); bytes = the "
+                "algorithmic bytes of the storage variant the kernel reads (magnus_describe)",
+         "frac_of_nominal_8TBs": achieved / 8000.0}
+    if cfg.kind != "dense":
+        eq = csr_bytes / (ms * 1e-3) / 1e9
+        r["csr_equivalent"] = {"bytes_per_launch": csr_bytes, "gbs": eq, "frac": eq / peaks["hbm_gbs"],
+                               "note": "SURVEY 8(d) plain-CSR bytes (20 B per stored entry) over the same time: what a "
+                                       "CSR-reading kernel would have to sustain to be as fast; not a bandwidth the "
+                                       "kernel achieves"}
+        if path and path.get("slots"):
+            r["layout"] = {k: path[k] for k in ("slices", "slots", "entries")}
+    return r
 
 
 def max_over_ranks(seconds: float, dist=None, device="cpu") -> float:
@@ -357,7 +379,7 @@ def measure_extra(M, W, torch, dev, peaks, dmma_tf):
         sampler = ClockSampler(torch.cuda.current_device())
         res = measure_workload(M, W, torch, cfg, scheme, steps, 1, dev, lambda: None, sampler, shortcuts)
         st = res["stats"]
-        roof = roofline_for(cfg, scheme, st, peaks, dmma_tf)
+        roof = roofline_for(cfg, scheme, st, peaks, dmma_tf, res.get("path"))
         out[key] = {"workload": workload_description(cfg, scheme), "steps": steps, "warmup": 1,
                                  "shortcut": ("beyond-paper shortcut, NOT the mandated path: [H0,H1] cached at create, no GEMM per "
                                               "step (SURVEY 8f-4)") if shortcuts else None,
@@ -412,7 +434,7 @@ def run_ours(args):
     torch.cuda.empty_cache()
 
     if rank == 0:
-        roof = roofline_for(cfg, scheme, st, peaks, dmma_tf)
+        roof = roofline_for(cfg, scheme, st, peaks, dmma_tf, res.get("path"))
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": sec / args.steps * 1e3, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "complex128 (f64)", "data": "synthetic",

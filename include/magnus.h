@@ -233,6 +233,21 @@ int magnus_commutator_csr(const magnus_matrix* A, const magnus_matrix* B, int64_
                           int64_t* nnz_out, int32_t* row_ptr_out, int32_t* col_idx_out,
                           void* values_out, void* stream);
 
+/* What the handle will run for the fused Leja iteration (row S6) and what that kernel moves per launch.
+ * Measurement support (bench.py reports the roofline against THESE bytes: "never count bytes a
+ * variant does not move").  leja_kernel is the kernel's name; bytes_per_iteration its algorithmic HBM bytes for
+ * one iteration of the handle's operator (CSR: all terms of the scheme -- H0, H1 and, for M4, C; dense:
+ * 16 n^2 + 64 n); csr_bytes_per_iteration the same for plain CSR storage, 20 nnz + 4 (n + 1) terms + 64 n
+ * (0 for dense).  slices / slots / entries describe the slice-major copy when one was built (else 0):
+ * the offset-slot layout moves 16 B per entry + 8 B per slot + 24 B per slice + 64 B per row. */
+typedef struct magnus_path_info {
+  char leja_kernel[64];
+  int64_t bytes_per_iteration;
+  int64_t csr_bytes_per_iteration;
+  int64_t slices, slots, entries;
+} magnus_path_info;
+int magnus_describe(magnus_handle h, magnus_path_info* out);
+
 /* Register-resident micro-benchmarks that fix the ALU-side roofline denominators
  * (no FP64 peak is in MEASURED_PEAKS.json): DMMA m8n8k4 and plain DFMA, TFLOP/s. */
 int magnus_fp64_peaks(double* dmma_tflops, double* dfma_tflops, void* stream);

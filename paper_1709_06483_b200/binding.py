@@ -57,10 +57,16 @@ class Stats(C.Structure):
                 ("kernel_launches", C.c_int64)]
 
 
+class PathInfo(C.Structure):
+    _fields_ = [("leja_kernel", C.c_char * 64), ("bytes_per_iteration", C.c_int64),
+                ("csr_bytes_per_iteration", C.c_int64), ("slices", C.c_int64), ("slots", C.c_int64),
+                ("entries", C.c_int64)]
+
+
 DRIVE = C.CFUNCTYPE(C.c_double, C.c_double, C.c_void_p)
 
 EXPORTS = [
-    "magnus_create", "magnus_destroy", "leja_expmv", "magnus_step", "magnus_integrate", "magnus_integrate_host",
+    "magnus_create", "magnus_destroy", "magnus_describe", "leja_expmv", "magnus_step", "magnus_integrate", "magnus_integrate_host",
     "magnus_gershgorin", "magnus_leja_iteration", "magnus_zgemm", "magnus_commutator_dense", "magnus_commutator_csr", "magnus_omega_dense",
     "magnus_fp64_peaks", "magnus_host_leja_points", "magnus_host_divided_differences", "magnus_host_snap_interval",
     "magnus_host_step_coefficients", "magnus_strerror", "magnus_last_error", "magnus_version",
@@ -84,6 +90,7 @@ def lib():
         L.magnus_create.argtypes = [C.POINTER(C.c_void_p), C.POINTER(MatrixStruct), C.POINTER(MatrixStruct), DRIVE,
                                     C.c_void_p, C.c_int, C.POINTER(Options)]
         L.magnus_destroy.argtypes = [C.c_void_p]
+        L.magnus_describe.argtypes = [C.c_void_p, C.POINTER(PathInfo)]
         L.leja_expmv.argtypes = [C.POINTER(MatrixStruct), C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_void_p,
                                  C.POINTER(ExpmvInfo)]
         L.magnus_step.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_void_p, C.POINTER(StepInfo)]
@@ -221,6 +228,14 @@ class Handle:
         return {"total_matvecs": int(st.total_matvecs), "n_exp": int(st.n_exp), "iters": iters[:int(st.n_exp)].copy(),
                 "seconds_device": st.seconds_device, "seconds_leja": st.seconds_leja,
                 "seconds_commutator": st.seconds_commutator, "kernel_launches": int(st.kernel_launches)}
+
+    def describe(self) -> dict:
+        """The kernel that runs the fused Leja iteration for this handle and its algorithmic bytes per launch."""
+        info = PathInfo()
+        _check(lib().magnus_describe(self._h, C.byref(info)))
+        return {"leja_kernel": info.leja_kernel.decode(), "bytes_per_iteration": int(info.bytes_per_iteration),
+                "csr_bytes_per_iteration": int(info.csr_bytes_per_iteration), "slices": int(info.slices),
+                "slots": int(info.slots), "entries": int(info.entries)}
 
     def close(self):
         if self._h:

@@ -13,7 +13,9 @@
 
 namespace magnus {
 
-const int kM6DenseMaxN = 16384;   // CSR input of MAGNUS_M6 is expanded into dense copies up to this n
+const int kM6DenseMaxN = 16384;
+const int64_t kSliceAutoMinN = 32768;     // csr_kernel 0: from this n on, try the offset-slot layout (kernels_csr_slice.cu)
+const double kSliceAutoMinFill = 8.0;     // ... and keep it if a slot holds at least this many entries on average   // CSR input of MAGNUS_M6 is expanded into dense copies up to this n
 
 static thread_local char g_err[512] = "";
 
@@ -422,6 +424,49 @@ int magnus_destroy(magnus_handle h) {
   return MAGNUS_OK;
 }
 
+int magnus_describe(magnus_handle h, magnus_path_info* out) {
+  if (!h || !out) { set_error("magnus_describe: NULL argument"); return MAGNUS_EINVAL; }
+  std::memset(out, 0, sizeof *out);
+  const int64_t n = h->n;
+  const char* name = "dense_leja_iter_kernel";
+  if (h->format == MAGNUS_DENSE) {
+    out->bytes_per_iteration = 16 * n * n + 64 * n;
+  } else {
+    int64_t nnz = h->H0.nnz + h->H1.nnz, terms = 2;
+    if (h->scheme == MAGNUS_M4 && h->c_nnz > 0) {
+      nnz += h->c_nnz;
+      terms = 3;
+    }
+    out->csr_bytes_per_iteration = 20 * nnz + 4 * (n + 1) * terms + 64 * n;
+    out->bytes_per_iteration = out->csr_bytes_per_iteration;
+    const int k = h->ws.csr_kernel;
+    if (n <= kSmallSweepMaxN && k == 0) {
+      name = "csr_leja_sweep_small_kernel";
+    } else if (h->slice.meta && (k == 0 || slice_layout_kind(k) != 0)) {
+      out->slices = h->slice.nslices;
+      out->slots = h->slice.nslots;
+      out->entries = h->slice.nent;
+      if (h->slice.offsets) {
+        name = "csr_leja_iter_sliceoff_kernel";
+        out->bytes_per_iteration = 16 * h->slice.nent + 8 * h->slice.nslots + 24 * h->slice.nslices + 64 * n;
+      } else {
+        name = "csr_leja_iter_slice_kernel";
+        out->bytes_per_iteration = 20 * h->slice.nent + 4 * h->slice.nslots + 24 * h->slice.nslices + 64 * n;
+      }
+    } else if (k == 3 || (k >= 20000 && k < 30000)) {
+      name = "csr_leja_iter_stream_kernel";
+    } else if (k == 4) {
+      name = "csr_leja_iter_rowtma_kernel";
+    } else if (k == 2 || k >= 1000 || (k == 0 && n >= 32768)) {
+      name = "csr_leja_iter_rowblock_kernel";
+    } else {
+      name = "csr_leja_iter_generic";
+    }
+  }
+  std::snprintf(out->leja_kernel, sizeof out->leja_kernel, "%s", name);
+  return MAGNUS_OK;
+}
+
 int magnus_create(magnus_handle* out, const magnus_matrix* H0, const magnus_matrix* H1, magnus_drive_fn f, void* user,
                   int scheme, const magnus_options* opt) {
   if (!out) { set_error("out is NULL"); return MAGNUS_EINVAL; }
@@ -535,7 +580,10 @@ int magnus_create(magnus_handle* out, const magnus_matrix* H0, const magnus_matr
   if (h->format == MAGNUS_CSR) {
     rc = csr_cache_rowstats(h);
     if (rc) { magnus_destroy(h); return rc; }
-    if (csr_kernel == 5 || (csr_kernel >= 5000 && csr_kernel < 6000)) {
+    // slice-major copy of the operator: asked for explicitly, or by default for large n when its slots are
+    // well filled (spin chains: about 20 entries per slot); otherwise the CSR kernels run
+    const int kind = slice_layout_kind(csr_kernel);
+    if (kind != 0 || (csr_kernel == 0 && h->n >= kSliceAutoMinN)) {
       CsrOp op;
       op.n = h->n;
       op.unit_cap = 0;
@@ -549,7 +597,10 @@ int magnus_create(magnus_handle* out, const magnus_matrix* H0, const magnus_matr
         op.t[2].v = h->c_v;
         op.t[2].nnz = h->c_nnz;
       }
-      slice_layout_build(op, &h->slice, h->stream);   // on failure the CSR kernels run
+      if (slice_layout_build(op, &h->slice, h->stream, kind != 1) == MAGNUS_OK && kind == 0 &&
+          (double)h->slice.nent < kSliceAutoMinFill * (double)h->slice.nslots)
+        slice_layout_free(&h->slice);                  // poorly filled slots: not worth it
+      // on failure the CSR kernels run
     }
   }
   if (cudaStreamSynchronize(h->stream) != cudaSuccess) { magnus_destroy(h); return MAGNUS_ECUDA; }
@@ -829,7 +880,9 @@ static int build_op(const magnus_matrix* H0, const magnus_matrix* H1, double g, 
     op->csr.t[2] = op->csr.t[0];
     op->csr.unit_cap = 0;
     if (csr_unit_cap(op->csr, st, &op->csr.unit_cap) != MAGNUS_OK) op->csr.unit_cap = 0;
-    if (tmpS && (ws->csr_kernel == 5 || (ws->csr_kernel >= 5000 && ws->csr_kernel < 6000)) && slice_layout_build(op->csr, tmpS, st) == MAGNUS_OK) op->csr.slice = tmpS;
+    if (tmpS && slice_layout_kind(ws->csr_kernel) != 0 &&
+        slice_layout_build(op->csr, tmpS, st, slice_layout_kind(ws->csr_kernel) == 2) == MAGNUS_OK)
+      op->csr.slice = tmpS;
   } else {
     op->dense = true;
     op->dns.n = H0->n;

@@ -90,8 +90,43 @@ int workspace_alloc(Workspace* ws, int64_t n) {
   return MAGNUS_OK;
 }
 
+// Buffers of the planned-batch path; allocated once per workspace, on first use.
+int ensure_sweep_jobs(Workspace* ws) {
+  if (ws->jobs) return MAGNUS_OK;
+  bool ok = cudaMalloc(&ws->jobs, sizeof(SweepJob) * kJobCap) == cudaSuccess &&
+            cudaMallocHost(&ws->jobs_host, sizeof(SweepJob) * kJobCap) == cudaSuccess &&
+            cudaMalloc(&ws->status_arr, sizeof(LejaStatus) * kJobCap) == cudaSuccess &&
+            cudaMallocHost(&ws->status_arr_host, sizeof(LejaStatus) * kJobCap) == cudaSuccess &&
+            cudaMalloc(&ws->ab_arr, sizeof(double) * 2 * kJobCap) == cudaSuccess &&
+            cudaMallocHost(&ws->ab_arr_host, sizeof(double) * 2 * kJobCap) == cudaSuccess &&
+            cudaMalloc(&ws->coef_arr, sizeof(double) * 4 * kJobCap) == cudaSuccess &&
+            cudaMallocHost(&ws->coef_arr_host, sizeof(double) * 4 * kJobCap) == cudaSuccess &&
+            cudaMalloc(&ws->leja_l, sizeof(double) * (kMaxDegree + 1)) == cudaSuccess &&
+            cudaMalloc(&ws->grid_bar, 64) == cudaSuccess &&
+            cudaMalloc(&ws->sweep_partials, sizeof(double) * 4 * kMaxPartials) == cudaSuccess;
+  if (ok)
+    ok = cudaMemcpy(ws->leja_l, leja_points(), sizeof(double) * (kMaxDegree + 1), cudaMemcpyHostToDevice) == cudaSuccess &&
+         cudaMemset(ws->grid_bar, 0, 64) == cudaSuccess;
+  if (!ok) {
+    cudaGetLastError();
+    return MAGNUS_ENOMEM;
+  }
+  return MAGNUS_OK;
+}
+
 void workspace_free(Workspace* ws) {
   stream_maps_free(ws);
+  cudaFree(ws->jobs);
+  cudaFree(ws->status_arr);
+  cudaFree(ws->ab_arr);
+  cudaFree(ws->coef_arr);
+  cudaFree(ws->leja_l);
+  cudaFree(ws->grid_bar);
+  cudaFree(ws->sweep_partials);
+  if (ws->jobs_host) cudaFreeHost(ws->jobs_host);
+  if (ws->status_arr_host) cudaFreeHost(ws->status_arr_host);
+  if (ws->ab_arr_host) cudaFreeHost(ws->ab_arr_host);
+  if (ws->coef_arr_host) cudaFreeHost(ws->coef_arr_host);
   cudaFree(ws->w[0]);
   cudaFree(ws->w[1]);
   cudaFree(ws->p);

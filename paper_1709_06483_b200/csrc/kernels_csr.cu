@@ -377,7 +377,7 @@ bool csr_rowblock_supported(const CsrOp& op);
 
 int launch_csr_leja_iter(const CsrOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma, double shift,
                          cplx dk, double abs_dk, double tol, Workspace* ws, cudaStream_t st) {
-  if (op.slice && (ws->csr_kernel == 5 || ws->csr_kernel == 0 || (ws->csr_kernel >= 5000 && ws->csr_kernel < 6000)))
+  if (op.slice && (ws->csr_kernel == 0 || slice_layout_kind(ws->csr_kernel) != 0))
     return launch_csr_leja_iter_slice(op, w_in, w_out, p, inv_gamma, shift, dk, abs_dk, tol, ws, st);
   if (ws->csr_kernel == 4 && csr_rowtma_supported(op)) {
     const int g = launch_csr_leja_iter_rowtma(op, w_in, w_out, p, inv_gamma, shift, dk, abs_dk, tol, ws, st);

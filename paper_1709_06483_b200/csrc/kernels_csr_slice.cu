@@ -256,10 +256,12 @@ __global__ void __launch_bounds__(SL_WARPS * 32, MINB)
 // ---- building the layout (once per handle) ------------------------------------------------
 // 32-way merge of the rows of a slice on key = column - row (ascending inside a CSR row).
 // FILL = false: count slots and entries per slice; FILL = true: write masks and packed entries.
-template <bool FILL>
+// OFFS = true: a slot is stored as the record {row mask, column - row} and no column array is written
+// (the offset-slot layout of csr_kernel 6); OFFS = false: masks and a column per entry (csr_kernel 5).
+template <bool FILL, bool OFFS>
 __global__ void __launch_bounds__(128)
-    slice_merge_kernel(CsrOp op, int64_t nslices, int4* meta, int64_t* ent_ptr, unsigned* slot_mask, int32_t* ci_out,
-                       cplx* v_out) {
+    slice_merge_kernel(CsrOp op, int64_t nslices, int4* meta, int64_t* ent_ptr, unsigned* slot_mask, uint2* slot_rec,
+                       int32_t* ci_out, cplx* v_out) {
   const int lane = threadIdx.x & 31;
   const unsigned lt = (1u << lane) - 1u;
   const int64_t s = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
@@ -290,10 +292,13 @@ __global__ void __launch_bounds__(128)
       const bool hit = key == kmin;
       const unsigned m = __ballot_sync(0xffffffffu, hit);
       if (FILL) {
-        if (lane == 0) slot_mask[sb + nslots] = m;
+        if (lane == 0) {
+          if (OFFS) slot_rec[sb + nslots] = make_uint2(m, (unsigned)kmin);
+          else slot_mask[sb + nslots] = m;
+        }
         if (hit) {
           const int64_t q = eb + ents + __popc(m & lt);
-          ci_out[q] = col;
+          if (!OFFS) ci_out[q] = col;
           v_out[q] = vv[cur];
         }
       }
@@ -360,6 +365,208 @@ __global__ void __launch_bounds__(1024) slice_scan_kernel(int64_t nslices, int4*
   }
 }
 
+
+// ---------------------------------------------------------------------------------------------
+// csr_kernel = 6: the OFFSET-SLOT layout.  All entries of a slot share column - row, so the slot
+// record {row mask, column - row} replaces the per-entry column array: per stored entry the kernel
+// reads the 16-byte value and nothing else (8 bytes per slot instead of 4 bytes per entry), and the
+// w-gather address row + offset is known without a dependent index load.  The warp keeps SO_U slots
+// in flight per lane in a ROTATING register pipeline: slot u of the batch being consumed is
+// multiplied and its registers are re-used at once for slot u of the next batch (which may belong to
+// the next slice), so value and w loads are outstanding all the time instead of draining at batch
+// boundaries.  Slot records reach the warp through a double-buffered per-warp shared-memory ring
+// (one 16-byte cp.async per lane and slice, requested a whole slice ahead).
+// Per-iteration HBM traffic: 16 B per stored entry + 8 B per slot + 24 B per slice + 64 B per row.
+// ---------------------------------------------------------------------------------------------
+constexpr int SO_CAP = 256;    // slots of one slice a ring buffer holds; a layout with a larger slice is refused
+
+struct SliceViewO {
+  int64_t n, nslices;
+  const int4* meta;            // per slice: {first slot (global), slots, first slot of term 1, of term 2}
+  const int64_t* ent_ptr;      // [nslices + 1]
+  const uint2* rec;            // per slot {row mask, column - row}
+  const cplx* v;
+  cplx coef[3];
+};
+
+__device__ __forceinline__ cplx ld_stream_hint_if(const cplx* p, unsigned ok, uint64_t pol) {
+  cplx r;
+  asm("{\n .reg .pred q;\n setp.ne.b32 q, %3, 0;\n mov.f64 %0, 0d0000000000000000;\n mov.f64 %1, 0d0000000000000000;\n"
+      " @q ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f64 {%0, %1}, [%2], %4;\n}"
+      : "=d"(r.x), "=d"(r.y)
+      : "l"(p), "r"(ok), "l"(pol));
+  return r;
+}
+__device__ __forceinline__ cplx ld_cached_hint_if(const cplx* p, unsigned ok, uint64_t pol) {
+  cplx r;
+  asm("{\n .reg .pred q;\n setp.ne.b32 q, %3, 0;\n mov.f64 %0, 0d0000000000000000;\n mov.f64 %1, 0d0000000000000000;\n"
+      " @q ld.global.nc.L2::cache_hint.v2.f64 {%0, %1}, [%2], %4;\n}"
+      : "=d"(r.x), "=d"(r.y)
+      : "l"(p), "r"(ok), "l"(pol));
+  return r;
+}
+__device__ __forceinline__ cplx ld_cached_if(const cplx* p, unsigned ok) {
+  cplx r;
+  asm("{\n .reg .pred q;\n setp.ne.b32 q, %3, 0;\n mov.f64 %0, 0d0000000000000000;\n mov.f64 %1, 0d0000000000000000;\n"
+      " @q ld.global.nc.v2.f64 {%0, %1}, [%2];\n}"
+      : "=d"(r.x), "=d"(r.y)
+      : "l"(p), "r"(ok));
+  return r;
+}
+
+// POL: 0 no L2 hints; 1 matrix values evict-first; 2 also w gathers evict-last.  SO_U slots in flight per lane.
+template <int SO_U, int MINB, int POL>
+__global__ void __launch_bounds__(SL_WARPS * 32, MINB)
+    csr_leja_iter_sliceoff_kernel(SliceViewO L, const cplx* __restrict__ w_in, cplx* __restrict__ w_out,
+                                  cplx* __restrict__ p, double inv_gamma, double shift, cplx dk, double abs_dk,
+                                  double tol, LejaStatus* status, double* partials, unsigned* ticket) {
+  static_assert(SL_PAD % SO_U == 0, "batches must not straddle terms (terms are padded to SL_PAD slots)");
+  if (status->done) return;
+  __shared__ __align__(16) uint2 s_rec[SL_WARPS][2][SO_CAP];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const unsigned lbit = 1u << lane, lt = lbit - 1u;
+  const int stride = (int)gridDim.x * SL_WARPS, nslices = (int)L.nslices;
+  double sw = 0.0, sp = 0.0;
+
+  const uint64_t pol_v = POL >= 1 ? policy_evict_first() : 0, pol_w = POL >= 2 ? policy_evict_last() : 0;
+  int sI = (int)blockIdx.x * SL_WARPS + warp;   // slice on the issue side
+  if (sI < nslices) {
+    struct Desc { int64_t eb; int sb, ns, b1, b2; };
+    auto load_desc = [&](int s, Desc& D) {
+      const int4 m = __ldg(L.meta + s);
+      D.eb = __ldg(L.ent_ptr + s);
+      D.sb = m.x;
+      D.ns = m.y;
+      D.b1 = m.z;
+      D.b2 = m.w;
+    };
+    auto stage = [&](const Desc& D, uint2* buf) {   // two records per 16-byte copy
+      for (int k = 2 * lane; k < D.ns; k += 64) {
+        const unsigned dst = (unsigned)__cvta_generic_to_shared(buf + k);
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(L.rec + D.sb + k) : "memory");
+      }
+    };
+    Desc DI, DN, D2;     // slice being issued, the next one (records staged), the one after (descriptor only)
+    load_desc(sI, DI);
+    stage(DI, s_rec[warp][0]);
+    bool haveN = sI + stride < nslices, have2 = sI + 2 * stride < nslices;
+    DN = DI;
+    D2 = DI;
+    if (haveN) {
+      load_desc(sI + stride, DN);
+      stage(DN, s_rec[warp][1]);
+    }
+    if (have2) load_desc(sI + 2 * stride, D2);
+    cp_async_wait_all();
+    __syncwarp();
+
+    // issue side
+    int bufI = 0, jI = 0;
+    unsigned runI = 0;                       // entries of the slice before slot jI
+    const cplx* vbI = L.v + DI.eb;
+    int64_t rowI = ((int64_t)sI << 5) + lane;
+    bool issuing = true;
+    // consume side (one batch behind)
+    int jC = 0, nsC = DI.ns, b1C = DI.b1, b2C = DI.b2, term = 0;
+    int64_t rowC = rowI;
+    cplx a = make_double2(0.0, 0.0), y = a, wi = a, pi = a;
+    if (rowC < L.n) {
+      wi = w_in[rowC];
+      pi = p[rowC];
+    }
+    cplx v[SO_U], x[SO_U];
+    auto issue_slot = [&](int u) {
+      const uint2 r = s_rec[warp][bufI][jI + u];
+      const unsigned ok = r.x & lbit;
+      v[u] = POL >= 1 ? ld_stream_hint_if(vbI + (runI + __popc(r.x & lt)), ok, pol_v)
+                      : ld_stream_if(vbI + (runI + __popc(r.x & lt)), ok);
+      x[u] = POL >= 2 ? ld_cached_hint_if(w_in + (rowI + (int)r.y), ok, pol_w)
+                      : ld_cached_if(w_in + (rowI + (int)r.y), ok);
+      runI += __popc(r.x);
+    };
+#pragma unroll
+    for (int u = 0; u < SO_U; ++u) issue_slot(u);
+    jI = SO_U;
+
+    while (true) {
+      // ---- issue side: next batch of the same slice, or the first batch of the next slice
+      if (jI >= DI.ns) {
+        if (haveN) {
+          sI += stride;
+          DI = DN;
+          DN = D2;
+          haveN = have2;
+          have2 = sI + 2 * stride < nslices;
+          cp_async_wait_all();   // the new slice's records were requested a slice ago
+          __syncwarp();          // ... and every lane is done with the old slice's
+          if (haveN) stage(DN, s_rec[warp][bufI]);
+          bufI ^= 1;
+          if (have2) load_desc(sI + 2 * stride, D2);
+          jI = 0;
+          runI = 0;
+          vbI = L.v + DI.eb;
+          rowI = ((int64_t)sI << 5) + lane;
+        } else {
+          issuing = false;
+        }
+      }
+      // ---- consume side: the batch belongs to one term (terms are padded to whole batches)
+      const int tnow = (jC >= b1C) + (jC >= b2C);
+      if (tnow != term) {
+        cfma(y, L.coef[term], a);
+        a = make_double2(0.0, 0.0);
+        term = tnow;
+      }
+      if (issuing) {
+#pragma unroll
+        for (int u = 0; u < SO_U; ++u) {
+          cfma(a, v[u], x[u]);
+          issue_slot(u);
+        }
+        jI += SO_U;
+      } else {
+#pragma unroll
+        for (int u = 0; u < SO_U; ++u) cfma(a, v[u], x[u]);
+      }
+      jC += SO_U;
+      if (jC >= nsC) {
+        // finish the rows of the slice
+        cfma(y, L.coef[term], a);
+        if (rowC < L.n) {
+          cplx wn;
+          wn.x = inv_gamma * y.x - shift * wi.x;
+          wn.y = inv_gamma * y.y - shift * wi.y;
+          cfma(pi, dk, wn);
+          w_out[rowC] = wn;
+          p[rowC] = pi;
+          sw += wn.x * wn.x + wn.y * wn.y;
+          sp += pi.x * pi.x + pi.y * pi.y;
+        }
+        if (!issuing) break;
+        // the issue side is exactly one batch ahead: it has just entered the slice consumed next
+        jC = 0;
+        nsC = DI.ns;
+        b1C = DI.b1;
+        b2C = DI.b2;
+        rowC = rowI;
+        term = 0;
+        a = make_double2(0.0, 0.0);
+        y = a;
+        if (rowC < L.n) {
+          wi = w_in[rowC];
+          pi = p[rowC];
+        }
+      }
+    }
+  }
+  block_reduce_sum2<SL_WARPS * 32>(sw, sp);
+  if (threadIdx.x == 0) {
+    partials[2 * blockIdx.x] = sw;
+    partials[2 * blockIdx.x + 1] = sp;
+  }
+  if (last_block_ticket(ticket)) leja_finalize_warp0(partials, gridDim.x, abs_dk, tol, false, status);   // S7
+}
+
 }  // namespace
 
 void slice_layout_free(SliceLayout* L) {
@@ -367,6 +574,7 @@ void slice_layout_free(SliceLayout* L) {
   cudaFree(L->meta);
   cudaFree(L->ent_ptr);
   cudaFree(L->slot_mask);
+  cudaFree(L->slot_rec);
   cudaFree(L->ci);
   cudaFree(L->v);
   *L = SliceLayout();
@@ -374,36 +582,52 @@ void slice_layout_free(SliceLayout* L) {
 
 // Returns MAGNUS_OK and a filled layout, or an error code with *out left empty (callers fall back to
 // the CSR kernels: the layout is an optimisation, never a requirement).  Synchronises the stream once.
-int slice_layout_build(const CsrOp& op, SliceLayout* out, cudaStream_t st) {
+// offsets = true builds the offset-slot layout of csr_kernel 6 (slot records, no column array).
+int slice_layout_build(const CsrOp& op, SliceLayout* out, cudaStream_t st, bool offsets) {
   *out = SliceLayout();
   SliceLayout L;
   L.n = op.n;
   L.nslices = (op.n + 31) >> 5;
   L.nterms = op.nterms;
+  L.offsets = offsets;
   int64_t* totals = nullptr;
   int64_t host_totals[3] = {0, 0, 0};
   bool ok = cudaMalloc(&L.meta, sizeof(int4) * (size_t)L.nslices) == cudaSuccess &&
             cudaMalloc(&L.ent_ptr, sizeof(int64_t) * (size_t)(L.nslices + 1)) == cudaSuccess &&
             cudaMalloc(&totals, 3 * sizeof(int64_t)) == cudaSuccess;
+  const int64_t blocks = (L.nslices * 32 + 127) / 128;
   if (ok) {
-    const int64_t blocks = (L.nslices * 32 + 127) / 128;
-    slice_merge_kernel<false><<<(unsigned)blocks, 128, 0, st>>>(op, L.nslices, L.meta, L.ent_ptr, nullptr, nullptr, nullptr);
+    slice_merge_kernel<false, false><<<(unsigned)blocks, 128, 0, st>>>(op, L.nslices, L.meta, L.ent_ptr, nullptr, nullptr,
+                                                                       nullptr, nullptr);
     slice_scan_kernel<<<1, 1024, 0, st>>>(L.nslices, L.meta, L.ent_ptr, totals);
     ok = cudaMemcpyAsync(host_totals, totals, sizeof host_totals, cudaMemcpyDeviceToHost, st) == cudaSuccess &&
          cudaStreamSynchronize(st) == cudaSuccess;
   }
-  if (ok) ok = host_totals[0] < ((int64_t)1 << 31) && host_totals[2] <= SL_CAP && host_totals[1] < ((int64_t)1 << 32);
+  if (ok) {
+    ok = host_totals[0] < ((int64_t)1 << 31) && host_totals[2] <= (offsets ? SO_CAP : SL_CAP) &&
+         host_totals[1] < ((int64_t)1 << 32);
+  }
   if (ok) {
     L.nslots = host_totals[0];
     L.nent = host_totals[1];
-    ok = cudaMalloc(&L.slot_mask, sizeof(unsigned) * (size_t)(L.nslots > 0 ? L.nslots : 1)) == cudaSuccess &&
-         cudaMalloc(&L.ci, sizeof(int32_t) * (size_t)(L.nent > 0 ? L.nent : 1)) == cudaSuccess &&
-         cudaMalloc(&L.v, sizeof(cplx) * (size_t)(L.nent > 0 ? L.nent : 1)) == cudaSuccess;
+    const size_t ns = (size_t)(L.nslots > 0 ? L.nslots : 1), ne = (size_t)(L.nent > 0 ? L.nent : 1);
+    ok = cudaMalloc(&L.v, sizeof(cplx) * ne) == cudaSuccess;
+    if (ok && offsets) {
+      ok = cudaMalloc(&L.slot_rec, sizeof(uint2) * ns) == cudaSuccess &&
+           cudaMemsetAsync(L.slot_rec, 0, sizeof(uint2) * ns, st) == cudaSuccess;
+    } else if (ok) {
+      ok = cudaMalloc(&L.slot_mask, sizeof(unsigned) * ns) == cudaSuccess &&
+           cudaMalloc(&L.ci, sizeof(int32_t) * ne) == cudaSuccess &&
+           cudaMemsetAsync(L.slot_mask, 0, sizeof(unsigned) * ns, st) == cudaSuccess;
+    }
   }
-  if (ok) ok = cudaMemsetAsync(L.slot_mask, 0, sizeof(unsigned) * (size_t)(L.nslots > 0 ? L.nslots : 1), st) == cudaSuccess;
   if (ok) {
-    const int64_t blocks = (L.nslices * 32 + 127) / 128;
-    slice_merge_kernel<true><<<(unsigned)blocks, 128, 0, st>>>(op, L.nslices, L.meta, L.ent_ptr, L.slot_mask, L.ci, L.v);
+    if (offsets)
+      slice_merge_kernel<true, true><<<(unsigned)blocks, 128, 0, st>>>(op, L.nslices, L.meta, L.ent_ptr, nullptr,
+                                                                       L.slot_rec, nullptr, L.v);
+    else
+      slice_merge_kernel<true, false><<<(unsigned)blocks, 128, 0, st>>>(op, L.nslices, L.meta, L.ent_ptr, L.slot_mask,
+                                                                        nullptr, L.ci, L.v);
     ok = cudaGetLastError() == cudaSuccess;
   }
   cudaFree(totals);
@@ -419,6 +643,41 @@ int slice_layout_build(const CsrOp& op, SliceLayout* out, cudaStream_t st) {
 int launch_csr_leja_iter_slice(const CsrOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma, double shift,
                                cplx dk, double abs_dk, double tol, Workspace* ws, cudaStream_t st) {
   const SliceLayout& S = *op.slice;
+  if (S.offsets) {
+    SliceViewO L;
+    L.n = S.n;
+    L.nslices = S.nslices;
+    L.meta = S.meta;
+    L.ent_ptr = S.ent_ptr;
+    L.rec = S.slot_rec;
+    L.v = S.v;
+    for (int t = 0; t < 3; ++t) L.coef[t] = t < op.nterms ? op.t[t].coef : make_double2(0.0, 0.0);
+    // tuning code 6000 + 100 POL + 10 [4 slots in flight instead of 8] + MINB (default 6004: no hints, 8 slots,
+    // 4 CTAs = 16 warps per SM)
+    const int code = ws->csr_kernel >= 6000 && ws->csr_kernel < 7000 ? ws->csr_kernel - 6000 : 4;
+    const int minb = code % 10, pol = code / 100, u = (code / 10) % 10 ? 4 : 8;
+#define SO_LAUNCH(U, MINB, POL)                                                                                      \
+  if (u == U && minb == MINB && pol == POL) {                                                                        \
+    int64_t g = (S.nslices + SL_WARPS - 1) / SL_WARPS;                                                               \
+    const int64_t cap = (int64_t)device_sm_count() * MINB;                                                           \
+    if (g > cap) g = cap;                                                                                            \
+    csr_leja_iter_sliceoff_kernel<U, MINB, POL><<<(int)g, SL_WARPS * 32, 0, st>>>(                                   \
+        L, w_in, w_out, p, inv_gamma, shift, dk, abs_dk, tol, ws->status, ws->partials, ws->tickets);                \
+    ws->launches += 1;                                                                                               \
+    return (int)g;                                                                                                   \
+  }
+    SO_LAUNCH(8, 4, 0)
+    SO_LAUNCH(8, 3, 0)
+    SO_LAUNCH(8, 4, 1)
+    SO_LAUNCH(8, 4, 2)
+    SO_LAUNCH(8, 5, 0)
+    SO_LAUNCH(4, 5, 0)
+    SO_LAUNCH(4, 6, 0)
+    SO_LAUNCH(4, 7, 0)
+    SO_LAUNCH(4, 8, 0)
+#undef SO_LAUNCH
+    return -1;
+  }
   SliceView L;
   L.n = S.n;
   L.nslices = S.nslices;

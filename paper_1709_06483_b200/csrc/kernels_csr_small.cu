@@ -63,12 +63,17 @@ __device__ __forceinline__ void block_reduce_sum2_ss(double& a, double& b, doubl
   }
 }
 
+// jobs[0..njobs): the exponentials of a planned batch, applied to psi in order (psi is read once and
+// stays in shared memory from job to job; every job still writes its result to global memory, so that
+// psi holds the state before a job that fails).  status[e] is written per job; the loop stops at the
+// first job that does not meet tol within its m_max (status[e].pad = 1).
 __global__ void __cluster_dims__(SS_CTAS, 1, 1) __launch_bounds__(SS_THREADS, 1)
-    csr_leja_sweep_small_kernel(CsrOp op, const cplx* v, cplx* out, double inv_gamma, double c_over_gamma, double tol,
-                                int m_max, cplx phase, const __grid_constant__ SweepTable tab, LejaStatus* status) {
+    csr_leja_sweep_small_kernel(CsrOp op, const cplx* v, cplx* out, const SweepJob* __restrict__ jobs, int njobs,
+                                const double* __restrict__ leja_l, double tol, LejaStatus* status) {
   extern __shared__ __align__(16) unsigned char ss_smem[];
   __shared__ double sa[SS_THREADS / 32], sb[SS_THREADS / 32];
   __shared__ double part[2][2];                     // [iteration parity](sw, sp) of this CTA, read by the others
+  __shared__ double s_l[kMaxDegree + 1];            // Leja points (c2)
   cg::cluster_group cluster = cg::this_cluster();
   const int rank = (int)cluster.block_rank();
   if (status->pad) return;                          // an earlier sub-step did not converge (cluster-uniform)
@@ -77,6 +82,7 @@ __global__ void __cluster_dims__(SS_CTAS, 1, 1) __launch_bounds__(SS_THREADS, 1)
   const int n = (int)op.n;
   const int per = (n + SS_CTAS - 1) / SS_CTAS;
   const int r0 = min(n, rank * per), r1 = min(n, r0 + per);
+  for (int k = tid; k <= kMaxDegree; k += SS_THREADS) s_l[k] = leja_l[k];
 
   // the CTA's slice of every term -> shared memory (values, columns, local row pointers)
   cplx* prow = reinterpret_cast<cplx*>(ss_smem + SS_W_BYTES);    // p of the CTA's rows (kept out of registers so that
@@ -100,129 +106,185 @@ __global__ void __cluster_dims__(SS_CTAS, 1, 1) __launch_bounds__(SS_THREADS, 1)
     }
   }
 
-  // S5: every CTA copies the whole v (fixed-order norm, identical in all CTAs); p_0 for its own rows
-  double s0 = 0.0, s1 = 0.0;
-  for (int i = tid; i < n; i += SS_THREADS) {
-    const cplx x = v[i];
-    wbuf[0][i] = x;
-    s0 += x.x * x.x + x.y * x.y;
-  }
-  block_reduce_sum2_ss(s0, s1, sa, sb);
-  if (tid == 0) part[0][0] = s0;
+  // every CTA copies the whole v
+  for (int i = tid; i < n; i += SS_THREADS) wbuf[0][i] = v[i];
+  int cur = 0;
   __syncthreads();
-  s0 = part[0][0];
-  for (int r = r0 + tid; r < r1; r += SS_THREADS) prow[r - r0] = cmul(tab.d[0], wbuf[0][r]);
-  double e_prev = hypot(tab.d[0].x, tab.d[0].y) * sqrt(s0);
-  double err = 0.0, sw = 0.0, sp = 0.0;
-  int k = 0, cur = 0;
-  bool done = false;
   cluster.sync();                                   // everybody's buffers exist before remote writes start
 
-  while (!done && k < m_max) {
-    ++k;
-    const cplx dk = tab.d[k];
-    const double shift = c_over_gamma + tab.l[k - 1];
-    const cplx* w_in = wbuf[cur];
-    double bw = 0.0, bp = 0.0;
 #pragma unroll 1
-    for (int j = 0; j * SS_GROUPS < per; ++j) {     // S6 on the CTA's row slice
-      const int row = r0 + grp + j * SS_GROUPS;
-      const bool valid = row < r1;
-      cplx y = make_double2(0.0, 0.0);
-      for (int t = 0; t < op.nterms; ++t) {
-        const CsrTerm& T = op.t[t];
-        cplx a = make_double2(0.0, 0.0);
-        if (valid) {
-          if (cached) {
-            const int* lrp = mrp + t * (SS_MAX_ROWS + 1) + (row - r0);
-            const int qe = lrp[1];
-            for (int q = lrp[0] + sub; q < qe; q += SS_G) cfma(a, mval[q], w_in[mcol[q]]);
-          } else {
-            const int qe = T.rp[row + 1];
-            for (int q = T.rp[row] + sub; q < qe; q += SS_G) cfma(a, T.v[q], w_in[T.ci[q]]);
-          }
-        }
-        const cplx ca = cmul(T.coef, a);
-        y.x += ca.x;
-        y.y += ca.y;
-      }
+  for (int e = 0; e < njobs; ++e) {
+    const SweepJob& J = jobs[e];
+    const int m_max = J.m_max, nterms = min(J.nterms, op.nterms);
+    const double inv_gamma = J.inv_gamma, c_over_gamma = J.c_over_gamma;
+    cplx coef[3];
 #pragma unroll
-      for (int o = SS_G / 2; o > 0; o >>= 1) {
-        y.x += shfl_xor_d(y.x, o);
-        y.y += shfl_xor_d(y.y, o);
-      }
-      if (valid && sub == 0) {
-        const cplx wi = w_in[row];
-        cplx wn;
-        wn.x = inv_gamma * y.x - shift * wi.x;
-        wn.y = inv_gamma * y.y - shift * wi.y;
-        cplx pi = prow[row - r0];
-        cfma(pi, dk, wn);
-        prow[row - r0] = pi;
-        bw += wn.x * wn.x + wn.y * wn.y;
-        bp += pi.x * pi.x + pi.y * pi.y;
-        wbuf[cur ^ 1][row] = wn;                    // own slice, own copy; the other CTAs pull it after the barrier
-      }
-    }
-    block_reduce_sum2_ss(bw, bp, sa, sb);
-    if (tid == 0) {
-      part[k & 1][0] = bw;
-      part[k & 1][1] = bp;
-    }
-    cluster.sync();                                 // every CTA's slice of the new w and its partials are written
-    // pull the other CTAs' slices into the local copy through distributed shared memory (independent
-    // 16-byte loads, all in flight at once) and their partial norms
+    for (int t = 0; t < 3; ++t) coef[t] = J.coef[t];
+    // S5 (fixed-order norm, identical in all CTAs); p_0 for the CTA's own rows
+    double s0 = 0.0, s1 = 0.0;
     for (int i = tid; i < n; i += SS_THREADS) {
-      const int owner = i / per;
-      if (owner != rank) wbuf[cur ^ 1][i] = cluster.map_shared_rank(wbuf[cur ^ 1], owner)[i];
+      const cplx x = wbuf[cur][i];
+      s0 += x.x * x.x + x.y * x.y;
     }
-    double pw[SS_CTAS], pp[SS_CTAS];
+    block_reduce_sum2_ss(s0, s1, sa, sb);
+    if (tid == 0) part[0][0] = s0;
+    __syncthreads();
+    s0 = part[0][0];
+    const cplx d0 = J.d[0];
+    for (int r = r0 + tid; r < r1; r += SS_THREADS) prow[r - r0] = cmul(d0, wbuf[cur][r]);
+    double e_prev = hypot(d0.x, d0.y) * sqrt(s0);
+    double err = 0.0, sw = 0.0, sp = 0.0;
+    int k = 0;
+    bool done = false;
+    __syncthreads();                                // part[0] is rewritten by iteration 2 at the earliest, but keep S5 whole
+
+    while (!done && k < m_max) {
+      ++k;
+      const cplx dk = J.d[k];
+      const double shift = c_over_gamma + s_l[k - 1];
+      const cplx* w_in = wbuf[cur];
+      double bw = 0.0, bp = 0.0;
+#pragma unroll 1
+      for (int j = 0; j * SS_GROUPS < per; ++j) {     // S6 on the CTA's row slice
+        const int row = r0 + grp + j * SS_GROUPS;
+        const bool valid = row < r1;
+        cplx y = make_double2(0.0, 0.0);
+        for (int t = 0; t < nterms; ++t) {
+          const CsrTerm& T = op.t[t];
+          cplx a = make_double2(0.0, 0.0);
+          if (valid) {
+            if (cached) {
+              const int* lrp = mrp + t * (SS_MAX_ROWS + 1) + (row - r0);
+              const int qe = lrp[1];
+              for (int q = lrp[0] + sub; q < qe; q += SS_G) cfma(a, mval[q], w_in[mcol[q]]);
+            } else {
+              const int qe = T.rp[row + 1];
+              for (int q = T.rp[row] + sub; q < qe; q += SS_G) cfma(a, T.v[q], w_in[T.ci[q]]);
+            }
+          }
+          const cplx ca = cmul(coef[t], a);
+          y.x += ca.x;
+          y.y += ca.y;
+        }
 #pragma unroll
-    for (int c = 0; c < SS_CTAS; ++c) {
-      const double* remote = cluster.map_shared_rank(&part[k & 1][0], c);
-      pw[c] = remote[0];
-      pp[c] = remote[1];
-    }
-    sw = 0.0;
-    sp = 0.0;
+        for (int o = SS_G / 2; o > 0; o >>= 1) {
+          y.x += shfl_xor_d(y.x, o);
+          y.y += shfl_xor_d(y.y, o);
+        }
+        if (valid && sub == 0) {
+          const cplx wi = w_in[row];
+          cplx wn;
+          wn.x = inv_gamma * y.x - shift * wi.x;
+          wn.y = inv_gamma * y.y - shift * wi.y;
+          cplx pi = prow[row - r0];
+          cfma(pi, dk, wn);
+          prow[row - r0] = pi;
+          bw += wn.x * wn.x + wn.y * wn.y;
+          bp += pi.x * pi.x + pi.y * pi.y;
+          wbuf[cur ^ 1][row] = wn;                    // own slice, own copy; the other CTAs pull it after the barrier
+        }
+      }
+      block_reduce_sum2_ss(bw, bp, sa, sb);
+      if (tid == 0) {
+        part[k & 1][0] = bw;
+        part[k & 1][1] = bp;
+      }
+      cluster.sync();                                 // every CTA's slice of the new w and its partials are written
+      // pull the other CTAs' slices into the local copy through distributed shared memory (independent
+      // 16-byte loads, all in flight at once) and their partial norms
+      for (int i = tid; i < n; i += SS_THREADS) {
+        const int owner = i / per;
+        if (owner != rank) wbuf[cur ^ 1][i] = cluster.map_shared_rank(wbuf[cur ^ 1], owner)[i];
+      }
+      double pw[SS_CTAS], pp[SS_CTAS];
 #pragma unroll
-    for (int c = 0; c < SS_CTAS; ++c) {             // same order in every CTA: same decision
-      sw += pw[c];
-      sp += pp[c];
+      for (int c = 0; c < SS_CTAS; ++c) {
+        const double* remote = cluster.map_shared_rank(&part[k & 1][0], c);
+        pw[c] = remote[0];
+        pp[c] = remote[1];
+      }
+      sw = 0.0;
+      sp = 0.0;
+#pragma unroll
+      for (int c = 0; c < SS_CTAS; ++c) {             // same order in every CTA: same decision
+        sw += pw[c];
+        sp += pp[c];
+      }
+      __syncthreads();                                // local copy of w complete before the next gathers
+      const double e_k = hypot(dk.x, dk.y) * sqrt(sw);   // S7
+      err = e_k + e_prev;
+      e_prev = e_k;
+      done = err <= tol * sqrt(sp);
+      cur ^= 1;
     }
-    __syncthreads();                                // local copy of w complete before the next gathers
-    const double e_k = hypot(dk.x, dk.y) * sqrt(sw);   // S7
-    err = e_k + e_prev;
-    e_prev = e_k;
-    done = err <= tol * sqrt(sp);
-    cur ^= 1;
+    if (rank == 0 && tid == 0) {
+      LejaStatus* S = status + e;
+      S->done = done ? 1 : 0;
+      S->pad = done ? 0 : 1;
+      S->k = k;
+      S->iters += k;
+      S->err_est = err;
+      S->e_prev = e_prev;
+      S->norm_w2 = sw;
+      S->norm_p2 = sp;
+    }
+    if (!done) break;                                 // cluster-uniform: psi (global) is the state before this job
+    // S8: the result becomes the next job's input.  It goes into the buffer nobody pulls from any more
+    // (remote reads of this iteration target wbuf[cur]); the others fetch it after one barrier.
+    const cplx phase = J.phase;
+    const bool more = e + 1 < njobs;
+    for (int r = r0 + tid; r < r1; r += SS_THREADS) {
+      const cplx o = cmul(phase, prow[r - r0]);
+      out[r] = o;
+      if (more) wbuf[cur ^ 1][r] = o;
+    }
+    if (more) {
+      cluster.sync();
+      for (int i = tid; i < n; i += SS_THREADS) {
+        const int owner = i / per;
+        if (owner != rank) wbuf[cur ^ 1][i] = cluster.map_shared_rank(wbuf[cur ^ 1], owner)[i];
+      }
+      cur ^= 1;
+      __syncthreads();
+    }
   }
-  if (done)
-    for (int r = r0 + tid; r < r1; r += SS_THREADS) out[r] = cmul(phase, prow[r - r0]);   // S8
-  if (rank == 0 && tid == 0) {
-    status->done = done ? 1 : 0;
-    status->pad = done ? 0 : 1;
-    status->k = k;
-    status->iters += k;
-    status->err_est = err;
-    status->e_prev = e_prev;
-    status->norm_w2 = sw;
-    status->norm_p2 = sp;
-  }
-  cluster.sync();                                   // no CTA leaves while its shared memory may still be written
+  cluster.sync();                                   // no CTA leaves while its shared memory may still be read
 }
 
 }  // namespace
 
-int launch_csr_leja_sweep_small(const CsrOp& op, const cplx* v, cplx* out, double inv_gamma, double c_over_gamma,
-                                double tol, int m_max, cplx phase, const SweepTable& tab, Workspace* ws,
-                                cudaStream_t st) {
+int launch_csr_leja_sweep_small_jobs(const CsrOp& op, cplx* psi, const SweepJob* jobs, int njobs, const double* leja_l,
+                                     double tol, LejaStatus* status, Workspace* ws, cudaStream_t st) {
   // per launch (cheap): the attribute is per device, a process-wide flag would miss a second GPU
   if (cudaFuncSetAttribute(csr_leja_sweep_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SS_SMEM) !=
       cudaSuccess)
     return MAGNUS_ECUDA;
-  csr_leja_sweep_small_kernel<<<SS_CTAS, SS_THREADS, SS_SMEM, st>>>(op, v, out, inv_gamma, c_over_gamma, tol, m_max,
-                                                                    phase, tab, ws->status);
+  csr_leja_sweep_small_kernel<<<SS_CTAS, SS_THREADS, SS_SMEM, st>>>(op, psi, psi, jobs, njobs, leja_l, tol, status);
+  ws->launches += 1;
+  return cudaGetLastError() == cudaSuccess ? MAGNUS_OK : MAGNUS_ECUDA;
+}
+
+// one sweep (leja_expmv, sub-steps, the fall-back after a failed batch): a one-job batch through the job slot 0
+int launch_csr_leja_sweep_small(const CsrOp& op, const cplx* v, cplx* out, double inv_gamma, double c_over_gamma,
+                                double tol, int m_max, cplx phase, const SweepTable& tab, Workspace* ws,
+                                cudaStream_t st) {
+  if (ensure_sweep_jobs(ws) != MAGNUS_OK) return MAGNUS_ENOMEM;
+  SweepJob& J = ws->jobs_host[0];
+  for (int t = 0; t < 3; ++t) J.coef[t] = op.t[t].coef;
+  J.phase = phase;
+  J.inv_gamma = inv_gamma;
+  J.c_over_gamma = c_over_gamma;
+  J.m_max = m_max;
+  J.nterms = op.nterms;
+  J.flags = 0;
+  J.pad = 0;
+  for (int k = 0; k <= m_max; ++k) J.d[k] = tab.d[k];
+  if (cudaMemcpyAsync(ws->jobs, &J, sizeof(SweepJob), cudaMemcpyHostToDevice, st) != cudaSuccess) return MAGNUS_ECUDA;
+  if (cudaFuncSetAttribute(csr_leja_sweep_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SS_SMEM) !=
+      cudaSuccess)
+    return MAGNUS_ECUDA;
+  csr_leja_sweep_small_kernel<<<SS_CTAS, SS_THREADS, SS_SMEM, st>>>(op, v, out, ws->jobs, 1, ws->leja_l, tol,
+                                                                    ws->status);
   ws->launches += 1;
   return cudaGetLastError() == cudaSuccess ? MAGNUS_OK : MAGNUS_ECUDA;
 }

@@ -45,7 +45,9 @@ struct SliceLayout {
   int nterms = 0;
   int4* meta = nullptr;          // per 32-row slice: {first slot, slots, first slot of term 1, of term 2}
   int64_t* ent_ptr = nullptr;    // [nslices + 1]
+  bool offsets = false;          // offset-slot layout (csr_kernel 6): slot_rec instead of slot_mask + ci
   unsigned* slot_mask = nullptr; // [nslots] rows of the slice with an entry in the slot
+  uint2* slot_rec = nullptr;     // [nslots] {row mask, column - row}: all entries of a slot share column - row
   int32_t* ci = nullptr;         // [nent] columns, slot-major
   cplx* v = nullptr;             // [nent] values, same order
 };
@@ -84,6 +86,21 @@ struct SweepTable {
   double l[kMaxDegree + 1];   // Leja points l_k (c2)
 };
 
+// One exponential of a planned batch (the whole-sweep kernels: kernels_csr_small.cu, kernels_dense_sweep.cu).
+// The host plans a batch ahead -- the Gershgorin intervals do not depend on psi -- and uploads one job per
+// exponential; the kernel runs the jobs in order and stops at the first one that does not converge.
+struct SweepJob {
+  cplx coef[3];          // CSR: coefficient of each term; dense: coef[1].x = g of M = H0 + g H1
+  cplx phase;            // e^{-i h c} (c7)
+  double inv_gamma, c_over_gamma;
+  int m_max;             // degrees 1..m_max are available in d[]
+  int nterms;            // CSR terms this job uses (the handle's terms in order)
+  int flags;             // dense: kSweepJobAssembled = M is already in place (M4, M6), no assembly
+  int pad;
+  cplx d[kMaxDegree + 1];   // divided differences d_k (c3)
+};
+const int kSweepJobAssembled = 1;
+
 const int kMaxPartials = 4096;   // upper bound on blocks that write partial sums
 
 struct Workspace {
@@ -102,7 +119,21 @@ struct Workspace {
   double leja_ms = 0.0;
   bool time_leja = false;
   void* stream_maps = nullptr;       // stream kernel: cached TMA tensor maps of the operator's terms (host)
+  // planned batches (whole-sweep kernels), allocated on first use by ensure_sweep_jobs
+  SweepJob* jobs = nullptr;          // device [kJobCap]
+  SweepJob* jobs_host = nullptr;     // pinned [kJobCap]
+  LejaStatus* status_arr = nullptr;  // device [kJobCap]
+  LejaStatus* status_arr_host = nullptr;   // pinned [kJobCap]
+  double* ab_arr = nullptr;          // device [2 kJobCap]: Gershgorin bounds of the batch's exponentials
+  double* ab_arr_host = nullptr;     // pinned [2 kJobCap]
+  double* coef_arr = nullptr;        // device [4 kJobCap]: per-exponential scalars of the batched Gershgorin kernels
+  double* coef_arr_host = nullptr;   // pinned
+  double* leja_l = nullptr;          // device [kMaxDegree + 1]: Leja points (c2)
+  unsigned* grid_bar = nullptr;      // device: grid-barrier counter of the dense sweep kernel
+  double* sweep_partials = nullptr;  // device [2][2 * kMaxPartials]: per-CTA partial norms of the dense sweep kernel
 };
+const int kJobCap = 256;             // exponentials per planned batch
+int ensure_sweep_jobs(Workspace* ws);
 
 // cudaDevAttrMultiProcessorCount of the current device (cached per device; 148 on B200)
 int device_sm_count();
@@ -154,7 +185,14 @@ int launch_csr_leja_iter_stream(const CsrOp& op, const cplx* w_in, cplx* w_out, 
 
 // ---- kernels_csr_slice.cu ---------------------------------------------------
 // slice-major copy of op's terms (coefficients ignored); an error leaves *out empty and callers keep the CSR kernels
-int slice_layout_build(const CsrOp& op, SliceLayout* out, cudaStream_t st);
+// offsets: slots stored as {row mask, column - row} records and no column array (csr_kernel 6)
+int slice_layout_build(const CsrOp& op, SliceLayout* out, cudaStream_t st, bool offsets);
+// which slice layout a csr_kernel option asks for: 0 none, 1 with columns (5, 5000..5999), 2 offset slots (6, 6000..6999)
+inline int slice_layout_kind(int csr_kernel) {
+  if (csr_kernel == 5 || (csr_kernel >= 5000 && csr_kernel < 6000)) return 1;
+  if (csr_kernel == 6 || (csr_kernel >= 6000 && csr_kernel < 7000)) return 2;
+  return 0;
+}
 void slice_layout_free(SliceLayout* L);
 int launch_csr_leja_iter_slice(const CsrOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma, double shift,
                                cplx dk, double abs_dk, double tol, Workspace* ws, cudaStream_t st);
@@ -165,6 +203,10 @@ int launch_csr_leja_iter_slice(const CsrOp& op, const cplx* w_in, cplx* w_out, c
 int launch_csr_leja_sweep_small(const CsrOp& op, const cplx* v, cplx* out, double inv_gamma, double c_over_gamma,
                                  double tol, int m_max, cplx phase, const SweepTable& tab, Workspace* ws,
                                  cudaStream_t st);
+// a planned batch in ONE launch: psi <- exp(job[njobs-1]) ... exp(job[0]) psi; status[e] per job (zeroed by the
+// caller); stops at the first job that does not converge within its m_max (status[e].pad = 1, psi = state before it)
+int launch_csr_leja_sweep_small_jobs(const CsrOp& op, cplx* psi, const SweepJob* jobs, int njobs, const double* leja_l,
+                                      double tol, LejaStatus* status, Workspace* ws, cudaStream_t st);
 
 // ---- kernels_dense.cu -------------------------------------------------------
 int launch_dense_gershgorin(const DenseOp& op, Workspace* ws, cudaStream_t st);

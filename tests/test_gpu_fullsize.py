@@ -20,6 +20,9 @@ from workloads import rng
 
 pytestmark = pytest.mark.gpu
 DEV = "cuda"
+# what a handle selects by default for n >= 32768 on well-filled slots (api.cu: kSliceAutoMinN); the single-iteration
+# entry point builds no layout unless asked to
+BENCH_CSR_KERNEL = 6
 
 
 @pytest.fixture(scope="module")
@@ -66,7 +69,7 @@ def test_cfg5_fused_iteration_sampled_rows(M, oracle, cfg5_inputs):
     p = rng.random_unit_vector(n, stream=9, device=DEV)
     p_before = p.clone()
     wo = torch.empty_like(w)
-    sw, sp, _ = M.magnus_leja_iteration(H0, H1, g, w, wo, p, inv_gamma, shift, d)
+    sw, sp, _ = M.magnus_leja_iteration(H0, H1, g, w, wo, p, inv_gamma, shift, d, csr_kernel=BENCH_CSR_KERNEL)
     r = np.random.default_rng(5)
     starts = np.concatenate([[0, n - 64], r.integers(0, n // 64, size=46) * 64])
     rows = torch.from_numpy(np.concatenate([np.arange(s, s + 64) for s in starts])).to(DEV)

@@ -126,7 +126,7 @@ def expected_iteration(oracle, Mh, w, p, inv_gamma, shift, d):
     return wn, pn
 
 
-@pytest.mark.parametrize("N,kernel", [(8, 1), (12, 1), (12, 2), (15, 2), (16, 0), (8, 3), (12, 3), (16, 3), (16, 24001), (16, 27081), (16, 22040), (8, 4), (12, 4), (16, 4), (3, 5), (8, 5), (12, 5), (16, 5), (16, 5083), (16, 5045)])
+@pytest.mark.parametrize("N,kernel", [(8, 1), (12, 1), (12, 2), (15, 2), (16, 0), (8, 3), (12, 3), (16, 3), (16, 24001), (16, 27081), (16, 22040), (8, 4), (12, 4), (16, 4), (3, 5), (8, 5), (12, 5), (16, 5), (16, 5083), (16, 5045), (3, 6), (8, 6), (12, 6), (16, 6), (16, 6003), (16, 6104), (16, 6204), (16, 6016), (12, 6018)])
 def test_fused_iteration_csr_xxz(M, oracle, N, kernel):
     n = 1 << N
     H0, H1 = xxz.xxz_h0(N), xxz.xxz_h1(N)
@@ -146,7 +146,7 @@ def test_fused_iteration_csr_xxz(M, oracle, N, kernel):
     assert math.isclose(sp, np.sum(np.abs(pn) ** 2), rel_tol=1e-12)
 
 
-@pytest.mark.parametrize("kernel,long_len", [(1, 1900), (2, 1900), (3, 1900), (3, 2990), (27001, 2990), (22030, 700), (23000, 40), (4, 1900), (4, 40), (5, 1900), (5, 40), (5045, 300)])
+@pytest.mark.parametrize("kernel,long_len", [(1, 1900), (2, 1900), (3, 1900), (3, 2990), (27001, 2990), (22030, 700), (23000, 40), (4, 1900), (4, 40), (5, 1900), (5, 40), (5045, 300), (6, 1900), (6, 40), (6003, 300)])
 def test_fused_iteration_csr_general_ragged(M, oracle, kernel, long_len):
     """Non-power-of-two n, empty rows, one row longer than the row-block staging buffer / than a ring stage of
     the stream kernel (kernel 3 and its 2000+ variants: that unit is read straight from global memory), rows
