@@ -103,6 +103,34 @@ static int launch_iter(const OpRef& op, const cplx* w_in, cplx* w_out, cplx* p, 
                   : launch_csr_leja_iter(op.csr, w_in, w_out, p, inv_gamma, shift, dk, abs_dk, tol, ws, st);
 }
 
+// Divided differences of one exponential (c3), computed lazily: first the terms a sweep can possibly need
+// for this theta, the rest (up to m_max) only if the stop test asks for more.
+struct LejaTable {
+  double theta;
+  int full, have;
+  double tol;
+  int m_max;
+  std::vector<std::complex<double>> d;
+  LejaTable(double theta_, const LejaParams& prm)
+      : theta(theta_), full(prm.m_max + 1), tol(prm.tol), m_max(prm.m_max), d((size_t)prm.m_max + 1) {
+    have = std::min(full, std::max(16, (int)std::ceil(2.5 * std::fabs(theta)) + 20));
+    divided_differences(theta, have, d.data());
+  }
+  void need(int k) {   // grows geometrically: a longer table costs O(length^2) host work
+    if (k < have) return;
+    while (k >= have) have = std::min(full, 2 * have);
+    divided_differences(theta, have, d.data());
+  }
+  // a-priori length of the first chunk: first k with |d_k| + |d_{k-1}| <= tol, plus 2
+  int first_chunk() {
+    for (int k = 1; k <= m_max; ++k) {
+      need(k);
+      if (std::abs(d[k]) + std::abs(d[k - 1]) <= tol) return std::min(m_max, k + 2);
+    }
+    return m_max;
+  }
+};
+
 // ---------------------------------------------------------------------------
 // exp(-i h M) v on the RAW Gershgorin interval [a_raw, b_raw] of M (S4-S8).
 //   B = (M - cI)/gamma, theta = (h/s) gamma, d_k = exp(-i theta x)[l_0..l_k]        (c3)
@@ -140,25 +168,11 @@ static int expmv_on_interval(const OpRef& op, double a_raw, double b_raw, const 
   loc.theta = theta;
 
   const double* l = leja_points();
-  const int full = prm.m_max + 1;
-  int have = std::min(full, std::max(24, (int)std::ceil(2.5 * std::fabs(theta)) + 32));
-  std::vector<std::complex<double>> d(full);
-  divided_differences(theta, have, d.data());
-  auto need = [&](int k) {
-    if (k >= have) {
-      have = full;
-      divided_differences(theta, have, d.data());
-    }
-  };
-  // a-priori length of the first chunk: first k with |d_k| + |d_{k-1}| <= tol, plus 2
-  int first_chunk = prm.m_max;
-  for (int k = 1; k <= prm.m_max; ++k) {
-    need(k);
-    if (std::abs(d[k]) + std::abs(d[k - 1]) <= prm.tol) {
-      first_chunk = std::min(prm.m_max, k + 2);
-      break;
-    }
-  }
+  LejaTable T(theta, prm);
+  std::vector<std::complex<double>>& d = T.d;
+  int& have = T.have;
+  auto need = [&](int k) { T.need(k); };
+  const int first_chunk = T.first_chunk();
 
   const double inv_gamma = 1.0 / gamma, c_over_gamma = c / gamma;
   const cplx phase = make_double2(std::cos(hs * c), -std::sin(hs * c));
@@ -356,6 +370,375 @@ static int csr_cache_rowstats(magnus_context* h) {
   return MAGNUS_OK;
 }
 
+// ---------------------------------------------------------------------------
+// Planned batches (small and medium problems, where a step is a handful of microseconds of kernel time
+// and every host round trip shows).  The Gershgorin interval of an exponential depends on t only, not
+// on psi, so a run of steps is planned ahead: every interval of the batch first (one host sync), the
+// tables d_k on the host, one SweepJob per exponential, then the whole-sweep kernel runs the jobs back
+// to back with no host in between and the host reads all the stop-test records at the end (second
+// sync).  A job that does not meet tol within its table stops the batch with psi untouched by it; the
+// host redoes that exponential on the stepwise path and resumes the batch behind it.
+// ---------------------------------------------------------------------------
+struct ExpSpec {
+  double g;       // coefficient of H1
+  double kappa;   // CSR M4: the coefficient of C = [H0, H1] is -i kappa
+  int nterms;     // CSR terms in use
+  double h;       // the exponential is exp(-i h M)
+};
+
+static void csr_op_from_spec(const magnus_context* h, const ExpSpec& sp, CsrOp* op) {
+  op->n = h->n;
+  op->nterms = sp.nterms;
+  op->t[0] = csr_term(&h->H0, 1.0, 0.0);
+  op->t[1] = csr_term(&h->H1, sp.g, 0.0);
+  op->t[2] = op->t[1];
+  if (h->c_v) {   // Omega_H = H0 + fbar H1 - i kappa [H0, H1]   (c1; [H(t2),H(t1)] = (f1 - f2)[H0,H1])
+    CsrTerm c;
+    c.rp = h->c_rp;
+    c.ci = h->c_ci;
+    c.v = h->c_v;
+    c.coef = make_double2(0.0, -sp.kappa);
+    c.nnz = h->c_nnz;
+    op->t[2] = c;
+  }
+  op->unit_cap = sp.nterms == 3 ? h->unit_cap3 : h->unit_cap2;
+  op->slice = h->slice.meta ? &h->slice : nullptr;
+}
+
+// the exponentials of one step (S1) for the operators that are a plain combination of stored terms:
+// commutator-free schemes on either format, and M4 on CSR with its cached commutator
+static int step_specs(magnus_context* h, double t, double tau, ExpSpec* out) {
+  double coef[MAGNUS_MAX_EXP_PER_STEP], hscale[MAGNUS_MAX_EXP_PER_STEP], kappa = 0.0;
+  const int n_exp = step_coefficients(h->scheme, h->f, h->user, t, tau, coef, hscale, &kappa);
+  for (int e = 0; e < n_exp; ++e) {
+    out[e].g = coef[e];
+    out[e].kappa = 0.0;
+    out[e].nterms = 2;
+    out[e].h = hscale[e] * tau;
+  }
+  if (h->scheme == MAGNUS_M4 && h->format == MAGNUS_CSR) {
+    out[0].g = 0.5 * (coef[0] + coef[1]);
+    out[0].kappa = kappa;
+    out[0].nterms = (h->c_nnz > 0 && kappa != 0.0) ? 3 : 2;
+  }
+  return n_exp;
+}
+
+static bool plan_supported(const magnus_context* h) {
+  if (h->format == MAGNUS_CSR) return h->n <= kSmallSweepMaxN && h->ws.csr_kernel == 0;
+  // dense: the commutator-free schemes (M = H0 + g H1 per exponential); M4 / M6 build Omega_H per step
+  return h->scheme != MAGNUS_M4 && h->scheme != MAGNUS_M6 && dense_sweep_supported(h->n) && h->ws.csr_kernel == 0;
+}
+
+const int kPlanDeclined = 1;   // internal: not a planned-path handle after all
+
+// Steps s0 .. s0 + ns - 1 of the grid t0 + s tau (at most kPlanCap exponentials); infos (nullable) gets one entry
+// per step.  Host planning (tables, jobs) of launch i + 1 overlaps the device's work on launch i: jobs go
+// through a ring of kJobRing slots of kJobsPerLaunch jobs, each guarded by the event of its last launch.
+static int run_planned(magnus_context* h, double t0, double tau, int64_t s0, int ns, cplx* psi, magnus_step_info* infos) {
+  Workspace* ws = &h->ws;
+  cudaStream_t st = h->stream;
+  if (ensure_sweep_jobs(ws) != MAGNUS_OK) { set_error("planned batch: buffer allocation failed"); return MAGNUS_ENOMEM; }
+  std::vector<ExpSpec> specs;
+  std::vector<int> first_of_step((size_t)ns + 1, 0);
+  for (int s = 0; s < ns; ++s) {
+    ExpSpec sp[MAGNUS_MAX_EXP_PER_STEP];
+    const int n_exp = step_specs(h, t0 + (double)(s0 + s) * tau, tau, sp);   // S1
+    first_of_step[s] = (int)specs.size();
+    for (int e = 0; e < n_exp; ++e) specs.push_back(sp[e]);
+  }
+  const int E = (int)specs.size();
+  first_of_step[ns] = E;
+  if (E > kPlanCap) { set_error("planned batch too long"); return MAGNUS_EINVAL; }
+
+  const bool dense = h->format == MAGNUS_DENSE;
+  const cplx* H0v = (const cplx*)h->H0.values;
+  const cplx* H1v = (const cplx*)h->H1.values;
+  std::vector<double> ab((size_t)2 * E);   // raw Gershgorin bounds of every exponential
+  // S3 for the whole batch: one launch when the cached row statistics apply to every exponential
+  bool all_cached = !dense;
+  for (int e = 0; e < E; ++e)
+    all_cached = all_cached && ((specs[e].nterms == 2 && h->gs_disjoint2) || (specs[e].nterms == 3 && h->gs_disjoint3));
+  if (all_cached || dense) {
+    for (int e = 0; e < E; ++e) {
+      ws->coef_arr_host[4 * e] = specs[e].g;
+      ws->coef_arr_host[4 * e + 1] = specs[e].kappa;
+      ws->coef_arr_host[4 * e + 2] = (double)specs[e].nterms;
+      ws->coef_arr_host[4 * e + 3] = 0.0;
+    }
+    CU_TRY(cudaMemcpyAsync(ws->coef_arr, ws->coef_arr_host, sizeof(double) * 4 * (size_t)E, cudaMemcpyHostToDevice, st));
+    if (dense) {
+      if (launch_dense_gershgorin_batch(h->n, H0v, dense_ld(&h->H0), H1v, dense_ld(&h->H1), ws->coef_arr, E, ws->ab_arr, ws,
+                                        st) != MAGNUS_OK) {
+        set_error("batched Gershgorin launch failed");
+        return MAGNUS_ECUDA;
+      }
+    } else {
+      launch_csr_gershgorin_cached_batch(h->n, h->gs_r, h->gs_diag, h->gs_r[2] ? 3 : 2, ws->coef_arr, E, ws->ab_arr, ws, st);
+    }
+  } else {
+    for (int e = 0; e < E; ++e) {
+      CsrOp op;
+      csr_op_from_spec(h, specs[e], &op);
+      ws->ab_out = ws->ab_arr + 2 * e;
+      if ((op.nterms == 2 && h->gs_disjoint2) || (op.nterms == 3 && h->gs_disjoint3))
+        launch_csr_gershgorin_cached(op, h->gs_r, h->gs_diag, ws, st);
+      else
+        launch_csr_gershgorin(op, ws, st);
+    }
+    ws->ab_out = nullptr;
+  }
+  CU_TRY(cudaMemcpyAsync(ws->ab_arr_host, ws->ab_arr, sizeof(double) * 2 * (size_t)E, cudaMemcpyDeviceToHost, st));
+  CU_TRY(cudaMemsetAsync(ws->status_arr, 0, sizeof(LejaStatus) * (size_t)E, st));
+  CU_TRY(cudaStreamSynchronize(st));
+  if (dense) dense_gershgorin_batch_decode(ws->ab_arr_host, E, ab.data());
+  else std::memcpy(ab.data(), ws->ab_arr_host, sizeof(double) * 2 * (size_t)E);
+
+  // S4, cheap part: interval -> (c, gamma, theta); an exponential the sweep kernel does not take (gamma = 0,
+  // sub-steps, non-finite bounds) is done on the stepwise path when the plan reaches it
+  std::vector<magnus_expmv_info> plan((size_t)E);
+  std::vector<double> cc((size_t)E), gg((size_t)E);
+  std::vector<char> plannable((size_t)E);
+  for (int e = 0; e < E; ++e) {
+    double a = ab[2 * e], b = ab[2 * e + 1];
+    std::memset(&plan[e], 0, sizeof plan[e]);
+    plannable[e] = 0;
+    if (!std::isfinite(a) || !std::isfinite(b)) continue;
+    snap_interval(&a, &b);
+    cc[e] = 0.5 * (a + b);
+    gg[e] = 0.25 * (b - a);
+    if (!(gg[e] > 0.0) || std::fabs(specs[e].h * gg[e]) > h->prm.theta_max) continue;
+    plannable[e] = 1;
+    plan[e].a = a;
+    plan[e].b = b;
+    plan[e].theta = specs[e].h * gg[e];
+    plan[e].substeps = 1;
+  }
+
+  CsrOp op_all;   // every term the handle has; a job says how many it uses and with which coefficients
+  if (!dense) {
+    ExpSpec widest = specs[0];
+    widest.nterms = h->c_v && h->c_nnz > 0 ? 3 : 2;
+    csr_op_from_spec(h, widest, &op_all);
+  }
+  auto stepwise = [&](int e) {
+    OpRef ref;
+    if (dense) {   // S2 (+S3, unused: the bounds are known) into the handle's matrix, then the per-iteration kernels
+      launch_dense_assemble(h->n, H0v, dense_ld(&h->H0), H1v, dense_ld(&h->H1), specs[e].g, h->M, ws, st);
+      ref.dense = true;
+      ref.dns.n = h->n;
+      ref.dns.ld = h->n;
+      ref.dns.M = h->M;
+    } else {
+      ref.dense = false;
+      csr_op_from_spec(h, specs[e], &ref.csr);
+    }
+    return expmv_on_interval(ref, ab[2 * e], ab[2 * e + 1], psi, psi, specs[e].h, h->prm, ws, st, &plan[e]);
+  };
+  bool slot_used[kJobRing];
+  auto drain_slot = [&](int slot) {   // the launch that used the slot is over: its time, and the slot is free
+    if (!slot_used[slot]) return;
+    cudaEventSynchronize(ws->ring_ev[2 * slot + 1]);
+    if (ws->time_leja) {
+      float ms = 0.f;
+      if (cudaEventElapsedTime(&ms, ws->ring_ev[2 * slot], ws->ring_ev[2 * slot + 1]) == cudaSuccess) ws->leja_ms += ms;
+    }
+    slot_used[slot] = false;
+  };
+
+  int rc = MAGNUS_OK, seg = 0;   // exponentials before seg are done
+  while (seg < E && rc == MAGNUS_OK) {
+    int seg_end = seg;
+    while (seg_end < E && plannable[seg_end]) ++seg_end;
+    // S4 (tables) and S5-S8 of [seg, seg_end): launches of a few jobs each, planned while the device works
+    for (int i = 0; i < kJobRing; ++i) slot_used[i] = false;
+    int e_next = seg, li = 0;
+    while (e_next < seg_end) {
+      const int slot = li % kJobRing;
+      drain_slot(slot);
+      const int nj = std::min(li == 0 ? 4 : kJobsPerLaunch, seg_end - e_next);   // a short first launch starts the device early
+      SweepJob* jh = ws->jobs_host + (size_t)slot * kJobsPerLaunch;
+      SweepJob* jd = ws->jobs + (size_t)slot * kJobsPerLaunch;
+      for (int i = 0; i < nj; ++i) {
+        const int e = e_next + i;
+        const double hh = specs[e].h, c = cc[e], gamma = gg[e];
+        LejaTable T(plan[e].theta, h->prm);
+        const int m_try = std::min(h->prm.m_max, std::max(T.have - 1, T.first_chunk()));
+        T.need(m_try);
+        SweepJob& J = jh[i];
+        J.coef[0] = make_double2(1.0, 0.0);
+        J.coef[1] = make_double2(specs[e].g, 0.0);
+        J.coef[2] = make_double2(0.0, -specs[e].kappa);
+        J.phase = make_double2(std::cos(hh * c), -std::sin(hh * c));
+        J.inv_gamma = 1.0 / gamma;
+        J.c_over_gamma = c / gamma;
+        J.m_max = m_try;
+        J.nterms = specs[e].nterms;
+        J.flags = 0;
+        J.pad = 0;
+        for (int k = 0; k <= m_try; ++k) J.d[k] = make_double2(T.d[k].real(), T.d[k].imag());
+      }
+      CU_TRY(cudaMemcpyAsync(jd, jh, sizeof(SweepJob) * (size_t)nj, cudaMemcpyHostToDevice, st));
+      CU_TRY(cudaEventRecord(ws->ring_ev[2 * slot], st));
+      const LejaStatus* gate = e_next > seg ? ws->status_arr + e_next - 1 : nullptr;
+      const int lrc = dense ? launch_dense_leja_sweep_jobs(h->n, H0v, dense_ld(&h->H0), H1v, dense_ld(&h->H1), h->M, psi, jd,
+                                                           nj, h->prm.tol, ws->status_arr + e_next, gate, ws, st)
+                            : launch_csr_leja_sweep_small_jobs(op_all, psi, jd, nj, ws->leja_l, h->prm.tol,
+                                                               ws->status_arr + e_next, gate, ws, st);
+      if (lrc != MAGNUS_OK) {
+        set_error("whole-sweep launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+        return MAGNUS_ECUDA;
+      }
+      CU_TRY(cudaEventRecord(ws->ring_ev[2 * slot + 1], st));
+      slot_used[slot] = true;
+      e_next += nj;
+      ++li;
+    }
+    int e = seg;
+    if (seg_end > seg) {
+      CU_TRY(cudaMemcpyAsync(ws->status_arr_host + seg, ws->status_arr + seg, sizeof(LejaStatus) * (size_t)(seg_end - seg),
+                             cudaMemcpyDeviceToHost, st));
+      CU_TRY(cudaStreamSynchronize(st));
+      for (int i = 0; i < kJobRing; ++i) drain_slot(i);
+      for (; e < seg_end && ws->status_arr_host[e].done; ++e) {
+        plan[e].iters = ws->status_arr_host[e].iters;
+        plan[e].err_est = ws->status_arr_host[e].err_est;
+      }
+      if (e < seg_end)   // the launches behind a failed job did nothing: forget their records
+        CU_TRY(cudaMemsetAsync(ws->status_arr + e, 0, sizeof(LejaStatus) * (size_t)(seg_end - e), st));
+    }
+    // e == seg_end: the segment is through and exponential seg_end (if any) is not for the sweep kernel;
+    // e <  seg_end: job e did not converge within its table and psi is the state before it.  Stepwise either way.
+    if (e < E) {
+      rc = stepwise(e);
+      ++e;
+    }
+    seg = e;
+  }
+  if (infos)
+    for (int s = 0; s < ns; ++s) {
+      std::memset(&infos[s], 0, sizeof infos[s]);
+      infos[s].n_exp = first_of_step[s + 1] - first_of_step[s];
+      for (int e = first_of_step[s]; e < first_of_step[s + 1]; ++e) infos[s].exp[e - first_of_step[s]] = plan[e];
+    }
+  return rc;
+}
+
+// One step on the stepwise path: interval, table and stop polling per exponential (rows S1-S8, D3, D4).
+static int magnus_step_unplanned(magnus_context* h, double t, double tau, cplx* psi, magnus_step_info* info) {
+  double coef[MAGNUS_MAX_EXP_PER_STEP], hscale[MAGNUS_MAX_EXP_PER_STEP], kappa = 0.0;
+  const int n_exp = step_coefficients(h->scheme, h->f, h->user, t, tau, coef, hscale, &kappa);   // S1
+  if (info) {
+    std::memset(info, 0, sizeof *info);
+    info->n_exp = n_exp;
+  }
+  cudaStream_t st = h->stream;
+  Workspace* ws = &h->ws;
+  int rc = MAGNUS_OK;
+  for (int e = 0; e < n_exp && rc == MAGNUS_OK; ++e) {
+    OpRef op;
+    double a = 0.0, b = 0.0;
+    if (h->format == MAGNUS_CSR) {
+      op.dense = false;
+      op.csr.n = h->n;
+      if (h->scheme == MAGNUS_M4) {
+        // Omega_H = H0 + fbar H1 - i kappa [H0, H1]   (c1; [H(t2),H(t1)] = (f1 - f2)[H0,H1])
+        op.csr.nterms = (h->c_nnz > 0 && kappa != 0.0) ? 3 : 2;
+        op.csr.t[0] = csr_term(&h->H0, 1.0, 0.0);
+        op.csr.t[1] = csr_term(&h->H1, 0.5 * (coef[0] + coef[1]), 0.0);
+        CsrTerm c;
+        c.rp = h->c_rp;
+        c.ci = h->c_ci;
+        c.v = h->c_v;
+        c.coef = make_double2(0.0, -kappa);
+        c.nnz = h->c_nnz;
+        op.csr.t[2] = c;
+      } else {
+        op.csr.nterms = 2;
+        op.csr.t[0] = csr_term(&h->H0, 1.0, 0.0);
+        op.csr.t[1] = csr_term(&h->H1, coef[e], 0.0);
+        op.csr.t[2] = op.csr.t[1];
+      }
+      op.csr.unit_cap = op.csr.nterms == 3 ? h->unit_cap3 : h->unit_cap2;
+      op.csr.slice = h->slice.meta ? &h->slice : nullptr;
+      if ((op.csr.nterms == 2 && h->gs_disjoint2) || (op.csr.nterms == 3 && h->gs_disjoint3)) {     // S3
+        const int nblk = launch_csr_gershgorin_cached(op.csr, h->gs_r, h->gs_diag, ws, st);
+        rc = read_interval(nblk, ws, st, &a, &b);
+      } else {
+        rc = op_interval(op, ws, st, &a, &b);
+      }
+    } else {
+      op.dense = true;
+      const cplx* H0v = (const cplx*)h->H0.values;
+      const cplx* H1v = (const cplx*)h->H1.values;
+      int nblk = 0;
+      if (h->scheme == MAGNUS_M6) {
+        // P:103-114 with A = -iH (reading m6); X1 = h->M, X2 = h->A2, X3 = h->P, X4, X5; see magnus.h at magnus_step
+        const int64_t n = h->n;
+        const double f1 = coef[0], f2 = coef[1], f3 = coef[2];
+        const double b2 = (std::sqrt(15.0) / 3.0) * tau * (f3 - f1), b3 = (10.0 / 3.0) * tau * (f3 - 2.0 * f2 + f1);
+        LinComb lc;
+        auto term = [&](int k, const cplx* x, double re, double im) {
+          lc.x[k] = x;
+          lc.c[k] = make_double2(re, im);
+        };
+        term(0, H0v, 1.0, 0.0); term(1, H1v, f2, 0.0); term(2, nullptr, 0.0, 0.0); term(3, nullptr, 0.0, 0.0);
+        if (dense_ld(&h->H0) != n || dense_ld(&h->H1) != n) { set_error("MAGNUS_M6 needs ld == n"); rc = MAGNUS_EINVAL; break; }
+        launch_dense_lincomb(n, h->M, lc, ws, st);                                   // X1 = H2 = H0 + f2 H1
+        if (h->time_comm) cudaEventRecord(h->ev_comm[0], st);
+        rc = launch_zgemm(n, h->M, n, H1v, n, h->A2, n, st);                          // X2 = P1 = H2 H1
+        if (rc) break;
+        launch_dense_antiherm(n, h->A2, h->P, -1.0, st);                              // X3 = G = P1 - P1^H = [H2, H1]
+        rc = launch_zgemm(n, h->M, n, h->P, n, h->A2, n, st);                         // X2 = P2 = H2 G
+        if (rc) break;
+        launch_dense_antiherm(n, h->A2, h->X4, 1.0, st);                              // X4 = S = P2 + P2^H = [H2, G]
+        term(0, h->M, 0.0, 20.0 * tau); term(1, H1v, 0.0, b3); term(2, h->P, -tau * b2, 0.0); term(3, nullptr, 0.0, 0.0);
+        launch_dense_lincomb(n, h->A2, lc, ws, st);                                  // X2 = L
+        term(0, H1v, 0.0, -b2); term(1, h->P, tau * b3 / 30.0, 0.0); term(2, h->X4, 0.0, -tau * tau * b2 / 60.0);
+        term(3, nullptr, 0.0, 0.0);
+        launch_dense_lincomb(n, h->X5, lc, ws, st);                                  // X5 = R
+        rc = launch_zgemm(n, h->A2, n, h->X5, n, h->X4, n, st);                       // X4 = P3 = L R
+        ws->launches += 5;
+        if (h->time_comm) cudaEventRecord(h->ev_comm[1], st);
+        if (rc) break;
+        // Omega_H = H2 + (b3/(12 tau)) H1 + (i/(240 tau)) (P3 - P3^H), over X1, with its Gershgorin bounds
+        nblk = launch_dense_omega(n, h->M, H1v, h->X4, 1.0, b3 / (12.0 * tau), -1.0 / (240.0 * tau), ws, st);
+      } else if (h->scheme == MAGNUS_M4 && h->cached_p0) {
+        // shortcut: Omega_H = H0 + fbar H1 - i kappa (P0 - P0^H), kappa = (sqrt(3) tau/12)(f1 - f2), no GEMM
+        LinComb lc;
+        lc.x[0] = H0v; lc.c[0] = make_double2(1.0, 0.0);
+        lc.x[1] = H1v; lc.c[1] = make_double2(0.5 * (coef[0] + coef[1]), 0.0);
+        lc.x[2] = lc.x[3] = nullptr; lc.c[2] = lc.c[3] = make_double2(0.0, 0.0);
+        launch_dense_lincomb(h->n, h->M, lc, ws, st);
+        nblk = launch_dense_omega(h->n, h->M, H1v, h->P, 1.0, 0.0, kappa, ws, st);
+      } else if (h->scheme == MAGNUS_M4) {
+        launch_dense_assemble2(h->n, H0v, dense_ld(&h->H0), H1v, dense_ld(&h->H1), coef[0], coef[1], h->M, h->A2, ws,
+                               st);                                                                // S2: A1, A2
+        if (h->time_comm) cudaEventRecord(h->ev_comm[0], st);
+        rc = launch_zgemm(h->n, h->A2, h->n, h->M, h->n, h->P, h->n, st);                          // D3: P = A2 A1
+        ws->launches += 1;
+        if (h->time_comm) cudaEventRecord(h->ev_comm[1], st);
+        if (rc) { set_error("zgemm launch failed: %s", cudaGetErrorString(cudaGetLastError())); break; }
+        nblk = launch_dense_omega(h->n, h->M, h->A2, h->P, 0.5, 0.5, std::sqrt(3.0) * tau / 12.0, ws, st);   // D4 (+S3)
+      } else {
+        nblk = launch_dense_assemble(h->n, H0v, dense_ld(&h->H0), H1v, dense_ld(&h->H1), coef[e], h->M, ws, st);
+      }
+      op.dns.n = h->n;
+      op.dns.ld = h->n;
+      op.dns.M = h->M;
+      rc = read_interval(nblk, ws, st, &a, &b);
+      if (rc == MAGNUS_OK && h->time_comm) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, h->ev_comm[0], h->ev_comm[1]) == cudaSuccess) h->comm_ms += ms;
+      }
+    }
+    if (rc) break;
+    rc = expmv_on_interval(op, a, b, psi, psi, hscale[e] * tau, h->prm, ws, st, info ? &info->exp[e] : nullptr);
+  }
+  return rc;
+}
+
+
 extern "C" {
 
 const char* magnus_strerror(int code) {
@@ -431,6 +814,7 @@ int magnus_describe(magnus_handle h, magnus_path_info* out) {
   const char* name = "dense_leja_iter_kernel";
   if (h->format == MAGNUS_DENSE) {
     out->bytes_per_iteration = 16 * n * n + 64 * n;
+    if (plan_supported(h)) name = "dense_leja_sweep_kernel";
   } else {
     int64_t nnz = h->H0.nnz + h->H1.nnz, terms = 2;
     if (h->scheme == MAGNUS_M4 && h->c_nnz > 0) {
@@ -611,116 +995,11 @@ int magnus_create(magnus_handle* out, const magnus_matrix* H0, const magnus_matr
 int magnus_step(magnus_handle h, double t, double tau, void* psi_, magnus_step_info* info) {
   if (!h || !psi_) { set_error("magnus_step: NULL handle or psi"); return MAGNUS_EINVAL; }
   cplx* psi = (cplx*)psi_;
-  double coef[MAGNUS_MAX_EXP_PER_STEP], hscale[MAGNUS_MAX_EXP_PER_STEP], kappa = 0.0;
-  const int n_exp = step_coefficients(h->scheme, h->f, h->user, t, tau, coef, hscale, &kappa);   // S1
-  if (info) {
-    std::memset(info, 0, sizeof *info);
-    info->n_exp = n_exp;
+  if (plan_supported(h)) {   // a batch of one step: two host syncs instead of two per exponential
+    const int rc = run_planned(h, t, tau, 0, 1, psi, info);
+    if (rc != kPlanDeclined) return rc;
   }
-  cudaStream_t st = h->stream;
-  Workspace* ws = &h->ws;
-  int rc = MAGNUS_OK;
-  for (int e = 0; e < n_exp && rc == MAGNUS_OK; ++e) {
-    OpRef op;
-    double a = 0.0, b = 0.0;
-    if (h->format == MAGNUS_CSR) {
-      op.dense = false;
-      op.csr.n = h->n;
-      if (h->scheme == MAGNUS_M4) {
-        // Omega_H = H0 + fbar H1 - i kappa [H0, H1]   (c1; [H(t2),H(t1)] = (f1 - f2)[H0,H1])
-        op.csr.nterms = (h->c_nnz > 0 && kappa != 0.0) ? 3 : 2;
-        op.csr.t[0] = csr_term(&h->H0, 1.0, 0.0);
-        op.csr.t[1] = csr_term(&h->H1, 0.5 * (coef[0] + coef[1]), 0.0);
-        CsrTerm c;
-        c.rp = h->c_rp;
-        c.ci = h->c_ci;
-        c.v = h->c_v;
-        c.coef = make_double2(0.0, -kappa);
-        c.nnz = h->c_nnz;
-        op.csr.t[2] = c;
-      } else {
-        op.csr.nterms = 2;
-        op.csr.t[0] = csr_term(&h->H0, 1.0, 0.0);
-        op.csr.t[1] = csr_term(&h->H1, coef[e], 0.0);
-        op.csr.t[2] = op.csr.t[1];
-      }
-      op.csr.unit_cap = op.csr.nterms == 3 ? h->unit_cap3 : h->unit_cap2;
-      op.csr.slice = h->slice.meta ? &h->slice : nullptr;
-      if ((op.csr.nterms == 2 && h->gs_disjoint2) || (op.csr.nterms == 3 && h->gs_disjoint3)) {     // S3
-        const int nblk = launch_csr_gershgorin_cached(op.csr, h->gs_r, h->gs_diag, ws, st);
-        rc = read_interval(nblk, ws, st, &a, &b);
-      } else {
-        rc = op_interval(op, ws, st, &a, &b);
-      }
-    } else {
-      op.dense = true;
-      const cplx* H0v = (const cplx*)h->H0.values;
-      const cplx* H1v = (const cplx*)h->H1.values;
-      int nblk = 0;
-      if (h->scheme == MAGNUS_M6) {
-        // P:103-114 with A = -iH (reading m6); X1 = h->M, X2 = h->A2, X3 = h->P, X4, X5; see magnus.h at magnus_step
-        const int64_t n = h->n;
-        const double f1 = coef[0], f2 = coef[1], f3 = coef[2];
-        const double b2 = (std::sqrt(15.0) / 3.0) * tau * (f3 - f1), b3 = (10.0 / 3.0) * tau * (f3 - 2.0 * f2 + f1);
-        LinComb lc;
-        auto term = [&](int k, const cplx* x, double re, double im) {
-          lc.x[k] = x;
-          lc.c[k] = make_double2(re, im);
-        };
-        term(0, H0v, 1.0, 0.0); term(1, H1v, f2, 0.0); term(2, nullptr, 0.0, 0.0); term(3, nullptr, 0.0, 0.0);
-        if (dense_ld(&h->H0) != n || dense_ld(&h->H1) != n) { set_error("MAGNUS_M6 needs ld == n"); rc = MAGNUS_EINVAL; break; }
-        launch_dense_lincomb(n, h->M, lc, ws, st);                                   // X1 = H2 = H0 + f2 H1
-        if (h->time_comm) cudaEventRecord(h->ev_comm[0], st);
-        rc = launch_zgemm(n, h->M, n, H1v, n, h->A2, n, st);                          // X2 = P1 = H2 H1
-        if (rc) break;
-        launch_dense_antiherm(n, h->A2, h->P, -1.0, st);                              // X3 = G = P1 - P1^H = [H2, H1]
-        rc = launch_zgemm(n, h->M, n, h->P, n, h->A2, n, st);                         // X2 = P2 = H2 G
-        if (rc) break;
-        launch_dense_antiherm(n, h->A2, h->X4, 1.0, st);                              // X4 = S = P2 + P2^H = [H2, G]
-        term(0, h->M, 0.0, 20.0 * tau); term(1, H1v, 0.0, b3); term(2, h->P, -tau * b2, 0.0); term(3, nullptr, 0.0, 0.0);
-        launch_dense_lincomb(n, h->A2, lc, ws, st);                                  // X2 = L
-        term(0, H1v, 0.0, -b2); term(1, h->P, tau * b3 / 30.0, 0.0); term(2, h->X4, 0.0, -tau * tau * b2 / 60.0);
-        term(3, nullptr, 0.0, 0.0);
-        launch_dense_lincomb(n, h->X5, lc, ws, st);                                  // X5 = R
-        rc = launch_zgemm(n, h->A2, n, h->X5, n, h->X4, n, st);                       // X4 = P3 = L R
-        ws->launches += 5;
-        if (h->time_comm) cudaEventRecord(h->ev_comm[1], st);
-        if (rc) break;
-        // Omega_H = H2 + (b3/(12 tau)) H1 + (i/(240 tau)) (P3 - P3^H), over X1, with its Gershgorin bounds
-        nblk = launch_dense_omega(n, h->M, H1v, h->X4, 1.0, b3 / (12.0 * tau), -1.0 / (240.0 * tau), ws, st);
-      } else if (h->scheme == MAGNUS_M4 && h->cached_p0) {
-        // shortcut: Omega_H = H0 + fbar H1 - i kappa (P0 - P0^H), kappa = (sqrt(3) tau/12)(f1 - f2), no GEMM
-        LinComb lc;
-        lc.x[0] = H0v; lc.c[0] = make_double2(1.0, 0.0);
-        lc.x[1] = H1v; lc.c[1] = make_double2(0.5 * (coef[0] + coef[1]), 0.0);
-        lc.x[2] = lc.x[3] = nullptr; lc.c[2] = lc.c[3] = make_double2(0.0, 0.0);
-        launch_dense_lincomb(h->n, h->M, lc, ws, st);
-        nblk = launch_dense_omega(h->n, h->M, H1v, h->P, 1.0, 0.0, kappa, ws, st);
-      } else if (h->scheme == MAGNUS_M4) {
-        launch_dense_assemble2(h->n, H0v, dense_ld(&h->H0), H1v, dense_ld(&h->H1), coef[0], coef[1], h->M, h->A2, ws,
-                               st);                                                                // S2: A1, A2
-        if (h->time_comm) cudaEventRecord(h->ev_comm[0], st);
-        rc = launch_zgemm(h->n, h->A2, h->n, h->M, h->n, h->P, h->n, st);                          // D3: P = A2 A1
-        ws->launches += 1;
-        if (h->time_comm) cudaEventRecord(h->ev_comm[1], st);
-        if (rc) { set_error("zgemm launch failed: %s", cudaGetErrorString(cudaGetLastError())); break; }
-        nblk = launch_dense_omega(h->n, h->M, h->A2, h->P, 0.5, 0.5, std::sqrt(3.0) * tau / 12.0, ws, st);   // D4 (+S3)
-      } else {
-        nblk = launch_dense_assemble(h->n, H0v, dense_ld(&h->H0), H1v, dense_ld(&h->H1), coef[e], h->M, ws, st);
-      }
-      op.dns.n = h->n;
-      op.dns.ld = h->n;
-      op.dns.M = h->M;
-      rc = read_interval(nblk, ws, st, &a, &b);
-      if (rc == MAGNUS_OK && h->time_comm) {
-        float ms = 0.f;
-        if (cudaEventElapsedTime(&ms, h->ev_comm[0], h->ev_comm[1]) == cudaSuccess) h->comm_ms += ms;
-      }
-    }
-    if (rc) break;
-    rc = expmv_on_interval(op, a, b, psi, psi, hscale[e] * tau, h->prm, ws, st, info ? &info->exp[e] : nullptr);
-  }
-  return rc;
+  return magnus_step_unplanned(h, t, tau, psi, info);
 }
 
 int magnus_integrate(magnus_handle h, double t0, double t_end, int64_t nsteps, void* psi, magnus_stats* stats) {
@@ -734,16 +1013,33 @@ int magnus_integrate(magnus_handle h, double t0, double t_end, int64_t nsteps, v
   CU_TRY(cudaEventRecord(ws->ev[2], st));
   int64_t total = 0, nexp = 0;
   int rc = MAGNUS_OK;
-  for (int64_t s = 0; s < nsteps; ++s) {
-    magnus_step_info si;
-    rc = magnus_step(h, t0 + (double)s * tau, tau, psi, &si);
+  auto account = [&](const magnus_step_info& si, int rc_step) {
     for (int e = 0; e < si.n_exp; ++e) {
-      if (rc != MAGNUS_OK && si.exp[e].iters == 0 && si.exp[e].substeps == 0) break;
+      if (rc_step != MAGNUS_OK && si.exp[e].iters == 0 && si.exp[e].substeps == 0) break;
       if (stats && stats->iters && nexp < stats->iters_cap) stats->iters[nexp] = si.exp[e].iters;
       total += si.exp[e].iters;
       ++nexp;
     }
-    if (rc != MAGNUS_OK) break;
+  };
+  const int batch_steps = kPlanCap / MAGNUS_MAX_EXP_PER_STEP;
+  std::vector<magnus_step_info> infos;
+  for (int64_t s = 0; s < nsteps && rc == MAGNUS_OK;) {
+    if (plan_supported(h)) {
+      const int ns = (int)std::min<int64_t>(batch_steps, nsteps - s);
+      infos.resize((size_t)ns);
+      std::memset(infos.data(), 0, sizeof(magnus_step_info) * (size_t)ns);
+      const int prc = run_planned(h, t0, tau, s, ns, (cplx*)psi, infos.data());
+      if (prc != kPlanDeclined) {
+        rc = prc;
+        for (int i = 0; i < ns; ++i) account(infos[(size_t)i], rc);
+        s += ns;
+        continue;
+      }
+    }
+    magnus_step_info si;
+    rc = magnus_step_unplanned(h, t0 + (double)s * tau, tau, (cplx*)psi, &si);
+    account(si, rc);
+    ++s;
   }
   CU_TRY(cudaEventRecord(ws->ev[3], st));
   CU_TRY(cudaStreamSynchronize(st));

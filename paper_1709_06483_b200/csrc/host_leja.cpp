@@ -77,31 +77,38 @@ const double* leja_points() {
 // every component with full relative accuracy.  long double arithmetic.
 // ---------------------------------------------------------------------------
 void divided_differences(double theta, int m, std::complex<double>* out) {
-  typedef std::complex<long double> lc;
   const double* l = leja_points();
-  std::vector<lc> v(m, lc(0.0L, 0.0L)), term(m), acc(m);
-  v[0] = lc(1.0L, 0.0L);
+  // real and imaginary parts in separate arrays (plain x87 multiplies and adds; no complex-multiply helper calls)
+  std::vector<long double> vr(m, 0.0L), vi(m, 0.0L), tr(m), ti(m), ar(m), ai(m), ll(m);
+  for (int k = 0; k < m; ++k) ll[k] = (long double)l[k];
+  vr[0] = 1.0L;
   const int s = std::max(1, (int)std::ceil(std::fabs(theta) / 0.25));
   const long double tp = (long double)theta / (long double)s;
   const int nterms = m + 24;
+  int top = 0;   // largest index with a nonzero entry in v: Z is lower bidiagonal, so a sweep's j-th term reaches top + j
   for (int sweep = 0; sweep < s; ++sweep) {
-    term = v;
-    acc = v;
+    tr = vr; ti = vi;
+    ar = vr; ai = vi;
     for (int j = 1; j <= nterms; ++j) {
-      // term <- (-i tp / j) Z term, with (Z x)_k = l_k x_k + x_{k-1}
+      // term <- (-i tp / j) Z term, with (Z x)_k = l_k x_k + x_{k-1}; entries above top + j are exactly zero
       const long double f = tp / (long double)j;
-      lc prev(0.0L, 0.0L);
-      for (int k = 0; k < m; ++k) {
-        const lc cur = term[k];
-        const lc z = (long double)l[k] * cur + prev;
-        term[k] = lc(f * z.imag(), -f * z.real());      // (-i f) z
-        prev = cur;
-        acc[k] += term[k];
+      const int kend = std::min(m - 1, top + j);
+      long double pr = 0.0L, pi = 0.0L;
+      for (int k = 0; k <= kend; ++k) {
+        const long double cr = tr[k], ci = ti[k];
+        const long double zr = ll[k] * cr + pr, zi = ll[k] * ci + pi;
+        tr[k] = f * zi;            // (-i f) z
+        ti[k] = -(f * zr);
+        pr = cr;
+        pi = ci;
+        ar[k] += tr[k];
+        ai[k] += ti[k];
       }
     }
-    v = acc;
+    vr = ar; vi = ai;
+    top = m - 1;   // after one sweep v is full
   }
-  for (int k = 0; k < m; ++k) out[k] = std::complex<double>((double)v[k].real(), (double)v[k].imag());
+  for (int k = 0; k < m; ++k) out[k] = std::complex<double>((double)vr[k], (double)vi[k]);
 }
 
 // Reading c4: widen [a,b] outward to the grid of spacing 2^(E-12), E = ceil(log2(b-a)).

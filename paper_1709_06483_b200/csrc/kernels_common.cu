@@ -90,43 +90,63 @@ int workspace_alloc(Workspace* ws, int64_t n) {
   return MAGNUS_OK;
 }
 
-// Buffers of the planned-batch path; allocated once per workspace, on first use.
+// Buffers of the planned-batch path; allocated once per workspace, on first use: ONE device block and ONE pinned
+// block carved into the arrays (a pinned allocation costs about a millisecond, which a small problem notices).
+namespace {
+struct PlanLayout {
+  size_t jobs, status, ab, coef, leja, bar, partials, total_dev, total_host;
+  PlanLayout() {
+    size_t o = 0;
+    auto take = [&](size_t bytes) { const size_t at = o; o += (bytes + 255) / 256 * 256; return at; };
+    jobs = take(sizeof(SweepJob) * kJobCap);
+    status = take(sizeof(LejaStatus) * kPlanCap);
+    ab = take(sizeof(double) * 2 * kPlanCap);
+    coef = take(sizeof(double) * 4 * kPlanCap);
+    total_host = o;                       // the host mirror stops here
+    leja = take(sizeof(double) * (kMaxDegree + 1));
+    bar = take(256);
+    partials = take(sizeof(double) * 4 * kMaxPartials);
+    total_dev = o;
+  }
+};
+}  // namespace
+
 int ensure_sweep_jobs(Workspace* ws) {
   if (ws->jobs) return MAGNUS_OK;
-  bool ok = cudaMalloc(&ws->jobs, sizeof(SweepJob) * kJobCap) == cudaSuccess &&
-            cudaMallocHost(&ws->jobs_host, sizeof(SweepJob) * kJobCap) == cudaSuccess &&
-            cudaMalloc(&ws->status_arr, sizeof(LejaStatus) * kJobCap) == cudaSuccess &&
-            cudaMallocHost(&ws->status_arr_host, sizeof(LejaStatus) * kJobCap) == cudaSuccess &&
-            cudaMalloc(&ws->ab_arr, sizeof(double) * 2 * kJobCap) == cudaSuccess &&
-            cudaMallocHost(&ws->ab_arr_host, sizeof(double) * 2 * kJobCap) == cudaSuccess &&
-            cudaMalloc(&ws->coef_arr, sizeof(double) * 4 * kJobCap) == cudaSuccess &&
-            cudaMallocHost(&ws->coef_arr_host, sizeof(double) * 4 * kJobCap) == cudaSuccess &&
-            cudaMalloc(&ws->leja_l, sizeof(double) * (kMaxDegree + 1)) == cudaSuccess &&
-            cudaMalloc(&ws->grid_bar, 64) == cudaSuccess &&
-            cudaMalloc(&ws->sweep_partials, sizeof(double) * 4 * kMaxPartials) == cudaSuccess;
+  const PlanLayout L;
+  char* dev = nullptr;
+  char* host = nullptr;
+  bool ok = cudaMalloc(&dev, L.total_dev) == cudaSuccess && cudaMallocHost(&host, L.total_host) == cudaSuccess;
+  for (int i = 0; ok && i < 2 * kJobRing; ++i) ok = cudaEventCreate(&ws->ring_ev[i]) == cudaSuccess;
   if (ok)
-    ok = cudaMemcpy(ws->leja_l, leja_points(), sizeof(double) * (kMaxDegree + 1), cudaMemcpyHostToDevice) == cudaSuccess &&
-         cudaMemset(ws->grid_bar, 0, 64) == cudaSuccess;
+    ok = cudaMemset(dev + L.bar, 0, 256) == cudaSuccess &&
+         cudaMemcpy(dev + L.leja, leja_points(), sizeof(double) * (kMaxDegree + 1), cudaMemcpyHostToDevice) == cudaSuccess;
   if (!ok) {
     cudaGetLastError();
+    cudaFree(dev);
+    if (host) cudaFreeHost(host);
     return MAGNUS_ENOMEM;
   }
+  ws->jobs = reinterpret_cast<SweepJob*>(dev + L.jobs);
+  ws->status_arr = reinterpret_cast<LejaStatus*>(dev + L.status);
+  ws->ab_arr = reinterpret_cast<double*>(dev + L.ab);
+  ws->coef_arr = reinterpret_cast<double*>(dev + L.coef);
+  ws->leja_l = reinterpret_cast<double*>(dev + L.leja);
+  ws->grid_bar = reinterpret_cast<unsigned*>(dev + L.bar);
+  ws->sweep_partials = reinterpret_cast<double*>(dev + L.partials);
+  ws->jobs_host = reinterpret_cast<SweepJob*>(host + L.jobs);
+  ws->status_arr_host = reinterpret_cast<LejaStatus*>(host + L.status);
+  ws->ab_arr_host = reinterpret_cast<double*>(host + L.ab);
+  ws->coef_arr_host = reinterpret_cast<double*>(host + L.coef);
   return MAGNUS_OK;
 }
 
 void workspace_free(Workspace* ws) {
   stream_maps_free(ws);
-  cudaFree(ws->jobs);
-  cudaFree(ws->status_arr);
-  cudaFree(ws->ab_arr);
-  cudaFree(ws->coef_arr);
-  cudaFree(ws->leja_l);
-  cudaFree(ws->grid_bar);
-  cudaFree(ws->sweep_partials);
-  if (ws->jobs_host) cudaFreeHost(ws->jobs_host);
-  if (ws->status_arr_host) cudaFreeHost(ws->status_arr_host);
-  if (ws->ab_arr_host) cudaFreeHost(ws->ab_arr_host);
-  if (ws->coef_arr_host) cudaFreeHost(ws->coef_arr_host);
+  cudaFree(ws->jobs);                                   // the one device block of ensure_sweep_jobs starts here
+  for (int i = 0; i < 2 * kJobRing; ++i)
+    if (ws->ring_ev[i]) cudaEventDestroy(ws->ring_ev[i]);
+  if (ws->jobs_host) cudaFreeHost(ws->jobs_host);       // ... and the one pinned block here
   cudaFree(ws->w[0]);
   cudaFree(ws->w[1]);
   cudaFree(ws->p);

@@ -17,7 +17,7 @@ namespace magnus {
 // merge over the (ascending) column lists, so overlapping patterns are summed
 // before the modulus is taken.  Block min/max go to ws->gersh.
 // ---------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) csr_gershgorin_kernel(CsrOp op, double* out, unsigned* ticket) {
+__global__ void __launch_bounds__(256) csr_gershgorin_kernel(CsrOp op, double* out, unsigned* ticket, double* fin) {
   double lo = INFINITY, hi = -INFINITY;
   for (int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; row < op.n;
        row += (int64_t)gridDim.x * blockDim.x) {
@@ -53,7 +53,7 @@ __global__ void __launch_bounds__(256) csr_gershgorin_kernel(CsrOp op, double* o
     out[2 * blockIdx.x] = lo;
     out[2 * blockIdx.x + 1] = hi;
   }
-  if (last_block_ticket(ticket)) minmax_finalize_warp0(out, gridDim.x, out + 2 * kMaxPartials);
+  if (last_block_ticket(ticket)) minmax_finalize_warp0(out, gridDim.x, fin);
 }
 
 // The same bounds for large n with every access coalesced: a warp owns 32 consecutive rows,
@@ -68,7 +68,8 @@ const int GS_SLOTS = GS_CAP + GS_CAP / 8;
 const int GS_BYTES_PER_WARP = GS_SLOTS * (int)(sizeof(cplx) + sizeof(int32_t));
 const int GS_SMEM = GS_WARPS * GS_BYTES_PER_WARP;
 
-__global__ void __launch_bounds__(GS_WARPS * 32, 1) csr_gershgorin_staged_kernel(CsrOp op, double* out, unsigned* ticket) {
+__global__ void __launch_bounds__(GS_WARPS * 32, 1) csr_gershgorin_staged_kernel(CsrOp op, double* out, unsigned* ticket,
+                                                                                 double* fin) {
   extern __shared__ __align__(16) unsigned char gs_smem[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   cplx* sv = reinterpret_cast<cplx*>(gs_smem + (size_t)warp * GS_BYTES_PER_WARP);
@@ -152,7 +153,7 @@ __global__ void __launch_bounds__(GS_WARPS * 32, 1) csr_gershgorin_staged_kernel
     out[2 * blockIdx.x] = lo;
     out[2 * blockIdx.x + 1] = hi;
   }
-  if (last_block_ticket(ticket)) minmax_finalize_warp0(out, gridDim.x, out + 2 * kMaxPartials);
+  if (last_block_ticket(ticket)) minmax_finalize_warp0(out, gridDim.x, fin);
 }
 
 int launch_csr_gershgorin(const CsrOp& op, Workspace* ws, cudaStream_t st) {
@@ -160,13 +161,13 @@ int launch_csr_gershgorin(const CsrOp& op, Workspace* ws, cudaStream_t st) {
     // per launch (cheap): the attribute is per device, a process-wide flag would miss a second GPU
     cudaFuncSetAttribute(csr_gershgorin_staged_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GS_SMEM);
     const int sms = device_sm_count();
-    csr_gershgorin_staged_kernel<<<sms, GS_WARPS * 32, GS_SMEM, st>>>(op, ws->gersh, ws->tickets + 1);
+    csr_gershgorin_staged_kernel<<<sms, GS_WARPS * 32, GS_SMEM, st>>>(op, ws->gersh, ws->tickets + 1, gersh_final(ws));
     ws->launches += 1;
     return sms;
   }
   int64_t g = (op.n + 255) / 256;
   if (g > (int64_t)device_sm_count() * 8) g = (int64_t)device_sm_count() * 8;
-  csr_gershgorin_kernel<<<(int)g, 256, 0, st>>>(op, ws->gersh, ws->tickets + 1);
+  csr_gershgorin_kernel<<<(int)g, 256, 0, st>>>(op, ws->gersh, ws->tickets + 1, gersh_final(ws));
   ws->launches += 1;
   return (int)g;
 }
@@ -232,7 +233,7 @@ struct RowStats {
 };
 
 __global__ void __launch_bounds__(256) csr_gershgorin_cached_kernel(RowStats S, int64_t n, double* out,
-                                                                     unsigned* ticket) {
+                                                                     unsigned* ticket, double* fin) {
   double lo = INFINITY, hi = -INFINITY;
   double ac[3];
 #pragma unroll
@@ -254,7 +255,7 @@ __global__ void __launch_bounds__(256) csr_gershgorin_cached_kernel(RowStats S, 
     out[2 * blockIdx.x] = lo;
     out[2 * blockIdx.x + 1] = hi;
   }
-  if (last_block_ticket(ticket)) minmax_finalize_warp0(out, gridDim.x, out + 2 * kMaxPartials);
+  if (last_block_ticket(ticket)) minmax_finalize_warp0(out, gridDim.x, fin);
 }
 
 static int row_grid256(int64_t n) {
@@ -281,9 +282,55 @@ int launch_csr_gershgorin_cached(const CsrOp& op, const double* const* r, const 
     S.coef[t] = op.t[t < op.nterms ? t : 0].coef;
   }
   const int g = row_grid256(op.n);
-  csr_gershgorin_cached_kernel<<<g, 256, 0, st>>>(S, op.n, ws->gersh, ws->tickets + 1);
+  csr_gershgorin_cached_kernel<<<g, 256, 0, st>>>(S, op.n, ws->gersh, ws->tickets + 1, gersh_final(ws));
   ws->launches += 1;
   return g;
+}
+
+// The same bounds for a whole planned batch in ONE launch: block e takes exponential e, whose term
+// coefficients are (1, g_e, -i kappa_e) = coefs[4e], coefs[4e+1], nterms = (int)coefs[4e+2].  Small n only
+// (a block walks all rows); the arithmetic per row is that of csr_gershgorin_cached_kernel.
+__global__ void __launch_bounds__(256) csr_gershgorin_cached_batch_kernel(RowStats S, int64_t n,
+                                                                           const double* __restrict__ coefs,
+                                                                           double* __restrict__ ab_out) {
+  const int e = blockIdx.x;
+  const double g = coefs[4 * e], kappa = coefs[4 * e + 1];
+  const int nterms = (int)coefs[4 * e + 2];
+  cplx coef[3] = {make_double2(1.0, 0.0), make_double2(g, 0.0), make_double2(0.0, -kappa)};
+  double ac[3];
+#pragma unroll
+  for (int t = 0; t < 3; ++t) ac[t] = t < nterms ? cabs_fast(coef[t]) : 0.0;
+  double lo = INFINITY, hi = -INFINITY;
+  for (int64_t row = threadIdx.x; row < n; row += blockDim.x) {
+    double R = 0.0, d = 0.0;
+#pragma unroll
+    for (int t = 0; t < 3; ++t)
+      if (t < nterms) {
+        const cplx dg = S.diag[t][row];
+        R = fma(ac[t], S.r[t][row], R);
+        d += coef[t].x * dg.x - coef[t].y * dg.y;
+      }
+    lo = fmin(lo, d - R);
+    hi = fmax(hi, d + R);
+  }
+  block_reduce_minmax<256>(lo, hi);
+  if (threadIdx.x == 0) {
+    ab_out[2 * e] = lo;
+    ab_out[2 * e + 1] = hi;
+  }
+}
+
+void launch_csr_gershgorin_cached_batch(int64_t n, const double* const* r, const cplx* const* diag, int nterms_max,
+                                        const double* coefs_dev, int E, double* ab_out, Workspace* ws, cudaStream_t st) {
+  RowStats S;
+  S.nterms = nterms_max;
+  for (int t = 0; t < 3; ++t) {
+    S.r[t] = r[t < nterms_max ? t : 0];
+    S.diag[t] = diag[t < nterms_max ? t : 0];
+    S.coef[t] = make_double2(0.0, 0.0);
+  }
+  csr_gershgorin_cached_batch_kernel<<<E, 256, 0, st>>>(S, n, coefs_dev, ab_out);
+  ws->launches += 1;
 }
 
 // ---------------------------------------------------------------------------

@@ -69,7 +69,8 @@ __device__ __forceinline__ void block_reduce_sum2_ss(double& a, double& b, doubl
 // first job that does not meet tol within its m_max (status[e].pad = 1).
 __global__ void __cluster_dims__(SS_CTAS, 1, 1) __launch_bounds__(SS_THREADS, 1)
     csr_leja_sweep_small_kernel(CsrOp op, const cplx* v, cplx* out, const SweepJob* __restrict__ jobs, int njobs,
-                                const double* __restrict__ leja_l, double tol, LejaStatus* status) {
+                                const double* __restrict__ leja_l, double tol, LejaStatus* status,
+                                const LejaStatus* gate) {
   extern __shared__ __align__(16) unsigned char ss_smem[];
   __shared__ double sa[SS_THREADS / 32], sb[SS_THREADS / 32];
   __shared__ double part[2][2];                     // [iteration parity](sw, sp) of this CTA, read by the others
@@ -77,6 +78,7 @@ __global__ void __cluster_dims__(SS_CTAS, 1, 1) __launch_bounds__(SS_THREADS, 1)
   cg::cluster_group cluster = cg::this_cluster();
   const int rank = (int)cluster.block_rank();
   if (status->pad) return;                          // an earlier sub-step did not converge (cluster-uniform)
+  if (gate && !gate->done) return;                  // an earlier job of the plan failed: psi stays as that job found it
   cplx* wbuf[2] = {reinterpret_cast<cplx*>(ss_smem), reinterpret_cast<cplx*>(ss_smem) + kSmallSweepMaxN};
   const int tid = threadIdx.x, grp = tid / SS_G, sub = tid % SS_G;
   const int n = (int)op.n;
@@ -254,12 +256,14 @@ __global__ void __cluster_dims__(SS_CTAS, 1, 1) __launch_bounds__(SS_THREADS, 1)
 }  // namespace
 
 int launch_csr_leja_sweep_small_jobs(const CsrOp& op, cplx* psi, const SweepJob* jobs, int njobs, const double* leja_l,
-                                     double tol, LejaStatus* status, Workspace* ws, cudaStream_t st) {
+                                     double tol, LejaStatus* status, const LejaStatus* gate, Workspace* ws,
+                                     cudaStream_t st) {
   // per launch (cheap): the attribute is per device, a process-wide flag would miss a second GPU
   if (cudaFuncSetAttribute(csr_leja_sweep_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SS_SMEM) !=
       cudaSuccess)
     return MAGNUS_ECUDA;
-  csr_leja_sweep_small_kernel<<<SS_CTAS, SS_THREADS, SS_SMEM, st>>>(op, psi, psi, jobs, njobs, leja_l, tol, status);
+  csr_leja_sweep_small_kernel<<<SS_CTAS, SS_THREADS, SS_SMEM, st>>>(op, psi, psi, jobs, njobs, leja_l, tol, status,
+                                                                    gate);
   ws->launches += 1;
   return cudaGetLastError() == cudaSuccess ? MAGNUS_OK : MAGNUS_ECUDA;
 }
@@ -284,7 +288,7 @@ int launch_csr_leja_sweep_small(const CsrOp& op, const cplx* v, cplx* out, doubl
       cudaSuccess)
     return MAGNUS_ECUDA;
   csr_leja_sweep_small_kernel<<<SS_CTAS, SS_THREADS, SS_SMEM, st>>>(op, v, out, ws->jobs, 1, ws->leja_l, tol,
-                                                                    ws->status);
+                                                                    ws->status, nullptr);
   ws->launches += 1;
   return cudaGetLastError() == cudaSuccess ? MAGNUS_OK : MAGNUS_ECUDA;
 }

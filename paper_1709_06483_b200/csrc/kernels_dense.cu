@@ -2,6 +2,8 @@
 // S2+S3), the Omega_H assembly of M4 (row D4), and the fused dense Leja
 // iteration (row S6).  Row-major complex128.
 // P:n = PAPER.md line n; c1..c7 = readings in DESIGN.md section 3.
+#include <cstring>
+
 #include "magnus_internal.h"
 #include "device_utils.cuh"
 #include "leja_finalize.cuh"
@@ -21,7 +23,8 @@ constexpr int DW = 8;   // warps per block; one row per warp
 template <bool HAS_B, bool WRITE>
 __global__ void __launch_bounds__(DW * 32) dense_assemble_kernel(int64_t n, const cplx* __restrict__ A, int64_t lda,
                                                                   const cplx* __restrict__ B, int64_t ldb, double g,
-                                                                  cplx* __restrict__ M, double* out, unsigned* ticket) {
+                                                                  cplx* __restrict__ M, double* out, unsigned* ticket,
+                                                                  double* fin) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   double lo = INFINITY, hi = -INFINITY;
   for (int64_t row = (int64_t)blockIdx.x * DW + warp; row < n; row += (int64_t)gridDim.x * DW) {
@@ -53,7 +56,7 @@ __global__ void __launch_bounds__(DW * 32) dense_assemble_kernel(int64_t n, cons
     out[2 * blockIdx.x] = lo;
     out[2 * blockIdx.x + 1] = hi;
   }
-  if (last_block_ticket(ticket)) minmax_finalize_warp0(out, gridDim.x, out + 2 * kMaxPartials);
+  if (last_block_ticket(ticket)) minmax_finalize_warp0(out, gridDim.x, fin);
 }
 
 // A1 = H0 + f1 H1, A2 = H0 + f2 H1 (P:262 l.3-4), one pass over H0 and H1.
@@ -80,7 +83,8 @@ __global__ void __launch_bounds__(256) dense_assemble2_kernel(int64_t n, const c
 // A1 = H(t2), A2 = H1 and P = L R, see magnus_step.
 __global__ void __launch_bounds__(256) dense_omega_kernel(int64_t n, cplx* __restrict__ A1, const cplx* __restrict__ A2,
                                                            const cplx* __restrict__ P, double wa, double wb,
-                                                           double kappa, double* out, unsigned* ticket) {
+                                                           double kappa, double* out, unsigned* ticket,
+                                                           double* fin) {
   __shared__ cplx tile[32][33];
   const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
   double lo = INFINITY, hi = -INFINITY;
@@ -131,7 +135,7 @@ __global__ void __launch_bounds__(256) dense_omega_kernel(int64_t n, cplx* __res
     out[2 * blockIdx.x] = lo;
     out[2 * blockIdx.x + 1] = hi;
   }
-  if (last_block_ticket(ticket)) minmax_finalize_warp0(out, gridDim.x, out + 2 * kMaxPartials);
+  if (last_block_ticket(ticket)) minmax_finalize_warp0(out, gridDim.x, fin);
 }
 
 // K = P + s P^H, s = -1 (K = P - P^H: the commutator of two Hermitian or two anti-Hermitian factors of P) or
@@ -254,6 +258,80 @@ __global__ void dense_hermitian_check_kernel(DenseOp op, int64_t samples, double
   if (threadIdx.x == 0) worst[blockIdx.x] = -neg;
 }
 
+// ---------------------------------------------------------------------------
+// S3 for a planned batch: the Gershgorin bounds of M_e = H0 + g_e H1 for E exponentials from ONE pass over
+// H0 and H1 (the bounds do not depend on psi, so a run of steps can be planned ahead).  A CTA takes a row,
+// every thread keeps its entries of the row (n <= 256 * DGB_EPT) in registers and walks the g_e in chunks
+// of DGB_CH; a chunk's row sums are reduced over the block and folded into keys[e] (min) / keys[E + e] (max)
+// with integer atomics on an order-preserving encoding of the double -- min and max do not depend on the
+// order, so the result is deterministic.  |z| = sqrt(re^2 + im^2) (cabs_fast); the last-ulp difference to
+// hypot is absorbed by the interval snapping (reading c4).
+// ---------------------------------------------------------------------------
+constexpr int DGB_EPT = 16, DGB_CH = 8;
+
+__device__ __forceinline__ unsigned long long ordered_key(double x) {
+  const unsigned long long u = (unsigned long long)__double_as_longlong(x);
+  return (u >> 63) ? ~u : (u | 0x8000000000000000ull);
+}
+
+__global__ void __launch_bounds__(256) dense_gershgorin_batch_kernel(int n, const cplx* __restrict__ H0, int64_t ld0,
+                                                                      const cplx* __restrict__ H1, int64_t ld1,
+                                                                      const double* __restrict__ coefs, int E,
+                                                                      unsigned long long* keys) {
+  __shared__ double s_part[8][DGB_CH];
+  __shared__ double s_diag[2];
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  for (int row = blockIdx.x; row < n; row += gridDim.x) {
+    cplx a[DGB_EPT], b[DGB_EPT];
+    const cplx* pa = H0 + (int64_t)row * ld0;
+    const cplx* pb = H1 + (int64_t)row * ld1;
+#pragma unroll
+    for (int i = 0; i < DGB_EPT; ++i) {
+      const int j = tid + 256 * i;
+      a[i] = j < n ? ld_gather_na(pa + j) : make_double2(0.0, 0.0);
+      b[i] = j < n ? ld_gather_na(pb + j) : make_double2(0.0, 0.0);
+      if (j == row) {                      // the diagonal enters the centre, not the radius
+        s_diag[0] = a[i].x;
+        s_diag[1] = b[i].x;
+        a[i] = make_double2(0.0, 0.0);
+        b[i] = make_double2(0.0, 0.0);
+      }
+    }
+    __syncthreads();
+    const double da = s_diag[0], db = s_diag[1];
+    for (int e0 = 0; e0 < E; e0 += DGB_CH) {
+      double R[DGB_CH];
+#pragma unroll
+      for (int c = 0; c < DGB_CH; ++c) {
+        const double g = coefs[4 * min(e0 + c, E - 1)];
+        double r = 0.0;
+#pragma unroll
+        for (int i = 0; i < DGB_EPT; ++i) {
+          const double zx = fma(g, b[i].x, a[i].x), zy = fma(g, b[i].y, a[i].y);
+          r += sqrt(fma(zx, zx, zy * zy));
+        }
+        R[c] = r;
+      }
+#pragma unroll
+      for (int c = 0; c < DGB_CH; ++c) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) R[c] += shfl_xor_d(R[c], o);
+        if (lane == 0) s_part[warp][c] = R[c];
+      }
+      __syncthreads();
+      if (tid < DGB_CH && e0 + tid < E) {
+        double r = 0.0;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) r += s_part[w][tid];
+        const double d = fma(coefs[4 * (e0 + tid)], db, da);
+        atomicMin(keys + e0 + tid, ordered_key(d - r));
+        atomicMax(keys + E + e0 + tid, ordered_key(d + r));
+      }
+      __syncthreads();
+    }
+  }
+}
+
 int row_grid(int64_t n) {
   int64_t g = (n + DW - 1) / DW;
   if (g > kMaxPartials) g = kMaxPartials;
@@ -265,15 +343,47 @@ int row_grid(int64_t n) {
 int launch_dense_gershgorin(const DenseOp& op, Workspace* ws, cudaStream_t st) {
   const int g = row_grid(op.n);
   dense_assemble_kernel<false, false><<<g, DW * 32, 0, st>>>(op.n, op.M, op.ld, nullptr, 0, 0.0, nullptr, ws->gersh,
-                                                             ws->tickets + 1);
+                                                             ws->tickets + 1, gersh_final(ws));
   ws->launches += 1;
   return g;
+}
+
+// keys (device, 2 E entries) come back as ordered keys: dense_gershgorin_batch_decode turns a host copy into doubles
+int launch_dense_gershgorin_batch(int64_t n, const cplx* H0, int64_t ld0, const cplx* H1, int64_t ld1,
+                                  const double* coefs_dev, int E, double* ab_keys_dev, Workspace* ws, cudaStream_t st) {
+  if (n > 256 * DGB_EPT) return MAGNUS_EINVAL;
+  unsigned long long* keys = reinterpret_cast<unsigned long long*>(ab_keys_dev);
+  if (cudaMemsetAsync(keys, 0xFF, sizeof(unsigned long long) * (size_t)E, st) != cudaSuccess ||
+      cudaMemsetAsync(keys + E, 0, sizeof(unsigned long long) * (size_t)E, st) != cudaSuccess)
+    return MAGNUS_ECUDA;
+  int64_t g = n;
+  if (g > (int64_t)device_sm_count() * 8) g = (int64_t)device_sm_count() * 8;
+  dense_gershgorin_batch_kernel<<<(int)g, 256, 0, st>>>((int)n, H0, ld0, H1, ld1, coefs_dev, E, keys);
+  ws->launches += 1;
+  return MAGNUS_OK;
+}
+
+// host: keys[e] (min), keys[E + e] (max) -> ab[2e], ab[2e + 1]
+void dense_gershgorin_batch_decode(const double* keys_host, int E, double* ab) {
+  auto dec = [](double kd) {
+    unsigned long long k;
+    memcpy(&k, &kd, sizeof k);
+    const unsigned long long u = (k >> 63) ? (k & 0x7FFFFFFFFFFFFFFFull) : ~k;
+    double x;
+    memcpy(&x, &u, sizeof x);
+    return x;
+  };
+  for (int e = 0; e < E; ++e) {
+    ab[2 * e] = dec(keys_host[e]);
+    ab[2 * e + 1] = dec(keys_host[E + e]);
+  }
 }
 
 int launch_dense_assemble(int64_t n, const cplx* A, int64_t lda, const cplx* B, int64_t ldb, double g, cplx* M,
                           Workspace* ws, cudaStream_t st) {
   const int grid = row_grid(n);
-  dense_assemble_kernel<true, true><<<grid, DW * 32, 0, st>>>(n, A, lda, B, ldb, g, M, ws->gersh, ws->tickets + 1);
+  dense_assemble_kernel<true, true><<<grid, DW * 32, 0, st>>>(n, A, lda, B, ldb, g, M, ws->gersh, ws->tickets + 1,
+                                                              gersh_final(ws));
   ws->launches += 1;
   return grid;
 }
@@ -290,7 +400,7 @@ int launch_dense_omega(int64_t n, cplx* A1, const cplx* A2, const cplx* P, doubl
                        Workspace* ws, cudaStream_t st) {
   int64_t g = (n + 31) / 32;
   if (g > kMaxPartials) g = kMaxPartials;
-  dense_omega_kernel<<<(int)g, 256, 0, st>>>(n, A1, A2, P, wa, wb, kappa, ws->gersh, ws->tickets + 1);
+  dense_omega_kernel<<<(int)g, 256, 0, st>>>(n, A1, A2, P, wa, wb, kappa, ws->gersh, ws->tickets + 1, gersh_final(ws));
   ws->launches += 1;
   return (int)g;
 }

@@ -81,6 +81,7 @@ struct LejaStatus {
 
 // Small CSR problems run a whole Leja sweep in one launch of an 8-CTA cluster (kernels_csr_small.cu).
 const int kSmallSweepMaxN = 4096;
+const int kDenseSweepMaxN = 4096;   // dense problems up to this n run whole sweeps in one cooperative launch
 struct SweepTable {
   cplx d[kMaxDegree + 1];     // divided differences d_k (c3)
   double l[kMaxDegree + 1];   // Leja points l_k (c2)
@@ -102,6 +103,10 @@ struct SweepJob {
 const int kSweepJobAssembled = 1;
 
 const int kMaxPartials = 4096;   // upper bound on blocks that write partial sums
+const int kJobCap = 256;             // job slots on the device (a ring of kJobRing launches of kJobsPerLaunch jobs)
+const int kJobsPerLaunch = 16;
+const int kJobRing = kJobCap / kJobsPerLaunch;
+const int kPlanCap = 4096;           // exponentials planned ahead at once (intervals, stop-test records)
 
 struct Workspace {
   int64_t n = 0;
@@ -122,17 +127,20 @@ struct Workspace {
   // planned batches (whole-sweep kernels), allocated on first use by ensure_sweep_jobs
   SweepJob* jobs = nullptr;          // device [kJobCap]
   SweepJob* jobs_host = nullptr;     // pinned [kJobCap]
-  LejaStatus* status_arr = nullptr;  // device [kJobCap]
-  LejaStatus* status_arr_host = nullptr;   // pinned [kJobCap]
-  double* ab_arr = nullptr;          // device [2 kJobCap]: Gershgorin bounds of the batch's exponentials
-  double* ab_arr_host = nullptr;     // pinned [2 kJobCap]
-  double* coef_arr = nullptr;        // device [4 kJobCap]: per-exponential scalars of the batched Gershgorin kernels
+  LejaStatus* status_arr = nullptr;  // device [kPlanCap]
+  LejaStatus* status_arr_host = nullptr;   // pinned [kPlanCap]
+  double* ab_out = nullptr;          // set by the planner while it enqueues the interval kernels of a batch
+  double* ab_arr = nullptr;          // device [2 kPlanCap]: Gershgorin bounds of the batch's exponentials
+  double* ab_arr_host = nullptr;     // pinned [2 kPlanCap]
+  double* coef_arr = nullptr;        // device [4 kPlanCap]: per-exponential scalars of the batched Gershgorin kernels
   double* coef_arr_host = nullptr;   // pinned
+  cudaEvent_t ring_ev[2 * kJobRing] = {};   // start / end of the launch that last used a ring slot
   double* leja_l = nullptr;          // device [kMaxDegree + 1]: Leja points (c2)
   unsigned* grid_bar = nullptr;      // device: grid-barrier counter of the dense sweep kernel
   double* sweep_partials = nullptr;  // device [2][2 * kMaxPartials]: per-CTA partial norms of the dense sweep kernel
 };
-const int kJobCap = 256;             // exponentials per planned batch
+// where the Gershgorin kernels put their final (min, max): the slot the planner set, else the workspace's own
+inline double* gersh_final(const Workspace* ws) { return ws->ab_out ? ws->ab_out : ws->gersh + 2 * kMaxPartials; }
 int ensure_sweep_jobs(Workspace* ws);
 
 // cudaDevAttrMultiProcessorCount of the current device (cached per device; 148 on B200)
@@ -162,6 +170,9 @@ void launch_csr_rowstats(const CsrTerm& T, int64_t n, double* r, cplx* diag, cud
 void launch_csr_overlap(const CsrOp& op, int* flag, cudaStream_t st);
 int launch_csr_gershgorin_cached(const CsrOp& op, const double* const* r, const cplx* const* diag, Workspace* ws,
                                  cudaStream_t st);
+// the bounds of E exponentials (coefficients 1, g_e, -i kappa_e; coefs_dev[4e..4e+2] = g, kappa, terms) in one launch
+void launch_csr_gershgorin_cached_batch(int64_t n, const double* const* r, const cplx* const* diag, int nterms_max,
+                                        const double* coefs_dev, int E, double* ab_out, Workspace* ws, cudaStream_t st);
 int launch_csr_leja_iter(const CsrOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma, double shift,
                          cplx dk, double abs_dk, double tol, Workspace* ws, cudaStream_t st);
 int csr_commutator(const magnus_matrix* A, const magnus_matrix* B, int64_t cap, int64_t* nnz_out, int32_t* rp_out,
@@ -205,8 +216,10 @@ int launch_csr_leja_sweep_small(const CsrOp& op, const cplx* v, cplx* out, doubl
                                  cudaStream_t st);
 // a planned batch in ONE launch: psi <- exp(job[njobs-1]) ... exp(job[0]) psi; status[e] per job (zeroed by the
 // caller); stops at the first job that does not converge within its m_max (status[e].pad = 1, psi = state before it)
+// gate (nullable): the stop-test record of the job before jobs[0]; the launch does nothing unless that job converged
 int launch_csr_leja_sweep_small_jobs(const CsrOp& op, cplx* psi, const SweepJob* jobs, int njobs, const double* leja_l,
-                                      double tol, LejaStatus* status, Workspace* ws, cudaStream_t st);
+                                      double tol, LejaStatus* status, const LejaStatus* gate, Workspace* ws,
+                                      cudaStream_t st);
 
 // ---- kernels_dense.cu -------------------------------------------------------
 int launch_dense_gershgorin(const DenseOp& op, Workspace* ws, cudaStream_t st);
@@ -227,6 +240,14 @@ struct LinComb {
 };
 void launch_dense_lincomb(int64_t n, cplx* out, LinComb lc, Workspace* ws, cudaStream_t st);
 void launch_csr_to_dense(int64_t n, const int32_t* rp, const int32_t* ci, const cplx* v, cplx* A, cudaStream_t st);
+// planned batches on medium dense problems (kernels_dense_sweep.cu, dense_gershgorin_batch_kernel)
+int launch_dense_gershgorin_batch(int64_t n, const cplx* H0, int64_t ld0, const cplx* H1, int64_t ld1,
+                                  const double* coefs_dev, int E, double* ab_keys_dev, Workspace* ws, cudaStream_t st);
+void dense_gershgorin_batch_decode(const double* keys_host, int E, double* ab);
+bool dense_sweep_supported(int64_t n);
+int launch_dense_leja_sweep_jobs(int64_t n, const cplx* H0, int64_t ld0, const cplx* H1, int64_t ld1, cplx* M, cplx* psi,
+                                 const SweepJob* jobs, int njobs, double tol, LejaStatus* status, const LejaStatus* gate,
+                                 Workspace* ws, cudaStream_t st);
 int launch_dense_leja_iter(const DenseOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma, double shift,
                            cplx dk, double abs_dk, double tol, Workspace* ws, cudaStream_t st);
 int dense_hermitian_check(const DenseOp& op, cudaStream_t st, double* max_violation);
