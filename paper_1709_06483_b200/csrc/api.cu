@@ -177,9 +177,12 @@ static int expmv_on_interval(const OpRef& op, double a_raw, double b_raw, const 
   const double inv_gamma = 1.0 / gamma, c_over_gamma = c / gamma;
   const cplx phase = make_double2(std::cos(hs * c), -std::sin(hs * c));
   float ms = 0.f;
-  if (!op.dense && n <= kSmallSweepMaxN && ws->csr_kernel == 0) {
-    // small CSR problem: each sub-step sweep is ONE launch (kernels_csr_small.cu); the table first
-    // covers `have` terms and is extended to m_max only if the sweep asks for more
+  const bool small_csr = !op.dense && n <= kSmallSweepMaxN && ws->csr_kernel == 0;
+  const bool mid_dense = op.dense && dense_sweep_supported(n) && op.dns.ld == n && ws->csr_kernel == 0;
+  if (small_csr || mid_dense) {
+    // small CSR / medium dense problem: each sub-step sweep is ONE launch (kernels_csr_small.cu,
+    // kernels_dense_sweep.cu) on an already assembled operator; the table first covers `have` terms and is
+    // extended only if the sweep asks for more
     SweepTable tab;
     for (int sub = 0; sub < s; ++sub) {
       const cplx* src = sub == 0 ? v_in : v_out;
@@ -192,8 +195,12 @@ static int expmv_on_interval(const OpRef& op, double a_raw, double b_raw, const 
         }
         CU_TRY(cudaMemsetAsync(ws->status, 0, sizeof(LejaStatus), st));
         if (ws->time_leja) CU_TRY(cudaEventRecord(ws->ev[0], st));
-        if (launch_csr_leja_sweep_small(op.csr, src, v_out, inv_gamma, c_over_gamma, prm.tol, m_try, phase, tab, ws, st)) {
-          set_error("small-sweep cluster launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+        const int lrc = small_csr ? launch_csr_leja_sweep_small(op.csr, src, v_out, inv_gamma, c_over_gamma, prm.tol, m_try,
+                                                                phase, tab, ws, st)
+                                  : launch_dense_leja_sweep(op.dns, src, v_out, inv_gamma, c_over_gamma, prm.tol, m_try,
+                                                            phase, tab, ws, st);
+        if (lrc) {
+          set_error("whole-sweep launch failed: %s", cudaGetErrorString(cudaGetLastError()));
           return MAGNUS_ECUDA;
         }
         if (ws->time_leja) CU_TRY(cudaEventRecord(ws->ev[1], st));

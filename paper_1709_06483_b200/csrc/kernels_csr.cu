@@ -488,16 +488,250 @@ __device__ __forceinline__ void comm_expand(const CsrRaw& A, const CsrRaw& B, in
   }
 }
 
+// Bitonic sorting network over 32 R keys held R per lane (element e = lane R + r), ascending.  Strides below R
+// are compare-exchanges between registers of a lane, the others exchange with lane ^ (stride / R) by shuffle;
+// everything is unrolled at compile time, so the network touches no memory.
+template <int R, typename T>
+__device__ __forceinline__ void warp_bitonic_sort(T (&k)[R], int lane) {
+#pragma unroll
+  for (int size = 2; size <= 32 * R; size <<= 1) {
+#pragma unroll
+    for (int stride = size >> 1; stride > 0; stride >>= 1) {
+      if (stride < R) {
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+          if (r & stride) continue;
+          const bool asc = size < R ? (r & size) == 0 : (lane & (size / R)) == 0;   // size == 32 R: always ascending
+          const T a = k[r], b = k[r | stride];
+          const T lo = a < b ? a : b, hi = a < b ? b : a;
+          k[r] = asc ? lo : hi;
+          k[r | stride] = asc ? hi : lo;
+        }
+      } else {
+        const int lm = stride / R;
+        const bool lower = (lane & lm) == 0;
+        const bool asc = (lane & (size / R)) == 0;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+          const T o = __shfl_xor_sync(0xffffffffu, k[r], lm);
+          const bool take_min = lower == asc;
+          k[r] = take_min ? (o < k[r] ? o : k[r]) : (o > k[r] ? o : k[r]);
+        }
+      }
+    }
+  }
+}
+
+// keys[0..total) of a warp: (column << 32 | position) -> the same, sorted; T = unsigned packs the key as
+// column * 1024 + position for the network and unpacks it again
+template <int R, typename T, bool DUMMY>
+__device__ __forceinline__ void sort_keys(unsigned long long* skey, int total, int lane) {
+  T k[R];
+#pragma unroll
+  for (int r = 0; r < R; ++r) {
+    const int e = lane * R + r;
+    if (e < total) {
+      const unsigned long long full = skey[e];
+      k[r] = sizeof(T) == 4 ? (T)(((unsigned)(full >> 32) << 10) | ((unsigned)full & 1023u)) : (T)full;
+    } else {
+      k[r] = (T)~(T)0;
+    }
+  }
+  warp_bitonic_sort<R, T>(k, lane);
+  __syncwarp();
+#pragma unroll
+  for (int r = 0; r < R; ++r) {
+    const int e = lane * R + r;
+    if (e < total)
+      skey[e] = sizeof(T) == 4 ? (((unsigned long long)((unsigned)k[r] >> 10) << 32) | ((unsigned)k[r] & 1023u))
+                               : (unsigned long long)k[r];
+  }
+}
+
+// Row i of C = A B - B A is a linear combination of sparse rows: + a_ik B_k for the entries of A's row i and
+// - b_ik A_k for those of B's row i, L = len A_i + len B_i source rows ("lists").  ONE WARP per row:
+//   1. every lane looks up its lists (lane, lane + 32, ...) and a warp scan gives each list its place in a
+//      per-warp candidate buffer in shared memory;
+//   2. expand: the lane copies its lists there -- key = (column << 32) | position, value = +-coefficient times
+//      entry -- all loads independent of one another;
+//   3. the warp sorts the 64-bit keys with a bitonic network in REGISTERS (16 or 32 keys per lane, shuffles
+//      between lanes, fully unrolled);
+//   4. every lane takes a contiguous piece of the sorted keys, sums each run of equal columns that starts in
+//      its piece IN POSITION ORDER (positions are unique, so the sorted order and therefore every sum is
+//      fixed: the A-part in k order, then the B-part in k order), drops exact zeros, and a warp scan places
+//      the survivors, which are already in column order.
+// The spin chains need (N/2 + 1) N 2 candidates per row (624 at N = 24); a row with more than kSortCap
+// candidates or more than kCommLists lists is left to the CTA-wide sorting kernel below.
+const int kCommLists = 256;
+const int kMergeWarps = 2;
+const int kSortCap = 1024;
+const int kCommTmp = 32;      // entries of a row of C the warp kernel parks in the temporary buffer
+const int kMergeSmem = kMergeWarps * (kSortCap * (int)(sizeof(cplx) + sizeof(unsigned long long)) + 3 * kCommLists * (int)sizeof(int));
+
+// counts[row] = entries of row i of C; the entries themselves go to tmp_ci / tmp_v at row * kCommTmp (the gather
+// kernel moves them to their CSR place once the row pointers are known).  A row this kernel does not take --
+// too many lists or candidates, or more than kCommTmp entries -- is appended to `work` (work[0] = how many).
+__global__ void __launch_bounds__(kMergeWarps * 32) csr_commutator_merge_kernel(CsrRaw A, CsrRaw B, int64_t n,
+                                                                                int32_t* __restrict__ counts,
+                                                                                int32_t* __restrict__ tmp_ci,
+                                                                                cplx* __restrict__ tmp_v, int* work) {
+  constexpr bool WRITE = false;
+  extern __shared__ __align__(16) unsigned char cm_smem[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  cplx* sval = reinterpret_cast<cplx*>(cm_smem) + warp * kSortCap;
+  unsigned long long* skey = reinterpret_cast<unsigned long long*>(cm_smem + kMergeWarps * kSortCap * sizeof(cplx)) + warp * kSortCap;
+  int* lq = reinterpret_cast<int*>(cm_smem + kMergeWarps * kSortCap * (sizeof(cplx) + sizeof(unsigned long long))) +
+            warp * 3 * kCommLists;
+  int* llen = lq + kCommLists;
+  int* lo = llen + kCommLists;
+  const int64_t nwarps = (int64_t)gridDim.x * kMergeWarps;
+  const bool narrow = n <= ((int64_t)1 << 22);
+  for (int64_t row = (int64_t)blockIdx.x * kMergeWarps + warp; row < n; row += nwarps) {
+    const int pa = A.rp[row], lenA = A.rp[row + 1] - pa, pb = B.rp[row], lenB = B.rp[row + 1] - pb;
+    const int L = lenA + lenB;
+    int total = 0;
+    if (L <= kCommLists) {
+      __syncwarp();
+      for (int t0 = 0; t0 < L; t0 += 32) {               // 1. the lists and their places
+        const int t = t0 + lane;
+        int q = 0, len = 0;
+        if (t < L) {
+          const bool fromA = t < lenA;                   // + a_ik B_k  or  - b_ik A_k
+          const int k = fromA ? A.ci[pa + t] : B.ci[pb + t - lenA];
+          const CsrRaw& S = fromA ? B : A;
+          q = S.rp[k];
+          len = S.rp[k + 1] - q;
+        }
+        int inc = len;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+          const int up = __shfl_up_sync(0xffffffffu, inc, d);
+          if (lane >= d) inc += up;
+        }
+        if (t < L) {
+          lq[t] = q;
+          llen[t] = len;
+          lo[t] = total + inc - len;
+        }
+        total += __shfl_sync(0xffffffffu, inc, 31);
+      }
+    }
+    if (L > kCommLists || total > kSortCap) {            // warp-uniform: the CTA-wide kernel takes this row
+      if (lane == 0) {
+        counts[row] = 0;
+        work[1 + atomicAdd(work, 1)] = (int)row;
+      }
+      continue;
+    }
+    __syncwarp();
+    for (int t = lane; t < L; t += 32) {                 // 2. expand
+      const bool fromA = t < lenA;
+      const CsrRaw& S = fromA ? B : A;
+      cplx coef = fromA ? A.v[pa + t] : B.v[pb + t - lenA];
+      if (!fromA) {
+        coef.x = -coef.x;
+        coef.y = -coef.y;
+      }
+      const int q = lq[t], len = llen[t], o = lo[t];
+#pragma unroll 4
+      for (int j = 0; j < len; ++j) {
+        skey[o + j] = ((unsigned long long)(unsigned)S.ci[q + j] << 32) | (unsigned)(o + j);
+        sval[o + j] = cmul(coef, S.v[q + j]);
+      }
+    }
+    __syncwarp();
+    // 3. sort the keys: into registers (lane-contiguous), network, back to shared memory.  When column and
+    // position fit 32 bits together (n * 1024 <= 2^32) the network runs on 32-bit keys (min / max per exchange).
+    if (narrow) {
+      if (total <= 16 * 32) sort_keys<16, unsigned, WRITE>(skey, total, lane);
+      else sort_keys<32, unsigned, WRITE>(skey, total, lane);
+    } else {
+      if (total <= 16 * 32) sort_keys<16, unsigned long long, WRITE>(skey, total, lane);
+      else sort_keys<32, unsigned long long, WRITE>(skey, total, lane);
+    }
+    __syncwarp();
+    // 4. runs of equal columns; a lane owns the runs that start in its piece
+    const int per = (total + 31) >> 5, s0 = min(total, lane * per), s1 = min(total, s0 + per);
+    int cnt = 0;
+    for (int p = s0; p < s1; ++p) {
+      const unsigned c = (unsigned)(skey[p] >> 32);
+      if (p > 0 && (unsigned)(skey[p - 1] >> 32) == c) continue;
+      cplx z = sval[(unsigned)skey[p]];
+      for (int u = p + 1; u < total && (unsigned)(skey[u] >> 32) == c; ++u) {
+        const cplx y = sval[(unsigned)skey[u]];
+        z.x += y.x;
+        z.y += y.y;
+      }
+      if (z.x != 0.0 || z.y != 0.0) ++cnt;
+    }
+    int inc = cnt;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const int up = __shfl_up_sync(0xffffffffu, inc, d);
+      if (lane >= d) inc += up;
+    }
+    const int nrow = __shfl_sync(0xffffffffu, inc, 31);
+    if (nrow > kCommTmp) {                               // warp-uniform
+      if (lane == 0) {
+        counts[row] = 0;
+        work[1 + atomicAdd(work, 1)] = (int)row;
+      }
+      continue;
+    }
+    if (lane == 0) counts[row] = nrow;
+    int o = inc - cnt;
+    int32_t* oc = tmp_ci + row * kCommTmp;
+    cplx* ov = tmp_v + row * kCommTmp;
+    for (int p = s0; p < s1; ++p) {
+      const unsigned c = (unsigned)(skey[p] >> 32);
+      if (p > 0 && (unsigned)(skey[p - 1] >> 32) == c) continue;
+      cplx z = sval[(unsigned)skey[p]];
+      for (int u = p + 1; u < total && (unsigned)(skey[u] >> 32) == c; ++u) {
+        const cplx y = sval[(unsigned)skey[u]];
+        z.x += y.x;
+        z.y += y.y;
+      }
+      if (z.x != 0.0 || z.y != 0.0) {
+        oc[o] = (int)c;
+        ov[o] = z;
+        ++o;
+      }
+    }
+  }
+}
+
+// rows the warp kernel finished: tmp -> CSR place (one warp per row)
+__global__ void __launch_bounds__(256) csr_commutator_gather_kernel(int64_t n, const int32_t* __restrict__ counts,
+                                                                     const int32_t* __restrict__ rp,
+                                                                     const int32_t* __restrict__ tmp_ci,
+                                                                     const cplx* __restrict__ tmp_v,
+                                                                     int32_t* __restrict__ ci_out, cplx* __restrict__ v_out) {
+  const int lane = threadIdx.x & 31;
+  const int64_t row = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (row >= n) return;
+  const int o = rp[row], len = rp[row + 1] - o;
+  if (len > kCommTmp) return;   // a row of the CTA-wide kernel, which writes after this kernel (so does it for its
+                                // shorter rows: what is copied here for them is overwritten)
+  for (int j = lane; j < len; j += 32) {
+    ci_out[o + j] = tmp_ci[row * kCommTmp + j];
+    v_out[o + j] = tmp_v[row * kCommTmp + j];
+  }
+}
+
 template <bool WRITE>
 __global__ void __launch_bounds__(kCommThreads) csr_commutator_kernel(CsrRaw A, CsrRaw B, int64_t n,
                                                                        int32_t* __restrict__ counts,
                                                                        const int32_t* __restrict__ rp_out,
                                                                        int32_t* __restrict__ ci_out,
-                                                                       cplx* __restrict__ v_out, int* overflow) {
+                                                                       cplx* __restrict__ v_out, int* overflow,
+                                                                       const int* __restrict__ work) {
   __shared__ int keys[kCommCap];
   __shared__ cplx vals[kCommCap];
   __shared__ int scan[kCommThreads + 1];
-  for (int64_t row = blockIdx.x; row < n; row += gridDim.x) {
+  (void)n;
+  const int nwork = work[0];                     // the rows the warp kernel left over
+  for (int wi = blockIdx.x; wi < nwork; wi += gridDim.x) {
+    const int64_t row = work[1 + wi];
     int total = 0;
     comm_expand(A, B, row, 1.0, keys, vals, total, overflow);
     if (total <= kCommCap) comm_expand(B, A, row, -1.0, keys, vals, total, overflow);
@@ -579,6 +813,9 @@ int csr_commutator_build(const CsrRaw& A, const CsrRaw& B, int64_t n, int32_t** 
   int32_t* counts = nullptr;
   int32_t* rp = nullptr;
   int* overflow = nullptr;
+  int* work = nullptr;          // [0] = rows left to the CTA-wide kernel, then the rows
+  int32_t* tmp_ci = nullptr;
+  cplx* tmp_v = nullptr;
   void* tmp = nullptr;
   size_t tmp_bytes = 0;
   int rc = MAGNUS_OK;
@@ -587,19 +824,35 @@ int csr_commutator_build(const CsrRaw& A, const CsrRaw& B, int64_t n, int32_t** 
   *v_out = nullptr;
   if (cudaMalloc(&counts, sizeof(int32_t) * (size_t)(n + 1)) != cudaSuccess ||
       cudaMalloc(&rp, sizeof(int32_t) * (size_t)(n + 1)) != cudaSuccess ||
-      cudaMalloc(&overflow, sizeof(int)) != cudaSuccess) {
+      cudaMalloc(&overflow, sizeof(int)) != cudaSuccess ||
+      cudaMalloc(&work, sizeof(int) * (size_t)(n + 1)) != cudaSuccess ||
+      cudaMalloc(&tmp_ci, sizeof(int32_t) * (size_t)n * kCommTmp) != cudaSuccess ||
+      cudaMalloc(&tmp_v, sizeof(cplx) * (size_t)n * kCommTmp) != cudaSuccess) {
+    cudaGetLastError();
+    set_error("sparse commutator: workspace allocation failed (n=%lld)", (long long)n);
     rc = MAGNUS_ENOMEM;
   }
   const int64_t gmax = (int64_t)device_sm_count() * 16;
-  int grid = (int)(n < gmax ? n : gmax);
-  int h_over = 0;
+  const int64_t mrows = (n + kMergeWarps - 1) / kMergeWarps;
+  const int mgrid = (int)(mrows < gmax ? mrows : gmax);
+  int h_over = 0, h_work = 0, grid = 1;
   int32_t h_nnz = 0;
   if (rc == MAGNUS_OK) {
     cudaMemsetAsync(overflow, 0, sizeof(int), st);
-    cudaMemsetAsync(counts, 0, sizeof(int32_t) * (size_t)(n + 1), st);
-    csr_commutator_kernel<false><<<grid, kCommThreads, 0, st>>>(A, B, n, counts, nullptr, nullptr, nullptr, overflow);
-    cub::DeviceScan::ExclusiveSum(nullptr, tmp_bytes, counts, rp, (int)(n + 1), st);
-    if (cudaMalloc(&tmp, tmp_bytes) != cudaSuccess) rc = MAGNUS_ENOMEM;
+    cudaMemsetAsync(work, 0, sizeof(int), st);
+    cudaMemsetAsync(counts + n, 0, sizeof(int32_t), st);
+    cudaFuncSetAttribute(csr_commutator_merge_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMergeSmem);
+    csr_commutator_merge_kernel<<<mgrid, kMergeWarps * 32, kMergeSmem, st>>>(A, B, n, counts, tmp_ci, tmp_v, work);
+    cudaMemcpyAsync(&h_work, work, sizeof(int), cudaMemcpyDeviceToHost, st);
+    if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) rc = MAGNUS_ECUDA;
+    grid = (int)(h_work < gmax ? (h_work > 0 ? h_work : 1) : gmax);
+    if (rc == MAGNUS_OK && h_work)   // rows with too many source rows, candidates or entries: expand / sort / merge
+      csr_commutator_kernel<false><<<grid, kCommThreads, 0, st>>>(A, B, n, counts, nullptr, nullptr, nullptr, overflow,
+                                                                  work);
+    if (rc == MAGNUS_OK) {
+      cub::DeviceScan::ExclusiveSum(nullptr, tmp_bytes, counts, rp, (int)(n + 1), st);
+      if (cudaMalloc(&tmp, tmp_bytes) != cudaSuccess) rc = MAGNUS_ENOMEM;
+    }
   }
   if (rc == MAGNUS_OK) {
     cub::DeviceScan::ExclusiveSum(tmp, tmp_bytes, counts, rp, (int)(n + 1), st);
@@ -619,11 +872,16 @@ int csr_commutator_build(const CsrRaw& A, const CsrRaw& B, int64_t n, int32_t** 
       rc = MAGNUS_ENOMEM;
   }
   if (rc == MAGNUS_OK) {
-    csr_commutator_kernel<true><<<grid, kCommThreads, 0, st>>>(A, B, n, nullptr, rp, ci, v, overflow);
+    const int64_t gblocks = (n * 32 + 255) / 256;
+    csr_commutator_gather_kernel<<<(unsigned)gblocks, 256, 0, st>>>(n, counts, rp, tmp_ci, tmp_v, ci, v);
+    if (h_work) csr_commutator_kernel<true><<<grid, kCommThreads, 0, st>>>(A, B, n, nullptr, rp, ci, v, overflow, work);
     if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) rc = MAGNUS_ECUDA;
   }
   cudaFree(counts);
   cudaFree(overflow);
+  cudaFree(work);
+  cudaFree(tmp_ci);
+  cudaFree(tmp_v);
   cudaFree(tmp);
   if (rc != MAGNUS_OK) {
     cudaFree(rp);

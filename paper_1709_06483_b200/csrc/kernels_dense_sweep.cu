@@ -269,4 +269,28 @@ int launch_dense_leja_sweep_jobs(int64_t n, const cplx* H0, int64_t ld0, const c
   return MAGNUS_OK;
 }
 
+// one sweep on an assembled matrix (leja_expmv, M4 / M6 steps, sub-steps, the fall-back after a failed batch): a
+// one-job batch through job slot 0.  out != v: v is copied first (the kernel works in place); a sweep that does
+// not converge leaves out as that copy.
+int launch_dense_leja_sweep(const DenseOp& op, const cplx* v, cplx* out, double inv_gamma, double c_over_gamma,
+                            double tol, int m_max, cplx phase, const SweepTable& tab, Workspace* ws, cudaStream_t st) {
+  if (ensure_sweep_jobs(ws) != MAGNUS_OK) return MAGNUS_ENOMEM;
+  SweepJob& J = ws->jobs_host[0];
+  J.coef[0] = J.coef[1] = J.coef[2] = make_double2(0.0, 0.0);
+  J.phase = phase;
+  J.inv_gamma = inv_gamma;
+  J.c_over_gamma = c_over_gamma;
+  J.m_max = m_max;
+  J.nterms = 1;
+  J.flags = kSweepJobAssembled;
+  J.pad = 0;
+  for (int k = 0; k <= m_max; ++k) J.d[k] = tab.d[k];
+  if (cudaMemcpyAsync(ws->jobs, &J, sizeof(SweepJob), cudaMemcpyHostToDevice, st) != cudaSuccess) return MAGNUS_ECUDA;
+  if (out != v &&
+      cudaMemcpyAsync(out, v, sizeof(cplx) * (size_t)op.n, cudaMemcpyDeviceToDevice, st) != cudaSuccess)
+    return MAGNUS_ECUDA;
+  return launch_dense_leja_sweep_jobs(op.n, nullptr, 0, nullptr, 0, const_cast<cplx*>(op.M), out, ws->jobs, 1, tol,
+                                      ws->status, nullptr, ws, st);
+}
+
 }  // namespace magnus

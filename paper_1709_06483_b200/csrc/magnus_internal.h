@@ -248,6 +248,8 @@ bool dense_sweep_supported(int64_t n);
 int launch_dense_leja_sweep_jobs(int64_t n, const cplx* H0, int64_t ld0, const cplx* H1, int64_t ld1, cplx* M, cplx* psi,
                                  const SweepJob* jobs, int njobs, double tol, LejaStatus* status, const LejaStatus* gate,
                                  Workspace* ws, cudaStream_t st);
+int launch_dense_leja_sweep(const DenseOp& op, const cplx* v, cplx* out, double inv_gamma, double c_over_gamma,
+                            double tol, int m_max, cplx phase, const SweepTable& tab, Workspace* ws, cudaStream_t st);
 int launch_dense_leja_iter(const DenseOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma, double shift,
                            cplx dk, double abs_dk, double tol, Workspace* ws, cudaStream_t st);
 int dense_hermitian_check(const DenseOp& op, cudaStream_t st, double* max_violation);

@@ -580,3 +580,66 @@ def test_small_csr_sweep_paths(M, oracle):
             st = h.integrate(0.0, 0.2, 4, psi)
         res[ck] = (st["iters"], host(psi))
     assert np.array_equal(res[0][0], res[1][0]) and relerr(res[0][1], res[1][1]) <= 1e-13
+
+
+# ------------------------------------------------------------------ planned batches (whole-sweep kernels)
+@pytest.mark.parametrize("scheme", ["cf4", "cf4:3"])
+@pytest.mark.parametrize("n", [1, 2, 33, 150, 777, 1237])
+def test_planned_dense_sweep_ragged_sizes(M, oracle, scheme, n):
+    """Dense n <= 4096 with a commutator-free scheme runs planned batches on the persistent sweep kernel:
+    sizes below the CTA count (CTAs without rows), ragged row/column tails, n = 1 (gamma = 0: that exponential
+    takes the stepwise path inside the batch).  Against the oracle and against the per-iteration kernels."""
+    cfg = W.scaled(W.CONFIGS["cfg2"], n, 5)
+    H0, H1, psi0, f = W.build(cfg)
+    ref, riters = oracle.magnus_integrate(H0.numpy(), H1.numpy(), f, scheme, cfg.t0, cfg.t_end, cfg.nsteps, psi0.numpy(), cfg.tol)
+    res = {}
+    for ck in (0, 1):
+        psi = psi0.to(DEV).clone()
+        with M.magnus_create(H0.to(DEV), H1.to(DEV), f, scheme, tol=cfg.tol, csr_kernel=ck) as h:
+            if ck == 0 and n > 1:
+                assert h.describe()["leja_kernel"] == "dense_leja_sweep_kernel"
+            st = h.integrate(cfg.t0, cfg.t_end, cfg.nsteps, psi)
+        res[ck] = (st["iters"], host(psi))
+        assert np.array_equal(st["iters"], riters)
+        assert relerr(host(psi), ref) <= 1e-9
+    assert relerr(res[0][1], res[1][1]) <= 1e-13
+
+
+@pytest.mark.parametrize("kind", ["xxz", "dense"])
+def test_planned_batch_with_substeps_and_nonconvergence(M, oracle, kind):
+    """A theta_max between the smallest and the largest theta of the run: some exponentials need sub-steps (the
+    planner hands those to the stepwise path and resumes behind them), the rest run as jobs.  Same counts and
+    psi as the all-stepwise run.  Then tol = 1e-300: the first job fails, the stepwise redo reports ENOCONV and
+    psi is still the initial state."""
+    cfg = W.scaled(W.CONFIGS["cfg1"], 8, 12) if kind == "xxz" else W.scaled(W.CONFIGS["cfg2"], 300, 12)
+    H0, H1, psi0, f = W.build(cfg)
+    d0, d1 = H0.to(DEV), H1.to(DEV)
+    psi = psi0.to(DEV).clone()
+    with M.magnus_create(d0, d1, f, "cf4", tol=cfg.tol, csr_kernel=1) as h:
+        thetas = sorted(abs(i["theta"]) for s in range(cfg.nsteps) for i in h.step(cfg.t0 + s * cfg.tau, cfg.tau, psi))
+    theta_max = 0.5 * (thetas[len(thetas) // 2 - 1] + thetas[len(thetas) // 2])
+    assert thetas[0] < theta_max < thetas[-1]
+    res = {}
+    for ck in (0, 1):
+        psi = psi0.to(DEV).clone()
+        with M.magnus_create(d0, d1, f, "cf4", tol=cfg.tol, csr_kernel=ck, theta_max=theta_max) as h:
+            infos = [i for s in range(0, cfg.nsteps, 4) for i in [h.integrate(cfg.t0 + s * cfg.tau, cfg.t0 + (s + 4) * cfg.tau, 4, psi)]]
+        res[ck] = (np.concatenate([i["iters"] for i in infos]), host(psi))
+    assert np.array_equal(res[0][0], res[1][0]) and relerr(res[0][1], res[1][1]) <= 1e-13
+    o0, o1 = (oracle.CsrHost.of(H0), oracle.CsrHost.of(H1)) if kind == "xxz" else (H0.numpy(), H1.numpy())
+    ref, _ = oracle.magnus_integrate(o0, o1, f, "cf4", cfg.t0, cfg.t_end, cfg.nsteps, psi0.numpy(), cfg.tol)
+    assert relerr(res[0][1], ref) <= 1e-9          # sub-steps change the counts, not the result
+    psi = psi0.to(DEV).clone()
+    with M.magnus_create(d0, d1, f, "cf4", tol=1e-300) as h:   # planned path: the first job fails, then the stepwise redo
+        with pytest.raises(M.MagnusError) as e:
+            h.integrate(cfg.t0, cfg.t0 + 6.0, 3, psi)    # tau = 2: theta about 10, |d_128| about 1e-88 > tol
+    assert e.value.code == -4 and torch.equal(psi, psi0.to(DEV))
+
+
+def test_planned_batch_longer_than_the_plan_capacity(M, oracle):
+    """1500 CF4 steps = 3000 exponentials > the ring of job slots (256) and two plans of 1365 steps: counts
+    and psi against the oracle."""
+    cfg = W.scaled(W.CONFIGS["cfg1"], 6, 1500)
+    psi, st, ref, riters = run_config(M, oracle, cfg, "cf4")
+    assert st["n_exp"] == 3000 and np.array_equal(st["iters"], riters)
+    assert relerr(psi, ref) <= 1e-9
