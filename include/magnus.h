@@ -228,7 +228,12 @@ int magnus_omega_dense(int64_t n, const void* H0, int64_t ld0, const void* H1, i
 
 /* C = A B - B A for CSR A, B (device), exact zeros dropped.  Two-call protocol:
  * with cap_nnz == 0 only *nnz_out is written; otherwise row_ptr_out[n+1],
- * col_idx_out, values_out (device, capacity cap_nnz) are filled. */
+ * col_idx_out, values_out (device, capacity cap_nnz) are filled.
+ * Limits (also for magnus_create with MAGNUS_M4 on CSR input, which calls this): a row i is built from
+ * the rows B_k (k in A's row i) and A_k (k in B's row i); up to 256 such source rows with at most 1024
+ * entries in total and 32 resulting entries are handled by a warp, anything beyond by a CTA that holds at
+ * most 2048 candidate products -- a row that needs more returns MAGNUS_EINVAL (spin chains need 2 N^2).
+ * Needs temporary device memory of 640 bytes per row. */
 int magnus_commutator_csr(const magnus_matrix* A, const magnus_matrix* B, int64_t cap_nnz,
                           int64_t* nnz_out, int32_t* row_ptr_out, int32_t* col_idx_out,
                           void* values_out, void* stream);

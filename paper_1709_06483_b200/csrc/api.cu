@@ -85,6 +85,7 @@ struct OpRef {
 
 static int read_interval(int nblk, Workspace* ws, cudaStream_t st, double* a, double* b) {
   (void)nblk;   // the min/max over blocks is taken by the last block of the producing kernel
+  CU_TRY(cudaGetLastError());   // a failed launch of the producing kernel must not turn into a garbage interval
   CU_TRY(cudaMemcpyAsync(ws->ab_host, ws->gersh + 2 * kMaxPartials, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
   CU_TRY(cudaStreamSynchronize(st));
   *a = ws->ab_host[0];
@@ -245,6 +246,7 @@ static int expmv_on_interval(const OpRef& op, double a_raw, double b_raw, const 
         launch_iter(op, ws->w[(k - 1) & 1], ws->w[k & 1], ws->p, inv_gamma, shift,
                     make_double2(d[k].real(), d[k].imag()), std::abs(d[k]), prm.tol, ws, st);
       }
+      CU_TRY(cudaGetLastError());   // a failed launch must surface as ECUDA, not as ENOCONV at m_max
       if (ws->time_leja) CU_TRY(cudaEventRecord(ws->ev[1], st));
       CU_TRY(cudaMemcpyAsync(ws->status_host, ws->status, sizeof(LejaStatus), cudaMemcpyDeviceToHost, st));
       CU_TRY(cudaStreamSynchronize(st));

@@ -30,9 +30,8 @@ __global__ void __launch_bounds__(256) leja_init_kernel(const cplx* __restrict__
 
 // S7 (the stop test) runs in the last block of the init / iteration kernels: leja_finalize.cuh.
 
-// S8 (c7): out = e^{-i (h/s) c} p.
-__global__ void __launch_bounds__(256) scale_copy_kernel(const cplx* __restrict__ in, cplx* __restrict__ out, int64_t n,
-                                                          cplx phase) {
+// S8 (c7): out = e^{-i (h/s) c} p.  in == out is allowed (gamma = 0 on an in-place step): no __restrict__.
+__global__ void __launch_bounds__(256) scale_copy_kernel(const cplx* in, cplx* out, int64_t n, cplx phase) {
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
     out[i] = cmul(phase, in[i]);
 }

@@ -25,7 +25,7 @@ namespace {
 constexpr int DS_THREADS = 512;
 constexpr int DS_WARPS = DS_THREADS / 32;
 constexpr int DS_MAX_ROWS = 32;                 // rows per CTA
-constexpr int DS_RG = 4;                        // rows in flight together
+constexpr int DS_RG = 7;                        // rows in flight together
 constexpr int DS_SMEM = kDenseSweepMaxN * (int)sizeof(cplx);   // the vector w
 
 __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {

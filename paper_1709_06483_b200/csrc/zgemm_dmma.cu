@@ -10,6 +10,10 @@
 // planes of a fragment element.  K is consumed in slabs of 16 complex through a
 // 3-stage cp.async ring (16-byte copies, zero-filled outside the matrix).
 // Row pitches of 20 (A) and 66 (B) double2 make the fragment loads conflict-free.
+// Two instantiations: 128 x 64 tiles (8 warps, one CTA per SM) and 64 x 64 tiles (4 warps, two CTAs per SM).
+// The small tile is for sizes whose 128 x 64 tile count leaves the last wave mostly empty (n = 2048: 512
+// tiles on 148 SMs = 3.46 waves): with two CTAs per SM the last, partial wave has an SM to itself per CTA
+// and runs at about twice the per-CTA speed, so the tail costs half a wave instead of a whole one.
 #include "magnus_internal.h"
 #include "device_utils.cuh"
 
@@ -17,12 +21,12 @@ namespace magnus {
 
 namespace {
 
-constexpr int BM = 128, BN = 64, BK = 16, STAGES = 3;
+constexpr int BN = 64, BK = 16, STAGES = 3;
 constexpr int LDA_S = BK + 4;    // double2 units
 constexpr int LDB_S = BN + 2;
-constexpr int A_STAGE = BM * LDA_S;          // double2 per stage
 constexpr int B_STAGE = BK * LDB_S;
-constexpr int ZGEMM_SMEM = STAGES * (A_STAGE + B_STAGE) * (int)sizeof(cplx);
+template <int BM>
+constexpr int zgemm_smem() { return STAGES * (BM * LDA_S + B_STAGE) * (int)sizeof(cplx); }
 
 __device__ __forceinline__ void cp_async16_zfill(void* dst_smem, const void* src, bool valid) {
   const unsigned s = (unsigned)__cvta_generic_to_shared(dst_smem);
@@ -41,10 +45,13 @@ __device__ __forceinline__ void dmma8x8x4(double& c0, double& c1, double a, doub
                : "d"(a), "d"(b));
 }
 
-__global__ void __launch_bounds__(256, 1) zgemm_dmma_kernel(int64_t n, const cplx* __restrict__ A, int64_t lda,
-                                                             const cplx* __restrict__ B, int64_t ldb,
-                                                             cplx* __restrict__ C, int64_t ldc, int tiles_m,
-                                                             int tiles_n) {
+template <int BM>
+__global__ void __launch_bounds__(BM * 2, BM == 128 ? 1 : 2) zgemm_dmma_kernel(int64_t n, const cplx* __restrict__ A, int64_t lda,
+                                                                       const cplx* __restrict__ B, int64_t ldb,
+                                                                       cplx* __restrict__ C, int64_t ldc, int tiles_m,
+                                                                       int tiles_n) {
+  constexpr int THREADS = BM * 2;              // BM / 32 x 2 warps
+  constexpr int A_STAGE = BM * LDA_S;          // double2 per stage
   extern __shared__ __align__(16) unsigned char zg_smem[];
   cplx* sA = reinterpret_cast<cplx*>(zg_smem);
   cplx* sB = sA + STAGES * A_STAGE;
@@ -61,7 +68,7 @@ __global__ void __launch_bounds__(256, 1) zgemm_dmma_kernel(int64_t n, const cpl
   const int64_t m0 = (int64_t)tm * BM, n0 = (int64_t)tn * BN;
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int wm = warp >> 1, wn = warp & 1;           // 4 x 2 warps
+  const int wm = warp >> 1, wn = warp & 1;           // BM / 32 x 2 warps
   const int g = lane >> 2, q = lane & 3;
 
   double cre[4][4][2], cim[4][4][2];
@@ -80,16 +87,16 @@ __global__ void __launch_bounds__(256, 1) zgemm_dmma_kernel(int64_t n, const cpl
     cplx* a_dst = sA + stage * A_STAGE;
     cplx* b_dst = sB + stage * B_STAGE;
 #pragma unroll
-    for (int i = 0; i < (BM * BK) / 256; ++i) {
-      const int idx = tid + i * 256;
+    for (int i = 0; i < (BM * BK) / THREADS; ++i) {
+      const int idx = tid + i * THREADS;
       const int r = idx / BK, kk = idx % BK;
       const int64_t gr = m0 + r, gk = k0 + kk;
       const bool ok = gr < n && gk < n;
       cp_async16_zfill(a_dst + r * LDA_S + kk, A + (ok ? gr * lda + gk : 0), ok);
     }
 #pragma unroll
-    for (int i = 0; i < (BK * BN) / 256; ++i) {
-      const int idx = tid + i * 256;
+    for (int i = 0; i < (BK * BN) / THREADS; ++i) {
+      const int idx = tid + i * THREADS;
       const int kk = idx / BN, c = idx % BN;
       const int64_t gk = k0 + kk, gc = n0 + c;
       const bool ok = gk < n && gc < n;
@@ -184,11 +191,26 @@ __global__ void __launch_bounds__(256) dfma_peak_kernel(int iters, double* __res
 
 int launch_zgemm(int64_t n, const cplx* A, int64_t lda, const cplx* B, int64_t ldb, cplx* C, int64_t ldc,
                  cudaStream_t st) {
+  // wave efficiency of the 128 x 64 tiling: tiles / (waves * SMs); below 0.93 the 64 x 64 tiling (two CTAs per SM,
+  // half-cost tail) is used
+  const int sms = device_sm_count();
+  const int tn = (int)((n + BN - 1) / BN);
+  const int64_t t128 = (int64_t)((n + 127) / 128) * tn;
+  const double eff128 = (double)t128 / (double)(((t128 + sms - 1) / sms) * sms);
   // per launch (cheap): the attribute is per device, a process-wide flag would miss a second GPU
-  if (cudaFuncSetAttribute(zgemm_dmma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ZGEMM_SMEM) != cudaSuccess)
-    return MAGNUS_ECUDA;
-  const int tiles_m = (int)((n + BM - 1) / BM), tiles_n = (int)((n + BN - 1) / BN);
-  zgemm_dmma_kernel<<<tiles_m * tiles_n, 256, ZGEMM_SMEM, st>>>(n, A, lda, B, ldb, C, ldc, tiles_m, tiles_n);
+  if (eff128 >= 0.93) {
+    if (cudaFuncSetAttribute(zgemm_dmma_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, zgemm_smem<128>()) !=
+        cudaSuccess)
+      return MAGNUS_ECUDA;
+    const int tm = (int)((n + 127) / 128);
+    zgemm_dmma_kernel<128><<<tm * tn, 256, zgemm_smem<128>(), st>>>(n, A, lda, B, ldb, C, ldc, tm, tn);
+  } else {
+    if (cudaFuncSetAttribute(zgemm_dmma_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, zgemm_smem<64>()) !=
+        cudaSuccess)
+      return MAGNUS_ECUDA;
+    const int tm = (int)((n + 63) / 64);
+    zgemm_dmma_kernel<64><<<tm * tn, 128, zgemm_smem<64>(), st>>>(n, A, lda, B, ldb, C, ldc, tm, tn);
+  }
   return cudaGetLastError() == cudaSuccess ? MAGNUS_OK : MAGNUS_ECUDA;
 }
 

@@ -298,16 +298,21 @@ def test_sparse_commutator_vs_oracle(M, oracle, N):
     assert np.array_equal(got.data, ref.data)               # small integers: exact
 
 
-def test_sparse_commutator_general(M, oracle):
-    A = random_sparse_hermitian(400, 0.02, 21)
-    B = random_sparse_hermitian(400, 0.02, 22)
+@pytest.mark.parametrize("n,density,long_row", [(400, 0.02, None), (1500, 0.002, (7, 300)), (900, 0.004, (11, 120))])
+def test_sparse_commutator_general(M, oracle, n, density, long_row):
+    """General CSR input.  Rows with more than 32 resulting entries (most rows of the first case), with more
+    than 256 source rows (the long row of the second) or with more than 1024 candidate products leave the
+    warp kernel through its worklist and are done by the CTA-wide kernel; the others stay with the warp."""
+    A = random_sparse_hermitian(n, density, 21, long_row=long_row)
+    B = random_sparse_hermitian(n, density, 22)
     rp, ci, v = M.magnus_commutator_csr(csr_from_scipy(A), csr_from_scipy(B))
     import scipy.sparse as sp
-    got = sp.csr_matrix((host(v), host(ci), host(rp)), shape=(400, 400)).toarray()
-    K = oracle.commutator(oracle.CsrHost(400, A.indptr.astype(np.int32), A.indices.astype(np.int32), A.data.astype(complex)),
-                          oracle.CsrHost(400, B.indptr.astype(np.int32), B.indices.astype(np.int32), B.data.astype(complex)))
-    ref = sp.csr_matrix((K.values, K.col_idx, K.row_ptr), shape=(400, 400)).toarray()
+    got = sp.csr_matrix((host(v), host(ci), host(rp)), shape=(n, n)).toarray()
+    K = oracle.commutator(oracle.CsrHost(n, A.indptr.astype(np.int32), A.indices.astype(np.int32), A.data.astype(complex)),
+                          oracle.CsrHost(n, B.indptr.astype(np.int32), B.indices.astype(np.int32), B.data.astype(complex)))
+    ref = sp.csr_matrix((K.values, K.col_idx, K.row_ptr), shape=(n, n)).toarray()
     assert np.max(np.abs(got - ref)) <= 1e-13 * max(1.0, np.max(np.abs(ref)))
+    assert np.all(np.diff(host(ci)[host(rp)[7]:host(rp)[8]]) > 0)      # columns ascending inside a row
 
 
 # ------------------------------------------------------------------ magnus_step / magnus_integrate
