@@ -370,23 +370,29 @@ def respawn_under_torchrun(args) -> int:
 
 
 def measure_extra(M, W, torch, dev, peaks, dmma_tf):
-    """Short secondary measurements for the default line: cfg4 CF4 (2 steps, dense GEMV), cfg4 M4 (1 step, DMMA) and,
-    reported separately from the mandated path, cfg4 M4 with the cached-commutator shortcut."""
+    """Short secondary measurements for the default line, so that the driver's record carries every part of the
+    metric: cfg4 CF4 (dense GEMV GB/s), cfg4 M4 (DMMA commutator TFLOP/s), the latency-bound configs cfg1 / cfg2
+    (whole-sweep kernels, planned batches) and cfg3 (the CSR kernel at N = 20) and, reported separately from the
+    mandated path, cfg4 M4 with the cached-commutator shortcut."""
     out = {}
-    cfg = W.CONFIGS["cfg4"]
-    for scheme, steps, shortcuts, key in (("cf4", 2, 0, "cfg4_cf4"), ("m4", 1, 0, "cfg4_m4"),
-                                          ("m4", 2, M.SHORTCUT_CACHED_COMMUTATOR, "cfg4_m4_shortcut_cached_commutator")):
+    runs = (("cfg4", "cf4", 2, 1, 0, "cfg4_cf4"), ("cfg4", "m4", 1, 1, 0, "cfg4_m4"),
+            ("cfg1", "cf4", 100, 20, 0, "cfg1_cf4"), ("cfg1", "m4", 100, 20, 0, "cfg1_m4"),
+            ("cfg2", "cf4", 50, 10, 0, "cfg2_cf4"), ("cfg2", "m4", 20, 3, 0, "cfg2_m4"),
+            ("cfg3", "cf4", 10, 3, 0, "cfg3_cf4"), ("cfg3", "m4", 10, 3, 0, "cfg3_m4"),
+            ("cfg4", "m4", 2, 1, M.SHORTCUT_CACHED_COMMUTATOR, "cfg4_m4_shortcut_cached_commutator"))
+    for name, scheme, steps, warmup, shortcuts, key in runs:
+        cfg = W.CONFIGS[name]
         sampler = ClockSampler(torch.cuda.current_device())
-        res = measure_workload(M, W, torch, cfg, scheme, steps, 1, dev, lambda: None, sampler, shortcuts)
+        res = measure_workload(M, W, torch, cfg, scheme, steps, warmup, dev, lambda: None, sampler, shortcuts)
         st = res["stats"]
         roof = roofline_for(cfg, scheme, st, peaks, dmma_tf, res.get("path"))
-        out[key] = {"workload": workload_description(cfg, scheme), "steps": steps, "warmup": 1,
-                                 "shortcut": ("beyond-paper shortcut, NOT the mandated path: [H0,H1] cached at create, no GEMM per "
-                                              "step (SURVEY 8f-4)") if shortcuts else None,
-                                 "value": steps / res["seconds"], "unit": UNIT, "ms_per_step": res["seconds"] / steps * 1e3,
-                                 "matvecs": st["total_matvecs"], "seconds_leja": st["seconds_leja"],
-                                 "seconds_commutator": st["seconds_commutator"], "gpu_launches": st["kernel_launches"],
-                                 "clocks": res["clocks"], "roofline": roof, "psi_norm_after": res["norm"]}
+        out[key] = {"workload": workload_description(cfg, scheme), "steps": steps, "warmup": warmup,
+                    "shortcut": ("beyond-paper shortcut, NOT the mandated path: [H0,H1] cached at create, no GEMM per "
+                                 "step (SURVEY 8f-4)") if shortcuts else None,
+                    "value": steps / res["seconds"], "unit": UNIT, "ms_per_step": res["seconds"] / steps * 1e3,
+                    "matvecs": st["total_matvecs"], "seconds_leja": st["seconds_leja"],
+                    "seconds_commutator": st["seconds_commutator"], "gpu_launches": st["kernel_launches"],
+                    "clocks": res["clocks"], "roofline": roof, "psi_norm_after": res["norm"]}
         res["inputs"] = None
         del res
         torch.cuda.empty_cache()
