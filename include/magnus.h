@@ -94,6 +94,22 @@ typedef struct magnus_options {
  * recomputes A2 A1 and A1 A2 every step, P:262 l.6-7; the CSR path always caches [H0, H1], row S0). */
 #define MAGNUS_SHORTCUT_CACHED_COMMUTATOR 1
 
+/* Shortcut (SURVEY 8f-4 "matrix-free XXZ apply", reported separately from the mandated CSR path): the periodic
+ * XXZ chain in a transverse field -- the structure of the paper's Example 2 and of BASELINE configs
+ * 1, 3, 5 -- described by its couplings instead of by matrices:
+ *   H0 = sum over the N periodic nearest-neighbour bonds of  jxy (sx sx + sy sy) + jz sz sz,   H1 = hx sum_i sx_i,
+ * n = 2^nspins, sz basis, site j on bit nspins - j (the layout of workloads/xxz.py).  magnus_create_xxz returns a
+ * handle for magnus_step / magnus_integrate / magnus_describe / magnus_destroy whose fused Leja iteration
+ * recomputes the matrix entries from the row bits and moves vector bytes only; the Gershgorin bounds come from
+ * their closed form.  Commutator-free schemes only (MAGNUS_CF4, MAGNUS_M2, MAGNUS_CF4_3; others: MAGNUS_EINVAL);
+ * 3 <= nspins <= 30.  Results agree with the CSR path on the same model to rounding (different summation order),
+ * iteration counts are equal. */
+typedef struct magnus_xxz_model {
+  int32_t nspins;
+  int32_t reserved;
+  double jxy, jz, hx;
+} magnus_xxz_model;
+
 /* What one exponential did (reading c4-c7). */
 typedef struct magnus_expmv_info {
   int32_t iters;       /* mat-vecs used, summed over sub-steps */
@@ -237,6 +253,9 @@ int magnus_omega_dense(int64_t n, const void* H0, int64_t ld0, const void* H1, i
 int magnus_commutator_csr(const magnus_matrix* A, const magnus_matrix* B, int64_t cap_nnz,
                           int64_t* nnz_out, int32_t* row_ptr_out, int32_t* col_idx_out,
                           void* values_out, void* stream);
+
+int magnus_create_xxz(magnus_handle* out, const magnus_xxz_model* model, magnus_drive_fn f, void* user, int scheme,
+                      const magnus_options* opt);
 
 /* What the handle will run for the fused Leja iteration (row S6) and what that kernel moves per launch.
  * Measurement support (bench.py reports the roofline against THESE bytes: "never count bytes a

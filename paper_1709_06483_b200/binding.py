@@ -63,10 +63,15 @@ class PathInfo(C.Structure):
                 ("entries", C.c_int64)]
 
 
+class XxzModel(C.Structure):
+    _fields_ = [("nspins", C.c_int32), ("reserved", C.c_int32), ("jxy", C.c_double), ("jz", C.c_double),
+                ("hx", C.c_double)]
+
+
 DRIVE = C.CFUNCTYPE(C.c_double, C.c_double, C.c_void_p)
 
 EXPORTS = [
-    "magnus_create", "magnus_destroy", "magnus_describe", "leja_expmv", "magnus_step", "magnus_integrate", "magnus_integrate_host",
+    "magnus_create", "magnus_create_xxz", "magnus_destroy", "magnus_describe", "leja_expmv", "magnus_step", "magnus_integrate", "magnus_integrate_host",
     "magnus_gershgorin", "magnus_leja_iteration", "magnus_zgemm", "magnus_commutator_dense", "magnus_commutator_csr", "magnus_omega_dense",
     "magnus_fp64_peaks", "magnus_host_leja_points", "magnus_host_divided_differences", "magnus_host_snap_interval",
     "magnus_host_step_coefficients", "magnus_strerror", "magnus_last_error", "magnus_version",
@@ -90,6 +95,8 @@ def lib():
         L.magnus_create.argtypes = [C.POINTER(C.c_void_p), C.POINTER(MatrixStruct), C.POINTER(MatrixStruct), DRIVE,
                                     C.c_void_p, C.c_int, C.POINTER(Options)]
         L.magnus_destroy.argtypes = [C.c_void_p]
+        L.magnus_create_xxz.argtypes = [C.POINTER(C.c_void_p), C.POINTER(XxzModel), DRIVE, C.c_void_p, C.c_int,
+                                        C.POINTER(Options)]
         L.magnus_describe.argtypes = [C.c_void_p, C.POINTER(PathInfo)]
         L.leja_expmv.argtypes = [C.POINTER(MatrixStruct), C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_void_p,
                                  C.POINTER(ExpmvInfo)]
@@ -212,6 +219,20 @@ class Handle:
         _check(lib().magnus_create(C.byref(self._h), self.H0.ref(), self.H1.ref(), self._cb, None, self.scheme,
                                    C.byref(self._opt)))
 
+    @classmethod
+    def xxz(cls, nspins: int, jxy: float, jz: float, hx: float, f: Callable[[float], float], scheme, **opts) -> "Handle":
+        """Shortcut handle: matrix-free periodic XXZ chain (magnus_create_xxz); commutator-free schemes only."""
+        self = cls.__new__(cls)
+        self.H0 = self.H1 = None
+        self._cb = _drive(f)
+        self.scheme = SCHEMES[scheme] if isinstance(scheme, str) else int(scheme)
+        self._opt = _options(**opts)
+        self._h = C.c_void_p()
+        model = XxzModel(int(nspins), 0, float(jxy), float(jz), float(hx))
+        _check(lib().magnus_create_xxz(C.byref(self._h), C.byref(model), self._cb, None, self.scheme,
+                                       C.byref(self._opt)))
+        return self
+
     def step(self, t: float, tau: float, psi) -> List[dict]:
         info = StepInfo()
         _check(lib().magnus_step(self._h, t, tau, _ptr(psi), C.byref(info)))
@@ -257,6 +278,10 @@ class Handle:
 
 def magnus_create(H0, H1, f, scheme, **opts) -> Handle:
     return Handle(H0, H1, f, scheme, **opts)
+
+
+def magnus_create_xxz(nspins: int, jxy: float, jz: float, hx: float, f, scheme, **opts) -> Handle:
+    return Handle.xxz(nspins, jxy, jz, hx, f, scheme, **opts)
 
 
 def magnus_step(handle: Handle, t: float, tau: float, psi) -> List[dict]:

@@ -81,6 +81,8 @@ struct OpRef {
   bool dense;
   CsrOp csr;
   DenseOp dns;
+  bool xxz = false;     // matrix-free XXZ chain (shortcut): csr and dns unused
+  XxzOp xx;
 };
 
 static int read_interval(int nblk, Workspace* ws, cudaStream_t st, double* a, double* b) {
@@ -100,6 +102,7 @@ static int op_interval(const OpRef& op, Workspace* ws, cudaStream_t st, double* 
 
 static int launch_iter(const OpRef& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma, double shift,
                        cplx dk, double abs_dk, double tol, Workspace* ws, cudaStream_t st) {
+  if (op.xxz) return launch_xxz_leja_iter(op.xx, w_in, w_out, p, inv_gamma, shift, dk, abs_dk, tol, ws, st);
   return op.dense ? launch_dense_leja_iter(op.dns, w_in, w_out, p, inv_gamma, shift, dk, abs_dk, tol, ws, st)
                   : launch_csr_leja_iter(op.csr, w_in, w_out, p, inv_gamma, shift, dk, abs_dk, tol, ws, st);
 }
@@ -145,7 +148,7 @@ struct LejaTable {
 // ---------------------------------------------------------------------------
 static int expmv_on_interval(const OpRef& op, double a_raw, double b_raw, const cplx* v_in, cplx* v_out, double h,
                              const LejaParams& prm, Workspace* ws, cudaStream_t st, magnus_expmv_info* info) {
-  const int64_t n = op.dense ? op.dns.n : op.csr.n;
+  const int64_t n = op.xxz ? (int64_t)1 << op.xx.nspins : op.dense ? op.dns.n : op.csr.n;
   double a = a_raw, b = b_raw;
   if (!std::isfinite(a) || !std::isfinite(b)) {
     set_error("Gershgorin interval is not finite (NaN/Inf in the matrix?)");
@@ -178,8 +181,8 @@ static int expmv_on_interval(const OpRef& op, double a_raw, double b_raw, const 
   const double inv_gamma = 1.0 / gamma, c_over_gamma = c / gamma;
   const cplx phase = make_double2(std::cos(hs * c), -std::sin(hs * c));
   float ms = 0.f;
-  const bool small_csr = !op.dense && n <= kSmallSweepMaxN && ws->csr_kernel == 0;
-  const bool mid_dense = op.dense && dense_sweep_supported(n) && op.dns.ld == n && ws->csr_kernel == 0;
+  const bool small_csr = !op.xxz && !op.dense && n <= kSmallSweepMaxN && ws->csr_kernel == 0;
+  const bool mid_dense = !op.xxz && op.dense && dense_sweep_supported(n) && op.dns.ld == n && ws->csr_kernel == 0;
   if (small_csr || mid_dense) {
     // small CSR / medium dense problem: each sub-step sweep is ONE launch (kernels_csr_small.cu,
     // kernels_dense_sweep.cu) on an already assembled operator; the table first covers `have` terms and is
@@ -292,6 +295,8 @@ struct magnus_context {
   int format = 0;
   int shortcuts = 0;
   bool cached_p0 = false;      // dense M4 shortcut: h->P holds P0 = H0 H1
+  bool is_xxz = false;         // matrix-free XXZ shortcut: no matrices, format is MAGNUS_CSR only nominally
+  magnus_xxz_model xxz_model;
   int64_t n = 0;
   magnus_matrix H0, H1;
   magnus_drive_fn f = nullptr;
@@ -434,6 +439,7 @@ static int step_specs(magnus_context* h, double t, double tau, ExpSpec* out) {
 }
 
 static bool plan_supported(const magnus_context* h) {
+  if (h->is_xxz) return false;
   if (h->format == MAGNUS_CSR) return h->n <= kSmallSweepMaxN && h->ws.csr_kernel == 0;
   // dense: the commutator-free schemes (M = H0 + g H1 per exponential); M4 / M6 build Omega_H per step
   return h->scheme != MAGNUS_M4 && h->scheme != MAGNUS_M6 && dense_sweep_supported(h->n) && h->ws.csr_kernel == 0;
@@ -647,7 +653,15 @@ static int magnus_step_unplanned(magnus_context* h, double t, double tau, cplx* 
   for (int e = 0; e < n_exp && rc == MAGNUS_OK; ++e) {
     OpRef op;
     double a = 0.0, b = 0.0;
-    if (h->format == MAGNUS_CSR) {
+    if (h->is_xxz) {   // S2, S3 without a matrix: entries from the row bits, bounds from their closed form
+      op.dense = false;
+      op.xxz = true;
+      op.xx.nspins = h->xxz_model.nspins;
+      op.xx.jz = h->xxz_model.jz;
+      op.xx.apair = 2.0 * h->xxz_model.jxy;
+      op.xx.asingle = coef[e] * h->xxz_model.hx;
+      xxz_gershgorin(op.xx, &a, &b);
+    } else if (h->format == MAGNUS_CSR) {
       op.dense = false;
       op.csr.n = h->n;
       if (h->scheme == MAGNUS_M4) {
@@ -821,7 +835,12 @@ int magnus_describe(magnus_handle h, magnus_path_info* out) {
   std::memset(out, 0, sizeof *out);
   const int64_t n = h->n;
   const char* name = "dense_leja_iter_kernel";
-  if (h->format == MAGNUS_DENSE) {
+  if (h->is_xxz) {
+    name = "xxz_leja_iter_kernel";
+    out->bytes_per_iteration = 64 * n;          // w gather (16 n ideal), w+ write, p read + write: no matrix bytes
+    const int64_t N = h->xxz_model.nspins;
+    out->csr_bytes_per_iteration = 20 * (n * (3 * N + 2) / 2) + 4 * (n + 1) * 2 + 64 * n;
+  } else if (h->format == MAGNUS_DENSE) {
     out->bytes_per_iteration = 16 * n * n + 64 * n;
     if (plan_supported(h)) name = "dense_leja_sweep_kernel";
   } else {
@@ -997,6 +1016,38 @@ int magnus_create(magnus_handle* out, const magnus_matrix* H0, const magnus_matr
     }
   }
   if (cudaStreamSynchronize(h->stream) != cudaSuccess) { magnus_destroy(h); return MAGNUS_ECUDA; }
+  *out = h;
+  return MAGNUS_OK;
+}
+
+int magnus_create_xxz(magnus_handle* out, const magnus_xxz_model* model, magnus_drive_fn f, void* user, int scheme,
+                      const magnus_options* opt) {
+  if (!out) { set_error("out is NULL"); return MAGNUS_EINVAL; }
+  *out = nullptr;
+  if (!model || !f) { set_error("magnus_create_xxz: NULL model or f"); return MAGNUS_EINVAL; }
+  if (model->nspins < 3 || model->nspins > 30) { set_error("magnus_create_xxz: nspins must be in [3, 30]"); return MAGNUS_EINVAL; }
+  if (scheme != MAGNUS_CF4 && scheme != MAGNUS_M2 && scheme != MAGNUS_CF4_3) {
+    set_error("magnus_create_xxz: commutator-free schemes only (got %d)", scheme);
+    return MAGNUS_EINVAL;
+  }
+  int rc = require_device();
+  if (rc) return rc;
+  magnus_context* h = new (std::nothrow) magnus_context();
+  if (!h) return MAGNUS_ENOMEM;
+  h->scheme = scheme;
+  h->format = MAGNUS_CSR;
+  h->is_xxz = true;
+  h->xxz_model = *model;
+  h->n = (int64_t)1 << model->nspins;
+  std::memset(&h->H0, 0, sizeof h->H0);
+  std::memset(&h->H1, 0, sizeof h->H1);
+  h->f = f;
+  h->user = user;
+  default_params(opt, &h->prm, &h->stream, &h->ws.csr_kernel, &h->shortcuts);
+  rc = workspace_alloc(&h->ws, h->n);
+  h->ws.csr_kernel = 1;       // no whole-sweep kernels on this path
+  h->ws.time_leja = true;
+  if (rc) { set_error("workspace allocation failed (n=%lld)", (long long)h->n); magnus_destroy(h); return rc; }
   *out = h;
   return MAGNUS_OK;
 }

@@ -8,12 +8,12 @@
 //   out = e^{-i (h/s) c} p_k                                                                          (c7)
 // Layout: CTA c owns the contiguous row slice [c n/8, (c+1) n/8); SS_G lanes share a row; p of the
 // slice lives in shared memory.  EVERY CTA holds the whole vector w in its shared memory (ping-pong,
-// 2 x 16 n bytes): after computing its slice of the new w a CTA passes one cluster barrier and pulls
-// the other seven slices through distributed shared memory, so the gathers of the next iteration are
-// local shared-memory reads.  The CTA's slice of the CSR terms is copied to shared memory once per
+// 2 x 16 n bytes): a CTA PUSHES every new w entry of its slice into all eight copies through distributed
+// shared memory as it is computed (fire-and-forget remote stores that overlap the rest of the row loop),
+// so after the one cluster barrier per iteration the gathers are local shared-memory reads and nothing is pulled.  The CTA's slice of the CSR terms is copied to shared memory once per
 // sweep when it fits (cluster barriers flush L1, so global reads would pay an L2 round trip per
 // dependent load in every iteration); otherwise it is read in place.  The per-CTA partial norms are
-// pulled the same way; every CTA sums the eight partials in the same order and takes the same stop
+// pushed the same way; every CTA sums the eight partials in the same order and takes the same stop
 // decision.  The divided differences and Leja points arrive as a kernel argument (3 KB,
 // __grid_constant__).  Deterministic: fixed lane->entry map, fixed trees.
 // Measured (clock64, CFG1): about 10,000 cycles per iteration -- row slice 4,000, block reduction
@@ -73,13 +73,21 @@ __global__ void __cluster_dims__(SS_CTAS, 1, 1) __launch_bounds__(SS_THREADS, 1)
                                 const LejaStatus* gate) {
   extern __shared__ __align__(16) unsigned char ss_smem[];
   __shared__ double sa[SS_THREADS / 32], sb[SS_THREADS / 32];
-  __shared__ double part[2][2];                     // [iteration parity](sw, sp) of this CTA, read by the others
+  __shared__ double part[2][SS_CTAS][2];            // [iteration parity][CTA](sw, sp): every CTA writes its entry in all copies
+  __shared__ double s_norm0;
   __shared__ double s_l[kMaxDegree + 1];            // Leja points (c2)
+  __shared__ double s_absd[kMaxDegree + 1];         // |d_k| of the current job
   cg::cluster_group cluster = cg::this_cluster();
   const int rank = (int)cluster.block_rank();
   if (status->pad) return;                          // an earlier sub-step did not converge (cluster-uniform)
   if (gate && !gate->done) return;                  // an earlier job of the plan failed: psi stays as that job found it
   cplx* wbuf[2] = {reinterpret_cast<cplx*>(ss_smem), reinterpret_cast<cplx*>(ss_smem) + kSmallSweepMaxN};
+  // element i of buffer b in EVERY CTA of the cluster (own included) <- x
+  auto push_w = [&](int b, int i, cplx x) {
+    cplx* local = wbuf[b] + i;
+#pragma unroll
+    for (int c = 0; c < SS_CTAS; ++c) *cluster.map_shared_rank(local, c) = x;
+  };
   const int tid = threadIdx.x, grp = tid / SS_G, sub = tid % SS_G;
   const int n = (int)op.n;
   const int per = (n + SS_CTAS - 1) / SS_CTAS;
@@ -129,12 +137,13 @@ __global__ void __cluster_dims__(SS_CTAS, 1, 1) __launch_bounds__(SS_THREADS, 1)
       s0 += x.x * x.x + x.y * x.y;
     }
     block_reduce_sum2_ss(s0, s1, sa, sb);
-    if (tid == 0) part[0][0] = s0;
+    if (tid == 0) s_norm0 = s0;
+    for (int k = tid; k <= m_max; k += SS_THREADS) s_absd[k] = hypot(J.d[k].x, J.d[k].y);
     __syncthreads();
-    s0 = part[0][0];
+    s0 = s_norm0;
     const cplx d0 = J.d[0];
     for (int r = r0 + tid; r < r1; r += SS_THREADS) prow[r - r0] = cmul(d0, wbuf[cur][r]);
-    double e_prev = hypot(d0.x, d0.y) * sqrt(s0);
+    double e_prev = s_absd[0] * sqrt(s0);
     double err = 0.0, sw = 0.0, sp = 0.0;
     int k = 0;
     bool done = false;
@@ -183,37 +192,25 @@ __global__ void __cluster_dims__(SS_CTAS, 1, 1) __launch_bounds__(SS_THREADS, 1)
           prow[row - r0] = pi;
           bw += wn.x * wn.x + wn.y * wn.y;
           bp += pi.x * pi.x + pi.y * pi.y;
-          wbuf[cur ^ 1][row] = wn;                    // own slice, own copy; the other CTAs pull it after the barrier
+          push_w(cur ^ 1, row, wn);
         }
       }
       block_reduce_sum2_ss(bw, bp, sa, sb);
-      if (tid == 0) {
-        part[k & 1][0] = bw;
-        part[k & 1][1] = bp;
+      if (tid < SS_CTAS) {                            // thread c pushes this CTA's partials into CTA c's copy
+        const double bw0 = __shfl_sync(0xffu, bw, 0), bp0 = __shfl_sync(0xffu, bp, 0);
+        double* remote = cluster.map_shared_rank(&part[k & 1][rank][0], tid);
+        remote[0] = bw0;
+        remote[1] = bp0;
       }
-      cluster.sync();                                 // every CTA's slice of the new w and its partials are written
-      // pull the other CTAs' slices into the local copy through distributed shared memory (independent
-      // 16-byte loads, all in flight at once) and their partial norms
-      for (int i = tid; i < n; i += SS_THREADS) {
-        const int owner = i / per;
-        if (owner != rank) wbuf[cur ^ 1][i] = cluster.map_shared_rank(wbuf[cur ^ 1], owner)[i];
-      }
-      double pw[SS_CTAS], pp[SS_CTAS];
-#pragma unroll
-      for (int c = 0; c < SS_CTAS; ++c) {
-        const double* remote = cluster.map_shared_rank(&part[k & 1][0], c);
-        pw[c] = remote[0];
-        pp[c] = remote[1];
-      }
+      cluster.sync();                                 // every CTA's slice of the new w and its partials have arrived
       sw = 0.0;
       sp = 0.0;
 #pragma unroll
       for (int c = 0; c < SS_CTAS; ++c) {             // same order in every CTA: same decision
-        sw += pw[c];
-        sp += pp[c];
+        sw += part[k & 1][c][0];
+        sp += part[k & 1][c][1];
       }
-      __syncthreads();                                // local copy of w complete before the next gathers
-      const double e_k = hypot(dk.x, dk.y) * sqrt(sw);   // S7
+      const double e_k = s_absd[k] * sqrt(sw);        // S7
       err = e_k + e_prev;
       e_prev = e_k;
       done = err <= tol * sqrt(sp);
@@ -231,26 +228,21 @@ __global__ void __cluster_dims__(SS_CTAS, 1, 1) __launch_bounds__(SS_THREADS, 1)
       S->norm_p2 = sp;
     }
     if (!done) break;                                 // cluster-uniform: psi (global) is the state before this job
-    // S8: the result becomes the next job's input.  It goes into the buffer nobody pulls from any more
-    // (remote reads of this iteration target wbuf[cur]); the others fetch it after one barrier.
+    // S8: the result becomes the next job's input: pushed into the buffer that was this iteration's input (nobody
+    // reads it any more: every CTA is past the last barrier), visible everywhere after one more barrier.
     const cplx phase = J.phase;
     const bool more = e + 1 < njobs;
     for (int r = r0 + tid; r < r1; r += SS_THREADS) {
       const cplx o = cmul(phase, prow[r - r0]);
       out[r] = o;
-      if (more) wbuf[cur ^ 1][r] = o;
+      if (more) push_w(cur ^ 1, r, o);
     }
     if (more) {
       cluster.sync();
-      for (int i = tid; i < n; i += SS_THREADS) {
-        const int owner = i / per;
-        if (owner != rank) wbuf[cur ^ 1][i] = cluster.map_shared_rank(wbuf[cur ^ 1], owner)[i];
-      }
       cur ^= 1;
-      __syncthreads();
     }
   }
-  cluster.sync();                                   // no CTA leaves while its shared memory may still be read
+  cluster.sync();                                   // no CTA leaves while its shared memory may still be written
 }
 
 }  // namespace

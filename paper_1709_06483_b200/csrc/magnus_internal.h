@@ -64,6 +64,13 @@ struct DenseOp {
   int64_t ld;
   const cplx* M;
 };
+// Matrix-free periodic XXZ chain (shortcut, kernels_xxz.cu): M = H0 + g H1 with the entries recomputed from the row bits
+struct XxzOp {
+  int nspins;
+  double jz;        // diagonal jz (N - 2k)
+  double apair;     // 2 jxy: amplitude of an antiparallel pair flip
+  double asingle;   // g hx: amplitude of a single flip
+};
 
 // Device-resident control block of one exponential (row S7): written by the
 // finalize kernel after every iteration, read by the next iteration kernel
@@ -207,6 +214,11 @@ inline int slice_layout_kind(int csr_kernel) {
 void slice_layout_free(SliceLayout* L);
 int launch_csr_leja_iter_slice(const CsrOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma, double shift,
                                cplx dk, double abs_dk, double tol, Workspace* ws, cudaStream_t st);
+
+// ---- kernels_xxz.cu ---------------------------------------------------------
+int launch_xxz_leja_iter(const XxzOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma, double shift,
+                         cplx dk, double abs_dk, double tol, Workspace* ws, cudaStream_t st);
+void xxz_gershgorin(const XxzOp& op, double* a, double* b);   // host, closed form
 
 // ---- kernels_csr_small.cu ---------------------------------------------------
 // one sub-step sweep (S5-S8) in one launch; on success status->done = 1, status->k = iterations and out is

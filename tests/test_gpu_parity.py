@@ -648,3 +648,49 @@ def test_planned_batch_longer_than_the_plan_capacity(M, oracle):
     psi, st, ref, riters = run_config(M, oracle, cfg, "cf4")
     assert st["n_exp"] == 3000 and np.array_equal(st["iters"], riters)
     assert relerr(psi, ref) <= 1e-9
+
+
+# ------------------------------------------------------------------ shortcut: matrix-free XXZ chain
+def xxz_with_couplings(N, jxy, jz, hx):
+    """The generator's H0, H1 rescaled to couplings (jxy, jz, hx): H0's diagonal is 0.5 (N - 2k), its off-diagonal 2."""
+    H0, H1 = xxz.xxz_h0(N), xxz.xxz_h1(N)
+    rows = torch.repeat_interleave(torch.arange(H0.n), (H0.row_ptr[1:] - H0.row_ptr[:-1]).long())
+    diag = H0.col_idx.long() == rows
+    v0 = torch.where(diag, H0.values * (jz / 0.5), H0.values * jxy)
+    return xxz.CSR(H0.n, H0.row_ptr, H0.col_idx, v0), xxz.CSR(H1.n, H1.row_ptr, H1.col_idx, H1.values * hx)
+
+
+@pytest.mark.parametrize("scheme", ["cf4", "cf4:3"])
+@pytest.mark.parametrize("N,jxy,jz,hx,tau,nsteps", [(3, 1.0, 0.5, 1.0, 0.05, 3), (4, 1.0, 0.5, 1.0, 0.05, 3),
+                                                    (5, -0.8, 0.4, 0.6, 0.05, 3), (6, 1.0, 0.5, 1.0, 0.05, 3),
+                                                    (7, 0.7, -0.3, 1.3, 0.04, 3), (10, 1.0, 0.5, 1.0, 0.01, 10),
+                                                    (13, 0.7, -0.3, 1.3, 0.03, 3), (16, 1.0, 0.5, 1.0, 0.05, 2)])
+def test_shortcut_matrix_free_xxz(M, oracle, scheme, N, jxy, jz, hx, tau, nsteps):
+    """`magnus_create_xxz`: the chain described by its couplings, no matrix in memory.  Against the oracle on the
+    CSR matrices of the same model (identical counts, psi <= 1e-9) and against the library's own CSR path
+    (psi <= 1e-12: same method, another summation order).  N <= 5: everything inside one warp (shuffles only)."""
+    H0, H1 = xxz_with_couplings(N, jxy, jz, hx)
+    psi0 = torch.from_numpy(rand_vec(1 << N, 31 + N))
+    f = xxz.f_cos2t
+    ref, riters = oracle.magnus_integrate(oracle.CsrHost.of(H0), oracle.CsrHost.of(H1), f, scheme, 0.1, 0.1 + tau * nsteps,
+                                          nsteps, psi0.numpy(), 1e-12)
+    psi = psi0.to(DEV).clone()
+    with M.magnus_create_xxz(N, jxy, jz, hx, f, scheme, tol=1e-12) as h:
+        d = h.describe()
+        assert d["leja_kernel"] == "xxz_leja_iter_kernel" and d["bytes_per_iteration"] == 64 * (1 << N)
+        st = h.integrate(0.1, 0.1 + tau * nsteps, nsteps, psi)
+    assert np.array_equal(st["iters"], riters)
+    assert relerr(host(psi), ref) <= 1e-9 and abs(np.linalg.norm(host(psi)) - 1) < 1e-10
+    psi2 = psi0.to(DEV).clone()
+    with M.magnus_create(H0.to(DEV), H1.to(DEV), f, scheme, tol=1e-12) as h:
+        st2 = h.integrate(0.1, 0.1 + tau * nsteps, nsteps, psi2)
+    assert np.array_equal(st["iters"], st2["iters"]) and relerr(host(psi), host(psi2)) <= 1e-12
+
+
+def test_shortcut_matrix_free_xxz_refuses_commutator_schemes(M):
+    for scheme in ("m4", "m6"):
+        with pytest.raises(M.MagnusError) as e:
+            M.magnus_create_xxz(10, 1.0, 0.5, 1.0, xxz.f_cos2t, scheme)
+        assert e.value.code == -1
+    with pytest.raises(M.MagnusError):
+        M.magnus_create_xxz(2, 1.0, 0.5, 1.0, xxz.f_cos2t, "cf4")
