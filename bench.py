@@ -391,6 +391,7 @@ def measure_extra(M, W, torch, dev, peaks, dmma_tf):
             ("cfg2", "cf4", 50, 10, 0, "cfg2_cf4"), ("cfg2", "m4", 20, 3, 0, "cfg2_m4"),
             ("cfg3", "cf4", 10, 3, 0, "cfg3_cf4"), ("cfg3", "m4", 10, 3, 0, "cfg3_m4"),
             ("cfg4", "m4", 2, 1, M.SHORTCUT_CACHED_COMMUTATOR, "cfg4_m4_shortcut_cached_commutator"),
+            ("cfg4", "cf4", 2, 1, M.SHORTCUT_TIGHT_INTERVAL, "cfg4_cf4_shortcut_tight_interval"),
             ("cfg5", "cf4", 5, 3, XXZ_MATRIX_FREE, "cfg5_cf4_shortcut_matrix_free"),
             ("cfg3", "cf4", 10, 3, XXZ_MATRIX_FREE, "cfg3_cf4_shortcut_matrix_free"))
     for name, scheme, steps, warmup, shortcuts, key in runs:
@@ -402,10 +403,14 @@ def measure_extra(M, W, torch, dev, peaks, dmma_tf):
         out[key] = {"workload": workload_description(cfg, scheme), "steps": steps, "warmup": warmup,
                     "shortcut": ("beyond-paper shortcut, NOT the mandated path: the chain is given by its couplings, "
                                  "no matrix in memory (magnus_create_xxz, SURVEY 8f-4)") if shortcuts == XXZ_MATRIX_FREE else
+                                ("beyond-paper shortcut, NOT the mandated path: spectral interval from 8 Lanczos steps per "
+                                 "exponential instead of Gershgorin (SURVEY 8f-4); its mat-vecs are in lanczos_matvecs, not "
+                                 "in matvecs") if shortcuts == M.SHORTCUT_TIGHT_INTERVAL else
                                 ("beyond-paper shortcut, NOT the mandated path: [H0,H1] cached at create, no GEMM per "
                                  "step (SURVEY 8f-4)") if shortcuts else None,
                     "value": steps / res["seconds"], "unit": UNIT, "ms_per_step": res["seconds"] / steps * 1e3,
-                    "matvecs": st["total_matvecs"], "seconds_leja": st["seconds_leja"],
+                    "matvecs": st["total_matvecs"], "lanczos_matvecs": st.get("lanczos_matvecs", 0),
+                    "seconds_leja": st["seconds_leja"],
                     "seconds_commutator": st["seconds_commutator"], "gpu_launches": st["kernel_launches"],
                     "clocks": res["clocks"], "roofline": roof, "psi_norm_after": res["norm"]}
         res["inputs"] = None

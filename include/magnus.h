@@ -85,7 +85,8 @@ typedef struct magnus_options {
                           16-byte aligned value and index arrays, else the row-block kernel runs); values >= 1000
                           select tuning variants of these kernels (see the kernel sources) */
   int32_t shortcuts;   /* bit mask of beyond-paper shortcuts, default 0 = the mandated path only:
-                          MAGNUS_SHORTCUT_CACHED_COMMUTATOR (dense M4) */
+                          MAGNUS_SHORTCUT_CACHED_COMMUTATOR (dense M4), MAGNUS_SHORTCUT_TIGHT_INTERVAL */
+  int32_t lanczos_steps; /* MAGNUS_SHORTCUT_TIGHT_INTERVAL: Lanczos steps per exponential; default 8, at most 64 */
 } magnus_options;
 
 /* Shortcut (reported separately from the mandated path): for H(t) = H0 + f(t) H1 the commutator of
@@ -93,6 +94,15 @@ typedef struct magnus_options {
  * magnus_create and a step assembles Omega_H = H0 + fbar H1 - i kappa (P0 - P0^H) without any GEMM (the paper
  * recomputes A2 A1 and A1 A2 every step, P:262 l.6-7; the CSR path always caches [H0, H1], row S0). */
 #define MAGNUS_SHORTCUT_CACHED_COMMUTATOR 1
+
+/* Shortcut (SURVEY 8f-4 "tighter spectral interval", reported separately from the mandated path): P:190 only asks
+ * for "an estimate on the spectrum"; NS fixes Gershgorin, which over-estimates the radius of a dense random Hermitian
+ * matrix 20x to 57x and so costs 1.6-3x more Leja iterations.  With this bit the interval of every exponential of
+ * magnus_step / magnus_integrate comes from lanczos_steps steps of the Lanczos process on the exponentiated matrix,
+ * started at the current psi:  [theta_min(T) - beta_m, theta_max(T) + beta_m]  (extreme Ritz values widened by the
+ * norm of the last residual), then snapped as usual (reading ti).  Costs lanczos_steps extra mat-vecs per
+ * exponential (magnus_stats.lanczos_matvecs); the interval now depends on psi, so steps are not planned ahead. */
+#define MAGNUS_SHORTCUT_TIGHT_INTERVAL 2
 
 /* Shortcut (SURVEY 8f-4 "matrix-free XXZ apply", reported separately from the mandated CSR path): the periodic
  * XXZ chain in a transverse field -- the structure of the paper's Example 2 and of BASELINE configs
@@ -136,6 +146,7 @@ typedef struct magnus_stats {
   double seconds_leja;     /* CUDA-event time spent inside fused Leja-iteration kernels (init..stop) */
   double seconds_commutator; /* CUDA-event time inside the dense commutator GEMM (M4 dense), else 0 */
   int64_t kernel_launches; /* kernels this call enqueued */
+  int64_t lanczos_matvecs; /* MAGNUS_SHORTCUT_TIGHT_INTERVAL: mat-vecs spent on interval estimates (not in total_matvecs) */
 } magnus_stats;
 
 typedef struct magnus_context* magnus_handle;

@@ -18,6 +18,7 @@
 //   Leja/Newton P:169-186 (formula and code fragment)               -> leja_expmv
 //   early stop  P:188, P:229-231 (reading c6)                       -> leja_expmv
 //   spectrum    P:190 (estimate "from the matrix"; Gershgorin, c4)  -> gershgorin_*
+//               shortcut beside it (reading ti): Lanczos interval     -> lanczos_interval
 //   Leja points P:169 ("see [11]"; reading c2)                      -> leja_points
 //   d_i         P:171 (definition; reading c3: __float128 table)    -> divided_differences
 //
@@ -297,6 +298,88 @@ struct oracle_expmv_info {
 namespace {
 
 // ---------------------------------------------------------------------------
+// Shortcut "tight spectral interval" (P:190 leaves the estimate of the spectrum open, NS fixes
+// Gershgorin for the mandated path; this is the option beside it, reading ti in DESIGN.md section 3).
+// m steps of the Lanczos process on the Hermitian M, started at the vector v that is about to be propagated:
+//   q_1 = v / ||v||;   for j = 1..m:   u = M q_j - beta_{j-1} q_{j-1};   alpha_j = Re(q_j^H u);
+//                                      r = u - alpha_j q_j;   beta_j = ||r||;   q_{j+1} = r / beta_j
+// (stopped early -- an invariant subspace -- when beta_j <= 1e-12 * max_i max(|alpha_i|, beta_i)).
+// T = tridiag(alpha_1..alpha_m; beta_1..beta_{m-1}); its extreme eigenvalues theta_min, theta_max (Ritz values: inside
+// the spectrum of M) are widened by the norm of the last residual:  [theta_min - beta_m, theta_max + beta_m].
+// The eigenvalues of the small T come from cyclic Jacobi rotations on the dense m x m matrix.
+// ---------------------------------------------------------------------------
+int g_lanczos_steps = 0;   // 0: Gershgorin (the mandated path); m > 0: the interval of every leja_expmv call from m Lanczos steps
+
+void jacobi_eigenvalues(std::vector<double>& A, int m, std::vector<double>& ev) {   // A: m x m symmetric, row-major
+  for (int sweep = 0; sweep < 60; ++sweep) {
+    double off = 0.0;
+    for (int p = 0; p < m; ++p)
+      for (int q = p + 1; q < m; ++q) off += A[p * m + q] * A[p * m + q];
+    if (off == 0.0) break;
+    for (int p = 0; p < m; ++p)
+      for (int q = p + 1; q < m; ++q) {
+        const double apq = A[p * m + q];
+        if (apq == 0.0) continue;
+        const double tau = (A[q * m + q] - A[p * m + p]) / (2.0 * apq);
+        const double t = (tau >= 0.0 ? 1.0 : -1.0) / (std::fabs(tau) + std::sqrt(1.0 + tau * tau));
+        const double c = 1.0 / std::sqrt(1.0 + t * t), sn = t * c;
+        for (int k = 0; k < m; ++k) {   // columns p, q
+          const double akp = A[k * m + p], akq = A[k * m + q];
+          A[k * m + p] = c * akp - sn * akq;
+          A[k * m + q] = sn * akp + c * akq;
+        }
+        for (int k = 0; k < m; ++k) {   // rows p, q
+          const double apk = A[p * m + k], aqk = A[q * m + k];
+          A[p * m + k] = c * apk - sn * aqk;
+          A[q * m + k] = sn * apk + c * aqk;
+        }
+      }
+  }
+  ev.resize(m);
+  for (int i = 0; i < m; ++i) ev[i] = A[i * m + i];
+}
+
+// returns the number of Lanczos steps actually taken (0: v = 0, interval left untouched); alpha, beta (nullable): m entries
+int lanczos_interval(const Matrix& M, const cplx* v, int m, double* a, double* b, double* alpha_out, double* beta_out) {
+  const int64_t n = M.n;
+  const double nv = norm2(v, n);
+  if (!(nv > 0.0) || m < 1) return 0;
+  std::vector<cplx> qp(n, cplx(0.0)), q(n), u(n);
+  for (int64_t i = 0; i < n; ++i) q[i] = v[i] / nv;
+  std::vector<double> alpha, beta;
+  double beta_prev = 0.0, scale = 0.0;
+  for (int j = 0; j < m; ++j) {
+    M.matvec(q.data(), u.data());
+    for (int64_t i = 0; i < n; ++i) u[i] -= beta_prev * qp[i];
+    double al = 0.0;
+    for (int64_t i = 0; i < n; ++i) al += (std::conj(q[i]) * u[i]).real();
+    for (int64_t i = 0; i < n; ++i) u[i] -= al * q[i];
+    const double be = norm2(u.data(), n);
+    alpha.push_back(al);
+    beta.push_back(be);
+    scale = std::max(scale, std::max(std::fabs(al), be));
+    if (be <= 1e-12 * scale) break;              // invariant subspace reached: T is exact
+    for (int64_t i = 0; i < n; ++i) { qp[i] = q[i]; q[i] = u[i] / be; }
+    beta_prev = be;
+  }
+  const int k = (int)alpha.size();
+  std::vector<double> T((size_t)k * k, 0.0), ev;
+  for (int i = 0; i < k; ++i) {
+    T[i * k + i] = alpha[i];
+    if (i + 1 < k) T[i * k + i + 1] = T[(i + 1) * k + i] = beta[i];
+  }
+  jacobi_eigenvalues(T, k, ev);
+  const double lo = *std::min_element(ev.begin(), ev.end()), hi = *std::max_element(ev.begin(), ev.end());
+  *a = lo - beta[k - 1];
+  *b = hi + beta[k - 1];
+  for (int i = 0; i < k; ++i) {
+    if (alpha_out) alpha_out[i] = alpha[i];
+    if (beta_out) beta_out[i] = beta[i];
+  }
+  return k;
+}
+
+// ---------------------------------------------------------------------------
 // exp(-i h M) v by Newton interpolation at Leja points (c3-c7).
 //   B = (M - cI)/gamma has its spectrum in [-2,2]; exp(-ihM) = e^{-ihc} exp(-i theta B).
 //   w_0 = v, p_0 = d_0 v;
@@ -309,7 +392,8 @@ int leja_expmv(const Matrix& M, const cplx* v_in, cplx* v_out, double h, double 
   const int64_t n = M.n;
   const std::vector<double>& l = leja_table();
   double a, b;
-  M.gershgorin(&a, &b);
+  if (g_lanczos_steps <= 0 || lanczos_interval(M, v_in, g_lanczos_steps, &a, &b, nullptr, nullptr) == 0)
+    M.gershgorin(&a, &b);
   snap_interval(&a, &b);
   const double c = 0.5 * (a + b);
   const double gamma = 0.25 * (b - a);
@@ -568,6 +652,21 @@ int step_csr(const CsrView& H0, const CsrView& H1, drive_fn f, void* user, int s
 extern "C" {
 
 int oracle_max_degree() { return kMaxDegree; }
+
+// 0 = Gershgorin interval (mandated path); m > 0 = shortcut "tight interval": m Lanczos steps per exponential
+void oracle_set_lanczos_steps(int m) { g_lanczos_steps = m; }
+int oracle_get_lanczos_steps() { return g_lanczos_steps; }
+
+// raw (unsnapped) interval; returns the steps taken; alpha, beta: capacity m
+int oracle_lanczos_interval_dense(int64_t n, const double* M, const double* v, int m, double* ab, double* alpha, double* beta) {
+  return lanczos_interval(DenseView(n, reinterpret_cast<const cplx*>(M)), reinterpret_cast<const cplx*>(v), m, &ab[0], &ab[1],
+                          alpha, beta);
+}
+int oracle_lanczos_interval_csr(int64_t n, const int32_t* rp, const int32_t* ci, const double* val, const double* v, int m,
+                                double* ab, double* alpha, double* beta) {
+  return lanczos_interval(CsrView(n, rp, ci, reinterpret_cast<const cplx*>(val)), reinterpret_cast<const cplx*>(v), m, &ab[0],
+                          &ab[1], alpha, beta);
+}
 
 int oracle_num_threads() {
 #ifdef _OPENMP

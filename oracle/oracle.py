@@ -109,6 +109,35 @@ def gershgorin(M):
     return tuple(raw), tuple(snp)
 
 
+def lanczos_interval(M, v, m: int):
+    """Shortcut "tight interval" (reading ti): raw interval from m Lanczos steps started at v.
+    Returns ((a, b), alpha, beta) with the steps actually taken."""
+    v = _c(v, np.complex128)
+    ab = np.zeros(2); al = np.zeros(m); be = np.zeros(m)
+    if isinstance(M, CsrHost):
+        k = lib().oracle_lanczos_interval_csr(C.c_int64(M.n), *M.args(), _p(v), C.c_int(m), _p(ab), _p(al), _p(be))
+    else:
+        M = _c(M, np.complex128)
+        k = lib().oracle_lanczos_interval_dense(C.c_int64(M.shape[0]), _p(M), _p(v), C.c_int(m), _p(ab), _p(al), _p(be))
+    return (float(ab[0]), float(ab[1])), al[:k].copy(), be[:k].copy()
+
+
+class tight_interval:
+    """Context manager: inside, every leja_expmv / magnus_step / magnus_integrate takes its interval from m
+    Lanczos steps (the shortcut) instead of Gershgorin (the mandated path)."""
+
+    def __init__(self, m: int):
+        self.m = int(m)
+
+    def __enter__(self):
+        self.old = int(lib().oracle_get_lanczos_steps())
+        lib().oracle_set_lanczos_steps(C.c_int(self.m))
+        return self
+
+    def __exit__(self, *exc):
+        lib().oracle_set_lanczos_steps(C.c_int(self.old))
+
+
 def matvec(M, w) -> np.ndarray:
     w = _c(w, np.complex128)
     y = np.empty_like(w)

@@ -36,7 +36,7 @@ class MatrixStruct(C.Structure):
 
 class Options(C.Structure):
     _fields_ = [("tol", C.c_double), ("theta_max", C.c_double), ("m_max", C.c_int32), ("check_hermitian", C.c_int32),
-                ("stream", C.c_void_p), ("csr_kernel", C.c_int32), ("shortcuts", C.c_int32)]
+                ("stream", C.c_void_p), ("csr_kernel", C.c_int32), ("shortcuts", C.c_int32), ("lanczos_steps", C.c_int32)]
 
 
 class ExpmvInfo(C.Structure):
@@ -54,7 +54,7 @@ class StepInfo(C.Structure):
 class Stats(C.Structure):
     _fields_ = [("total_matvecs", C.c_int64), ("n_exp", C.c_int64), ("iters", C.c_void_p), ("iters_cap", C.c_int64),
                 ("seconds_device", C.c_double), ("seconds_leja", C.c_double), ("seconds_commutator", C.c_double),
-                ("kernel_launches", C.c_int64)]
+                ("kernel_launches", C.c_int64), ("lanczos_matvecs", C.c_int64)]
 
 
 class PathInfo(C.Structure):
@@ -192,10 +192,11 @@ def _drive(f: Callable[[float], float]):
 
 
 SHORTCUT_CACHED_COMMUTATOR = 1
+SHORTCUT_TIGHT_INTERVAL = 2
 
 
 def _options(tol=None, theta_max=None, m_max=None, check_hermitian=False, stream=None, csr_kernel=0,
-             shortcuts=0) -> Options:
+             shortcuts=0, lanczos_steps=0) -> Options:
     o = Options()
     o.tol = tol or 0.0
     o.theta_max = theta_max or 0.0
@@ -204,6 +205,7 @@ def _options(tol=None, theta_max=None, m_max=None, check_hermitian=False, stream
     o.stream = _stream_ptr(stream)
     o.csr_kernel = csr_kernel
     o.shortcuts = shortcuts
+    o.lanczos_steps = lanczos_steps
     return o
 
 
@@ -248,7 +250,8 @@ class Handle:
         _check(lib().magnus_integrate(self._h, t0, t_end, nsteps, _ptr(psi), C.byref(st)))
         return {"total_matvecs": int(st.total_matvecs), "n_exp": int(st.n_exp), "iters": iters[:int(st.n_exp)].copy(),
                 "seconds_device": st.seconds_device, "seconds_leja": st.seconds_leja,
-                "seconds_commutator": st.seconds_commutator, "kernel_launches": int(st.kernel_launches)}
+                "seconds_commutator": st.seconds_commutator, "kernel_launches": int(st.kernel_launches),
+                "lanczos_matvecs": int(st.lanczos_matvecs)}
 
     def describe(self) -> dict:
         """The kernel that runs the fused Leja iteration for this handle and its algorithmic bytes per launch."""

@@ -295,6 +295,10 @@ struct magnus_context {
   int format = 0;
   int shortcuts = 0;
   bool cached_p0 = false;      // dense M4 shortcut: h->P holds P0 = H0 H1
+  int lanczos_steps = 8;       // tight-interval shortcut
+  cplx* lz[2] = {nullptr, nullptr};   // ... its Lanczos vectors q_j, q_{j-1}
+  double* lz_scal = nullptr;          // ... and device scalars (norm, beta_prev, alpha[], beta[])
+  int64_t lanczos_matvecs = 0;
   bool is_xxz = false;         // matrix-free XXZ shortcut: no matrices, format is MAGNUS_CSR only nominally
   magnus_xxz_model xxz_model;
   int64_t n = 0;
@@ -439,7 +443,7 @@ static int step_specs(magnus_context* h, double t, double tau, ExpSpec* out) {
 }
 
 static bool plan_supported(const magnus_context* h) {
-  if (h->is_xxz) return false;
+  if (h->is_xxz || (h->shortcuts & MAGNUS_SHORTCUT_TIGHT_INTERVAL)) return false;   // the interval depends on psi
   if (h->format == MAGNUS_CSR) return h->n <= kSmallSweepMaxN && h->ws.csr_kernel == 0;
   // dense: the commutator-free schemes (M = H0 + g H1 per exponential); M4 / M6 build Omega_H per step
   return h->scheme != MAGNUS_M4 && h->scheme != MAGNUS_M6 && dense_sweep_supported(h->n) && h->ws.csr_kernel == 0;
@@ -639,6 +643,55 @@ static int run_planned(magnus_context* h, double t0, double tau, int64_t s0, int
   return rc;
 }
 
+// Shortcut MAGNUS_SHORTCUT_TIGHT_INTERVAL: raw interval of op from Lanczos started at v (kernels_lanczos.cu).
+// Returns kPlanDeclined when v = 0 (the caller keeps the Gershgorin interval).
+static int lanczos_interval(magnus_context* h, const OpRef& op, const cplx* v, double* a, double* b) {
+  Workspace* ws = &h->ws;
+  cudaStream_t st = h->stream;
+  const int64_t n = h->n;
+  const int m = h->lanczos_steps;
+  if (!h->lz[0]) {
+    if (cudaMalloc(&h->lz[0], sizeof(cplx) * (size_t)n) != cudaSuccess || cudaMalloc(&h->lz[1], sizeof(cplx) * (size_t)n) != cudaSuccess ||
+        cudaMalloc(&h->lz_scal, sizeof(double) * (2 + 2 * 64)) != cudaSuccess) {
+      cudaGetLastError();
+      set_error("tight interval: allocation of the Lanczos vectors failed");
+      return MAGNUS_ENOMEM;
+    }
+  }
+  CU_TRY(cudaMemsetAsync(ws->status, 0, sizeof(LejaStatus), st));
+  CU_TRY(cudaMemsetAsync(ws->p, 0, sizeof(cplx) * (size_t)n, st));   // the mat-vec kernel's Newton sum: d_k = 0 keeps it 0
+  CU_TRY(cudaMemsetAsync(h->lz_scal, 0, sizeof(double) * (2 + 2 * 64), st));
+  cplx* q = h->lz[0];
+  cplx* qp = h->lz[1];
+  launch_lanczos_start(v, q, qp, n, h->lz_scal, ws, st);
+  for (int j = 0; j < m; ++j) {
+    // u = M q_j: the fused Leja iteration as a plain mat-vec (1/gamma = 1, shift = 0, d_k = 0; |d_k| = 1, tol = 0: no stop)
+    launch_iter(op, q, ws->w[0], ws->p, 1.0, 0.0, make_double2(0.0, 0.0), 1.0, 0.0, ws, st);
+    launch_lanczos_step(ws->w[0], q, qp, n, h->lz_scal, j, m, ws, st);
+    std::swap(q, qp);
+  }
+  h->lanczos_matvecs += m;
+  double sc[2 + 2 * 64];
+  CU_TRY(cudaGetLastError());
+  CU_TRY(cudaMemcpyAsync(sc, h->lz_scal, sizeof(double) * (size_t)(2 + 2 * m), cudaMemcpyDeviceToHost, st));
+  CU_TRY(cudaStreamSynchronize(st));
+  if (!(sc[0] > 0.0)) return kPlanDeclined;
+  const double* alpha = sc + 2;
+  const double* beta = sc + 2 + m;
+  int k = m;
+  double scale = 0.0;
+  for (int j = 0; j < m; ++j) {
+    if (!std::isfinite(alpha[j]) || !std::isfinite(beta[j])) { set_error("tight interval: Lanczos produced a non-finite value"); return MAGNUS_EINVAL; }
+    scale = std::max(scale, std::max(std::fabs(alpha[j]), beta[j]));
+    if (beta[j] <= 1e-12 * scale) { k = j + 1; break; }      // invariant subspace: T is exact, later steps are noise
+  }
+  double lo = 0.0, hi = 0.0;
+  tridiag_extreme_eigenvalues(alpha, beta, k, &lo, &hi);
+  *a = lo - beta[k - 1];
+  *b = hi + beta[k - 1];
+  return MAGNUS_OK;
+}
+
 // One step on the stepwise path: interval, table and stop polling per exponential (rows S1-S8, D3, D4).
 static int magnus_step_unplanned(magnus_context* h, double t, double tau, cplx* psi, magnus_step_info* info) {
   double coef[MAGNUS_MAX_EXP_PER_STEP], hscale[MAGNUS_MAX_EXP_PER_STEP], kappa = 0.0;
@@ -756,6 +809,18 @@ static int magnus_step_unplanned(magnus_context* h, double t, double tau, cplx* 
       }
     }
     if (rc) break;
+    if (h->shortcuts & MAGNUS_SHORTCUT_TIGHT_INTERVAL) {
+      double ta = 0.0, tb = 0.0;
+      rc = lanczos_interval(h, op, psi, &ta, &tb);
+      if (rc == MAGNUS_OK) {
+        a = ta;
+        b = tb;
+      } else if (rc == kPlanDeclined) {
+        rc = MAGNUS_OK;       // psi = 0: nothing to estimate from, the Gershgorin interval stays
+      } else {
+        break;
+      }
+    }
     rc = expmv_on_interval(op, a, b, psi, psi, hscale[e] * tau, h->prm, ws, st, info ? &info->exp[e] : nullptr);
   }
   return rc;
@@ -817,6 +882,9 @@ int magnus_destroy(magnus_handle h) {
   cudaFree(h->X5);
   cudaFree(h->d0);
   cudaFree(h->d1);
+  cudaFree(h->lz[0]);
+  cudaFree(h->lz[1]);
+  cudaFree(h->lz_scal);
   cudaFree(h->c_rp);
   cudaFree(h->c_ci);
   cudaFree(h->c_v);
@@ -903,6 +971,7 @@ int magnus_create(magnus_handle* out, const magnus_matrix* H0, const magnus_matr
   h->f = f;
   h->user = user;
   default_params(opt, &h->prm, &h->stream, &h->ws.csr_kernel, &h->shortcuts);
+  h->lanczos_steps = (opt && opt->lanczos_steps > 0) ? std::min(64, opt->lanczos_steps) : 8;
   const int csr_kernel = h->ws.csr_kernel;
   rc = workspace_alloc(&h->ws, h->n);
   h->ws.csr_kernel = csr_kernel;
@@ -1044,6 +1113,7 @@ int magnus_create_xxz(magnus_handle* out, const magnus_xxz_model* model, magnus_
   h->f = f;
   h->user = user;
   default_params(opt, &h->prm, &h->stream, &h->ws.csr_kernel, &h->shortcuts);
+  h->lanczos_steps = (opt && opt->lanczos_steps > 0) ? std::min(64, opt->lanczos_steps) : 8;
   rc = workspace_alloc(&h->ws, h->n);
   h->ws.csr_kernel = 1;       // no whole-sweep kernels on this path
   h->ws.time_leja = true;
@@ -1070,6 +1140,7 @@ int magnus_integrate(magnus_handle h, double t0, double t_end, int64_t nsteps, v
   const int64_t launches0 = ws->launches;
   ws->leja_ms = 0.0;
   h->comm_ms = 0.0;
+  h->lanczos_matvecs = 0;
   CU_TRY(cudaEventRecord(ws->ev[2], st));
   int64_t total = 0, nexp = 0;
   int rc = MAGNUS_OK;
@@ -1112,6 +1183,7 @@ int magnus_integrate(magnus_handle h, double t0, double t_end, int64_t nsteps, v
     stats->seconds_leja = ws->leja_ms * 1e-3;
     stats->seconds_commutator = h->comm_ms * 1e-3;
     stats->kernel_launches = ws->launches - launches0;
+    stats->lanczos_matvecs = h->lanczos_matvecs;
   }
   return rc;
 }

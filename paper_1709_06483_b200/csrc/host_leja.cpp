@@ -111,6 +111,41 @@ void divided_differences(double theta, int m, std::complex<double>* out) {
   for (int k = 0; k < m; ++k) out[k] = std::complex<double>((double)vr[k], (double)vi[k]);
 }
 
+// Extreme eigenvalues of the symmetric tridiagonal T = tridiag(alpha_0..alpha_{k-1}; beta_0..beta_{k-2}) by bisection on
+// the Sturm count (number of eigenvalues below x = number of negative pivots of T - xI); used by the tight-interval
+// shortcut (kernels_lanczos.cu).  Accurate to a few ulps of ||T||.
+static int sturm_count(const double* alpha, const double* beta, int k, double x) {
+  int cnt = 0;
+  double d = 1.0;
+  for (int i = 0; i < k; ++i) {
+    const double b2 = i > 0 ? beta[i - 1] * beta[i - 1] : 0.0;
+    d = (alpha[i] - x) - (i > 0 ? b2 / d : 0.0);
+    if (d == 0.0) d = -1e-300;          // a pivot of exactly 0 counts as negative (eigenvalue <= x)
+    if (d < 0.0) ++cnt;
+  }
+  return cnt;
+}
+
+void tridiag_extreme_eigenvalues(const double* alpha, const double* beta, int k, double* lo_out, double* hi_out) {
+  double lo = alpha[0], hi = alpha[0];
+  for (int i = 0; i < k; ++i) {         // Gershgorin bounds of T bracket its spectrum
+    const double r = (i > 0 ? std::fabs(beta[i - 1]) : 0.0) + (i + 1 < k ? std::fabs(beta[i]) : 0.0);
+    lo = std::min(lo, alpha[i] - r);
+    hi = std::max(hi, alpha[i] + r);
+  }
+  auto kth = [&](int want) {            // smallest x with count(x) >= want, i.e. the want-th eigenvalue
+    double a = lo, b = hi;
+    for (int it = 0; it < 200; ++it) {
+      const double mid = 0.5 * (a + b);
+      if (mid <= a || mid >= b) break;
+      if (sturm_count(alpha, beta, k, mid) >= want) b = mid; else a = mid;
+    }
+    return 0.5 * (a + b);
+  };
+  *lo_out = kth(1);
+  *hi_out = kth(k);
+}
+
 // Reading c4: widen [a,b] outward to the grid of spacing 2^(E-12), E = ceil(log2(b-a)).
 void snap_interval(double* a, double* b) {
   const double width = *b - *a;

@@ -16,6 +16,7 @@ const int kMaxDegree = 128;   // m_max (reading c6)
 const double* leja_points();                                  // kMaxDegree + 1 points
 void divided_differences(double theta, int m, std::complex<double>* out);
 void snap_interval(double* a, double* b);
+void tridiag_extreme_eigenvalues(const double* alpha, const double* beta, int k, double* lo, double* hi);
 int step_coefficients(int scheme, magnus_drive_fn f, void* user, double t, double tau,
                       double* coef_h1, double* h_scale, double* kappa);
 
@@ -214,6 +215,11 @@ inline int slice_layout_kind(int csr_kernel) {
 void slice_layout_free(SliceLayout* L);
 int launch_csr_leja_iter_slice(const CsrOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma, double shift,
                                cplx dk, double abs_dk, double tol, Workspace* ws, cudaStream_t st);
+
+// ---- kernels_lanczos.cu (shortcut: tight spectral interval) ------------------
+void launch_lanczos_start(const cplx* v, cplx* q, cplx* qprev, int64_t n, double* scal, Workspace* ws, cudaStream_t st);
+void launch_lanczos_step(cplx* u, const cplx* q, cplx* qprev, int64_t n, double* scal, int j, int m, Workspace* ws,
+                         cudaStream_t st);
 
 // ---- kernels_xxz.cu ---------------------------------------------------------
 int launch_xxz_leja_iter(const XxzOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma, double shift,

@@ -694,3 +694,38 @@ def test_shortcut_matrix_free_xxz_refuses_commutator_schemes(M):
         assert e.value.code == -1
     with pytest.raises(M.MagnusError):
         M.magnus_create_xxz(2, 1.0, 0.5, 1.0, xxz.f_cos2t, "cf4")
+
+
+# ------------------------------------------------------------------ shortcut: tight spectral interval
+@pytest.mark.parametrize("name,size,nsteps,scheme,m", [("cfg2", 33, 3, "cf4", 8), ("cfg2", 300, 3, "cf4", 8),
+                                                       ("cfg2", 300, 2, "m4", 6), ("cfg2", 1237, 2, "cf4:3", 8),
+                                                       ("cfg2", 5000, 1, "cf4", 8), ("cfg1", 10, 5, "cf4", 8),
+                                                       ("cfg1", 10, 5, "m4", 8), ("cfg3", 14, 2, "cf4", 12)])
+def test_shortcut_tight_interval_vs_oracle(M, oracle, name, size, nsteps, scheme, m):
+    """MAGNUS_SHORTCUT_TIGHT_INTERVAL: the interval of every exponential from m Lanczos steps started at psi.
+    Against the oracle in the same mode (its own Lanczos, Jacobi eigenvalues): identical snapped intervals,
+    identical iteration counts, psi <= 1e-9; on dense input fewer Leja iterations than with Gershgorin."""
+    cfg = W.scaled(W.CONFIGS[name], size, nsteps)
+    H0, H1, psi0, f = W.build(cfg)
+    if cfg.kind == "xxz":
+        o0, o1 = oracle.CsrHost.of(H0), oracle.CsrHost.of(H1)
+    else:
+        o0, o1 = H0.numpy(), H1.numpy()
+    d0, d1 = H0.to(DEV), H1.to(DEV)
+    with oracle.tight_interval(m):
+        ref, riters = oracle.magnus_integrate(o0, o1, f, scheme, cfg.t0, cfg.t_end, cfg.nsteps, psi0.numpy(), cfg.tol)
+        _, rinfo = oracle.magnus_step(o0, o1, f, scheme, cfg.t0, cfg.tau, psi0.numpy(), cfg.tol)
+    psi = psi0.to(DEV).clone()
+    with M.magnus_create(d0, d1, f, scheme, tol=cfg.tol, shortcuts=M.SHORTCUT_TIGHT_INTERVAL, lanczos_steps=m) as h:
+        info = h.step(cfg.t0, cfg.tau, psi0.to(DEV).clone())
+        st = h.integrate(cfg.t0, cfg.t_end, cfg.nsteps, psi)
+    for gi, ri in zip(info, rinfo):
+        assert gi["a"] == ri["a"] and gi["b"] == ri["b"] and gi["theta"] == ri["theta"] and gi["iters"] == ri["iters"]
+    assert np.array_equal(st["iters"], riters) and st["lanczos_matvecs"] == m * len(riters)
+    assert relerr(host(psi), ref) <= 1e-9 and abs(np.linalg.norm(host(psi)) - 1) < 1e-10
+    if cfg.kind == "dense":
+        psi2 = psi0.to(DEV).clone()
+        with M.magnus_create(d0, d1, f, scheme, tol=cfg.tol) as h:
+            st2 = h.integrate(cfg.t0, cfg.t_end, cfg.nsteps, psi2)
+        assert st["total_matvecs"] < st2["total_matvecs"]
+        assert relerr(host(psi), host(psi2)) <= 1e-9           # two intervals, one exponential
