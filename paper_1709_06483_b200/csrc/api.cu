@@ -295,6 +295,7 @@ struct magnus_context {
   int format = 0;
   int shortcuts = 0;
   bool cached_p0 = false;      // dense M4 shortcut: h->P holds P0 = H0 H1
+  ZgemmScratch zs;             // dense M4 / M6: workspace of the split-tail GEMM
   int lanczos_steps = 8;       // tight-interval shortcut
   cplx* lz[2] = {nullptr, nullptr};   // ... its Lanczos vectors q_j, q_{j-1}
   double* lz_scal = nullptr;          // ... and device scalars (norm, beta_prev, alpha[], beta[])
@@ -762,10 +763,10 @@ static int magnus_step_unplanned(magnus_context* h, double t, double tau, cplx* 
         if (dense_ld(&h->H0) != n || dense_ld(&h->H1) != n) { set_error("MAGNUS_M6 needs ld == n"); rc = MAGNUS_EINVAL; break; }
         launch_dense_lincomb(n, h->M, lc, ws, st);                                   // X1 = H2 = H0 + f2 H1
         if (h->time_comm) cudaEventRecord(h->ev_comm[0], st);
-        rc = launch_zgemm(n, h->M, n, H1v, n, h->A2, n, st);                          // X2 = P1 = H2 H1
+        rc = launch_zgemm(n, h->M, n, H1v, n, h->A2, n, st, &h->zs);                          // X2 = P1 = H2 H1
         if (rc) break;
         launch_dense_antiherm(n, h->A2, h->P, -1.0, st);                              // X3 = G = P1 - P1^H = [H2, H1]
-        rc = launch_zgemm(n, h->M, n, h->P, n, h->A2, n, st);                         // X2 = P2 = H2 G
+        rc = launch_zgemm(n, h->M, n, h->P, n, h->A2, n, st, &h->zs);                         // X2 = P2 = H2 G
         if (rc) break;
         launch_dense_antiherm(n, h->A2, h->X4, 1.0, st);                              // X4 = S = P2 + P2^H = [H2, G]
         term(0, h->M, 0.0, 20.0 * tau); term(1, H1v, 0.0, b3); term(2, h->P, -tau * b2, 0.0); term(3, nullptr, 0.0, 0.0);
@@ -773,7 +774,7 @@ static int magnus_step_unplanned(magnus_context* h, double t, double tau, cplx* 
         term(0, H1v, 0.0, -b2); term(1, h->P, tau * b3 / 30.0, 0.0); term(2, h->X4, 0.0, -tau * tau * b2 / 60.0);
         term(3, nullptr, 0.0, 0.0);
         launch_dense_lincomb(n, h->X5, lc, ws, st);                                  // X5 = R
-        rc = launch_zgemm(n, h->A2, n, h->X5, n, h->X4, n, st);                       // X4 = P3 = L R
+        rc = launch_zgemm(n, h->A2, n, h->X5, n, h->X4, n, st, &h->zs);                       // X4 = P3 = L R
         ws->launches += 5;
         if (h->time_comm) cudaEventRecord(h->ev_comm[1], st);
         if (rc) break;
@@ -791,7 +792,7 @@ static int magnus_step_unplanned(magnus_context* h, double t, double tau, cplx* 
         launch_dense_assemble2(h->n, H0v, dense_ld(&h->H0), H1v, dense_ld(&h->H1), coef[0], coef[1], h->M, h->A2, ws,
                                st);                                                                // S2: A1, A2
         if (h->time_comm) cudaEventRecord(h->ev_comm[0], st);
-        rc = launch_zgemm(h->n, h->A2, h->n, h->M, h->n, h->P, h->n, st);                          // D3: P = A2 A1
+        rc = launch_zgemm(h->n, h->A2, h->n, h->M, h->n, h->P, h->n, st, &h->zs);                          // D3: P = A2 A1
         ws->launches += 1;
         if (h->time_comm) cudaEventRecord(h->ev_comm[1], st);
         if (rc) { set_error("zgemm launch failed: %s", cudaGetErrorString(cudaGetLastError())); break; }
@@ -882,6 +883,7 @@ int magnus_destroy(magnus_handle h) {
   cudaFree(h->X5);
   cudaFree(h->d0);
   cudaFree(h->d1);
+  zgemm_scratch_free(&h->zs);
   cudaFree(h->lz[0]);
   cudaFree(h->lz[1]);
   cudaFree(h->lz_scal);
@@ -1037,6 +1039,7 @@ int magnus_create(magnus_handle* out, const magnus_matrix* H0, const magnus_matr
       return MAGNUS_ENOMEM;
     }
     if (scheme == MAGNUS_M4 || scheme == MAGNUS_M6) {
+      zgemm_scratch_alloc(&h->zs);     // on failure the plain one-CTA-per-tile form runs
       cudaEventCreate(&h->ev_comm[0]);
       cudaEventCreate(&h->ev_comm[1]);
       h->time_comm = true;
@@ -1047,7 +1050,7 @@ int magnus_create(magnus_handle* out, const magnus_matrix* H0, const magnus_matr
         magnus_destroy(h);
         return MAGNUS_EINVAL;
       }
-      rc = launch_zgemm(h->n, (const cplx*)H0->values, h->n, (const cplx*)H1->values, h->n, h->P, h->n, h->stream);
+      rc = launch_zgemm(h->n, (const cplx*)H0->values, h->n, (const cplx*)H1->values, h->n, h->P, h->n, h->stream, &h->zs);
       if (rc) { set_error("zgemm launch failed: %s", cudaGetErrorString(cudaGetLastError())); magnus_destroy(h); return rc; }
       h->cached_p0 = true;
       h->time_comm = false;
@@ -1417,8 +1420,10 @@ int magnus_zgemm(int64_t n, const void* A, int64_t lda, const void* B, int64_t l
   cudaEvent_t e0, e1;
   CU_TRY(cudaEventCreate(&e0));
   CU_TRY(cudaEventCreate(&e1));
+  ZgemmScratch zs;
+  zgemm_scratch_alloc(&zs);
   cudaEventRecord(e0, st);
-  rc = launch_zgemm(n, (const cplx*)A, lda, (const cplx*)B, ldb, (cplx*)C, ldc, st);
+  rc = launch_zgemm(n, (const cplx*)A, lda, (const cplx*)B, ldb, (cplx*)C, ldc, st, &zs);
   cudaEventRecord(e1, st);
   if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) {
     set_error("magnus_zgemm: kernel failed");
@@ -1428,6 +1433,7 @@ int magnus_zgemm(int64_t n, const void* A, int64_t lda, const void* B, int64_t l
   }
   cudaEventDestroy(e0);
   cudaEventDestroy(e1);
+  zgemm_scratch_free(&zs);
   return rc;
 }
 

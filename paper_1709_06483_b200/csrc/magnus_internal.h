@@ -273,8 +273,15 @@ int launch_dense_leja_iter(const DenseOp& op, const cplx* w_in, cplx* w_out, cpl
 int dense_hermitian_check(const DenseOp& op, cudaStream_t st, double* max_violation);
 
 // ---- zgemm_dmma.cu ----------------------------------------------------------
+// workspace of the split-tail form of the GEMM (partial tiles parked by the later K ranges of a split tile, one flag each)
+struct ZgemmScratch {
+  double* parked = nullptr;
+  unsigned* flags = nullptr;
+};
+int zgemm_scratch_alloc(ZgemmScratch* zs);
+void zgemm_scratch_free(ZgemmScratch* zs);
 int launch_zgemm(int64_t n, const cplx* A, int64_t lda, const cplx* B, int64_t ldb, cplx* C, int64_t ldc,
-                 cudaStream_t st);
+                 cudaStream_t st, const ZgemmScratch* zs = nullptr);
 int fp64_peaks(double* dmma_tflops, double* dfma_tflops, cudaStream_t st);
 
 }  // namespace magnus

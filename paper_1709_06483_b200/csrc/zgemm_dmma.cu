@@ -10,10 +10,13 @@
 // planes of a fragment element.  K is consumed in slabs of 16 complex through a
 // 3-stage cp.async ring (16-byte copies, zero-filled outside the matrix).
 // Row pitches of 20 (A) and 66 (B) double2 make the fragment loads conflict-free.
-// Two instantiations: 128 x 64 tiles (8 warps, one CTA per SM) and 64 x 64 tiles (4 warps, two CTAs per SM).
-// The small tile is for sizes whose 128 x 64 tile count leaves the last wave mostly empty (n = 2048: 512
-// tiles on 148 SMs = 3.46 waves): with two CTAs per SM the last, partial wave has an SM to itself per CTA
-// and runs at about twice the per-CTA speed, so the tail costs half a wave instead of a whole one.
+// Two launch shapes of the same kernel.  One CTA per 128 x 64 tile, all of K -- used when the tile count fills
+// its last wave (n = 16384: 221.4 waves).  SPLIT TAIL -- one persistent CTA per SM -- when it does not (n = 2048:
+// 512 tiles on 148 SMs = 3.46 waves, half of the machine idle in the last one): CTA b first does the tiles
+// b, b + SMs, ... of the full waves in the grouped raster order (so that concurrent tiles keep sharing their
+// panels in L2), then the R = tiles mod SMs leftover tiles are each split into s = SMs / R ranges of K: the
+// CTAs of the later ranges park their partial tile in a workspace, the CTA of the first range adds them in range
+// order (a fixed order) and stores.  The tail then costs 1/s of a wave.
 #include "magnus_internal.h"
 #include "device_utils.cuh"
 
@@ -45,31 +48,49 @@ __device__ __forceinline__ void dmma8x8x4(double& c0, double& c1, double a, doub
                : "d"(a), "d"(b));
 }
 
-template <int BM>
-__global__ void __launch_bounds__(BM * 2, BM == 128 ? 1 : 2) zgemm_dmma_kernel(int64_t n, const cplx* __restrict__ A, int64_t lda,
-                                                                       const cplx* __restrict__ B, int64_t ldb,
-                                                                       cplx* __restrict__ C, int64_t ldc, int tiles_m,
-                                                                       int tiles_n) {
+// STREAMK = false: grid = tiles, the CTA does tile blockIdx.x over all of K.
+// STREAMK = true:  grid = SMs (cooperative: all CTAs resident); `split` = s; parked[b] / flags[b] belong to CTA b.
+template <bool STREAMK>
+__global__ void __launch_bounds__(256, 1) zgemm_dmma_kernel(int64_t n, const cplx* __restrict__ A, int64_t lda,
+                                                             const cplx* __restrict__ B, int64_t ldb,
+                                                             cplx* __restrict__ C, int64_t ldc, int tiles_m, int tiles_n,
+                                                             double* parked, unsigned* flags, int split) {
+  constexpr int BM = 128;
   constexpr int THREADS = BM * 2;              // BM / 32 x 2 warps
   constexpr int A_STAGE = BM * LDA_S;          // double2 per stage
   extern __shared__ __align__(16) unsigned char zg_smem[];
   cplx* sA = reinterpret_cast<cplx*>(zg_smem);
   cplx* sB = sA + STAGES * A_STAGE;
-
-  // grouped rasterisation: 8 tile-rows share their B panels through L2
-  const int GROUP = 8;
-  const int bid = blockIdx.x;
-  const int per_group = GROUP * tiles_n;
-  const int group = bid / per_group;
-  const int first_m = group * GROUP;
-  const int gsize = min(tiles_m - first_m, GROUP);
-  const int tm = first_m + (bid % per_group) % gsize;
-  const int tn = (bid % per_group) / gsize;
-  const int64_t m0 = (int64_t)tm * BM, n0 = (int64_t)tn * BN;
-
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int wm = warp >> 1, wn = warp & 1;           // BM / 32 x 2 warps
   const int g = lane >> 2, q = lane & 3;
+  const int KT = (int)((n + BK - 1) / BK);
+  const int ntiles = tiles_m * tiles_n;
+  const int full = STREAMK ? ntiles / (int)gridDim.x : 0;      // full waves
+  const int nitems = STREAMK ? full + 1 : 1;                   // this CTA's tiles of the full waves, then its tail range
+
+  for (int item = 0; item < nitems; ++item) {
+  int tile, kt_begin = 0, kt_end = KT, piece = 0;
+  if (!STREAMK) {
+    tile = blockIdx.x;
+  } else if (item < full) {
+    tile = item * (int)gridDim.x + (int)blockIdx.x;
+  } else {
+    tile = full * (int)gridDim.x + (int)blockIdx.x / split;
+    piece = (int)blockIdx.x % split;
+    if (tile >= ntiles) break;                                 // CTAs beyond R * s have no tail work
+    kt_begin = (int)((int64_t)KT * piece / split);
+    kt_end = (int)((int64_t)KT * (piece + 1) / split);
+  }
+  // grouped rasterisation: 8 tile-rows share their B panels through L2
+  const int GROUP = 8;
+  const int per_group = GROUP * tiles_n;
+  const int group = tile / per_group;
+  const int first_m = group * GROUP;
+  const int gsize = min(tiles_m - first_m, GROUP);
+  const int tm = first_m + (tile % per_group) % gsize;
+  const int tn = (tile % per_group) / gsize;
+  const int64_t m0 = (int64_t)tm * BM, n0 = (int64_t)tn * BN;
 
   double cre[4][4][2], cim[4][4][2];
 #pragma unroll
@@ -79,8 +100,7 @@ __global__ void __launch_bounds__(BM * 2, BM == 128 ? 1 : 2) zgemm_dmma_kernel(i
       cre[i][j][0] = cre[i][j][1] = 0.0;
       cim[i][j][0] = cim[i][j][1] = 0.0;
     }
-
-  const int KT = (int)((n + BK - 1) / BK);
+  __syncthreads();                             // the previous segment's last slab is consumed before the ring is refilled
 
   auto load_stage = [&](int stage, int kt) {
     const int64_t k0 = (int64_t)kt * BK;
@@ -104,17 +124,18 @@ __global__ void __launch_bounds__(BM * 2, BM == 128 ? 1 : 2) zgemm_dmma_kernel(i
     }
   };
 
+  const int KS = kt_end - kt_begin;            // slabs of this segment; ring slots count from the segment start
 #pragma unroll
   for (int s = 0; s < STAGES - 1; ++s) {
-    if (s < KT) load_stage(s, s);
+    if (s < KS) load_stage(s, kt_begin + s);
     cp_async_commit();
   }
 
-  for (int kt = 0; kt < KT; ++kt) {
+  for (int kt = 0; kt < KS; ++kt) {
     cp_async_wait<STAGES - 2>();
     __syncthreads();
     const int nxt = kt + STAGES - 1;
-    if (nxt < KT) load_stage(nxt % STAGES, nxt);
+    if (nxt < KS) load_stage(nxt % STAGES, kt_begin + nxt);
     cp_async_commit();
 
     const cplx* a_s = sA + (kt % STAGES) * A_STAGE + (wm * 32 + g) * LDA_S + q;
@@ -141,6 +162,47 @@ __global__ void __launch_bounds__(BM * 2, BM == 128 ? 1 : 2) zgemm_dmma_kernel(i
   }
   cp_async_wait<0>();
 
+  if (STREAMK && piece > 0) {
+    // a later range of a split tile: park the partial tile, raise the flag
+    double* dst = parked + (size_t)blockIdx.x * 64 * THREADS + tid;
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const int s4 = (i * 4 + j) * 4;
+        __stcg(dst + (size_t)(s4 + 0) * THREADS, cre[i][j][0]);
+        __stcg(dst + (size_t)(s4 + 1) * THREADS, cre[i][j][1]);
+        __stcg(dst + (size_t)(s4 + 2) * THREADS, cim[i][j][0]);
+        __stcg(dst + (size_t)(s4 + 3) * THREADS, cim[i][j][1]);
+      }
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) atomicExch(flags + blockIdx.x, 1u);
+    continue;
+  }
+  if (STREAMK && item == full && split > 1) {
+    // the first range of a split tile: add the parked ranges in range order
+    for (int pc = 1; pc < split; ++pc) {
+      if (tid == 0) {
+        while (atomicAdd(flags + blockIdx.x + pc, 0u) == 0u) {
+        }
+        __threadfence();
+      }
+      __syncthreads();
+      const double* src = parked + (size_t)(blockIdx.x + pc) * 64 * THREADS + tid;
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const int s4 = (i * 4 + j) * 4;
+          cre[i][j][0] += __ldcg(src + (size_t)(s4 + 0) * THREADS);
+          cre[i][j][1] += __ldcg(src + (size_t)(s4 + 1) * THREADS);
+          cim[i][j][0] += __ldcg(src + (size_t)(s4 + 2) * THREADS);
+          cim[i][j][1] += __ldcg(src + (size_t)(s4 + 3) * THREADS);
+        }
+    }
+  }
+
   // epilogue: lane holds C[row g][cols 2q, 2q+1] of every 8x8 tile
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
@@ -154,6 +216,7 @@ __global__ void __launch_bounds__(BM * 2, BM == 128 ? 1 : 2) zgemm_dmma_kernel(i
       if (c + 1 < n) dst[1] = make_double2(cre[i][j][1], cim[i][j][1]);
     }
   }
+  }   // items of this CTA
 }
 
 // ---- register-resident peak probes ------------------------------------------
@@ -189,28 +252,55 @@ __global__ void __launch_bounds__(256) dfma_peak_kernel(int iters, double* __res
 
 }  // namespace
 
-int launch_zgemm(int64_t n, const cplx* A, int64_t lda, const cplx* B, int64_t ldb, cplx* C, int64_t ldc,
-                 cudaStream_t st) {
-  // wave efficiency of the 128 x 64 tiling: tiles / (waves * SMs); below 0.93 the 64 x 64 tiling (two CTAs per SM,
-  // half-cost tail) is used
+int zgemm_scratch_alloc(ZgemmScratch* zs) {
+  if (zs->parked) return MAGNUS_OK;
   const int sms = device_sm_count();
-  const int tn = (int)((n + BN - 1) / BN);
-  const int64_t t128 = (int64_t)((n + 127) / 128) * tn;
-  const double eff128 = (double)t128 / (double)(((t128 + sms - 1) / sms) * sms);
-  // per launch (cheap): the attribute is per device, a process-wide flag would miss a second GPU
-  if (eff128 >= 0.93) {
-    if (cudaFuncSetAttribute(zgemm_dmma_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, zgemm_smem<128>()) !=
-        cudaSuccess)
-      return MAGNUS_ECUDA;
-    const int tm = (int)((n + 127) / 128);
-    zgemm_dmma_kernel<128><<<tm * tn, 256, zgemm_smem<128>(), st>>>(n, A, lda, B, ldb, C, ldc, tm, tn);
-  } else {
-    if (cudaFuncSetAttribute(zgemm_dmma_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, zgemm_smem<64>()) !=
-        cudaSuccess)
-      return MAGNUS_ECUDA;
-    const int tm = (int)((n + 63) / 64);
-    zgemm_dmma_kernel<64><<<tm * tn, 128, zgemm_smem<64>(), st>>>(n, A, lda, B, ldb, C, ldc, tm, tn);
+  if (cudaMalloc(&zs->parked, sizeof(double) * 64 * 256 * (size_t)sms) != cudaSuccess ||
+      cudaMalloc(&zs->flags, sizeof(unsigned) * (size_t)sms) != cudaSuccess) {
+    cudaGetLastError();
+    zgemm_scratch_free(zs);
+    return MAGNUS_ENOMEM;
   }
+  return MAGNUS_OK;
+}
+
+void zgemm_scratch_free(ZgemmScratch* zs) {
+  cudaFree(zs->parked);
+  cudaFree(zs->flags);
+  zs->parked = nullptr;
+  zs->flags = nullptr;
+}
+
+// zs (nullable): the workspace of the split-tail form; without it one CTA per tile runs whatever the size
+int launch_zgemm(int64_t n, const cplx* A, int64_t lda, const cplx* B, int64_t ldb, cplx* C, int64_t ldc,
+                 cudaStream_t st, const ZgemmScratch* zs) {
+  const int sms = device_sm_count();
+  int tm = (int)((n + 127) / 128), tn = (int)((n + BN - 1) / BN);
+  const int KT = (int)((n + BK - 1) / BK);
+  const int64_t tiles = (int64_t)tm * tn;
+  // wave efficiency of one CTA per tile: tiles / (waves * SMs); the split tail needs at least one full wave, a
+  // leftover that can be split at least in two, and ranges of at least 8 slabs
+  const double eff = (double)tiles / (double)(((tiles + sms - 1) / sms) * sms);
+  const int R = (int)(tiles % sms);
+  int split = R > 0 ? sms / R : 1;
+  if (split > 4) split = 4;
+  while (split > 1 && KT / split < 8) --split;
+  const int smem = zgemm_smem<128>();
+  // per launch (cheap): the attribute is per device, a process-wide flag would miss a second GPU
+  if (cudaFuncSetAttribute(zgemm_dmma_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess ||
+      cudaFuncSetAttribute(zgemm_dmma_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
+    return MAGNUS_ECUDA;
+  if (zs && zs->parked && eff < 0.93 && tiles >= sms && split > 1 &&
+      cudaMemsetAsync(zs->flags, 0, sizeof(unsigned) * (size_t)sms, st) == cudaSuccess) {
+    double* parked = zs->parked;
+    unsigned* flags = zs->flags;
+    void* args[] = {&n, &A, &lda, &B, &ldb, &C, &ldc, &tm, &tn, &parked, &flags, &split};
+    if (cudaLaunchCooperativeKernel((const void*)zgemm_dmma_kernel<true>, dim3(sms), dim3(256), args, smem, st) == cudaSuccess)
+      return MAGNUS_OK;
+    cudaGetLastError();   // could not be launched cooperatively: one CTA per tile
+  }
+  int one = 1;
+  zgemm_dmma_kernel<false><<<(unsigned)tiles, 256, smem, st>>>(n, A, lda, B, ldb, C, ldc, tm, tn, nullptr, nullptr, one);
   return cudaGetLastError() == cudaSuccess ? MAGNUS_OK : MAGNUS_ECUDA;
 }
 

@@ -272,6 +272,30 @@ def test_zgemm_dmma_vs_oracle_product(M, oracle, n):
     assert np.max(np.abs(host(Cd) - ref)) <= 8 * n * np.finfo(float).eps * np.max(np.abs(ref)) + 1e-300
 
 
+@pytest.mark.parametrize("n", [2048, 2300, 2944, 3100])
+def test_zgemm_stream_k_sampled_rows_and_columns(M, oracle, n):
+    """Sizes whose 128 x 64 tile count leaves the last wave badly filled run the stream-K form of the DMMA GEMM
+    (tiles split between two CTAs, partial tile parked and added): 2048 = CFG2, 2300 and 3100 with ragged edge tiles,
+    2944 = 23 x 46 tiles.  Six whole rows and six whole columns of A B against the oracle's mat-vec, among them the
+    first and last and rows / columns of split tiles."""
+    A = dense.random_hermitian(n, stream=53)
+    B = dense.random_hermitian(n, stream=54) + 0.1j * torch.triu(torch.ones(n, n, dtype=torch.complex128), 1)
+    Cd = torch.empty(n, n, dtype=torch.complex128, device=DEV)
+    M.magnus_zgemm(A.to(DEV), B.to(DEV), Cd)
+    C = host(Cd)
+    An, Bn = A.numpy(), B.numpy()
+    idx = [0, n - 1, 127, 128, n // 2 + 3, (3 * n) // 4]
+    tol = 8 * n * np.finfo(float).eps
+    for j in idx:
+        col = oracle.matvec(An, np.ascontiguousarray(Bn[:, j]))               # column j of A B = A (B e_j)
+        assert np.max(np.abs(C[:, j] - col)) <= tol * np.max(np.abs(col))
+        row = oracle.matvec(np.ascontiguousarray(Bn.T), np.ascontiguousarray(An[j, :]))   # row j of A B = B^T (A^T e_j)
+        assert np.max(np.abs(C[j, :] - row)) <= tol * np.max(np.abs(row))
+    assert np.isfinite(C).all()
+    ref = An[5::97, :] @ Bn                                                         # a coarse sweep over all tiles
+    assert np.max(np.abs(C[5::97, :] - ref)) <= tol * np.max(np.abs(ref))
+
+
 @pytest.mark.parametrize("n", [48, 200, 333])
 def test_dense_commutator_vs_oracle(M, oracle, n):
     A = dense.random_hermitian(n, stream=53)
