@@ -562,31 +562,40 @@ __device__ __forceinline__ void sort_keys(unsigned long long* skey, int total, i
 //      the survivors, which are already in column order.
 // The spin chains need (N/2 + 1) N 2 candidates per row (624 at N = 24); a row with more than kSortCap
 // candidates or more than kCommLists lists is left to the CTA-wide sorting kernel below.
+// Two tiers of the warp kernel: candidate buffers of 512 entries for all rows (14 warps per SM), and of 1024 for the
+// rows the first tier hands on through a second worklist (the chains' rows with many antiparallel bonds).
 const int kCommLists = 256;
 const int kMergeWarps = 2;
-const int kSortCap = 1024;
+const int kSortCap = 1024;    // largest candidate buffer (second tier)
 const int kCommTmp = 32;      // entries of a row of C the warp kernel parks in the temporary buffer
-const int kMergeSmem = kMergeWarps * (kSortCap * (int)(sizeof(cplx) + sizeof(unsigned long long)) + 3 * kCommLists * (int)sizeof(int));
+template <int CAP>
+constexpr int merge_smem() { return kMergeWarps * (CAP * (int)(sizeof(cplx) + sizeof(unsigned long long)) + 3 * kCommLists * (int)sizeof(int)); }
 
 // counts[row] = entries of row i of C; the entries themselves go to tmp_ci / tmp_v at row * kCommTmp (the gather
 // kernel moves them to their CSR place once the row pointers are known).  A row this kernel does not take --
-// too many lists or candidates, or more than kCommTmp entries -- is appended to `work` (work[0] = how many).
+// too many lists, more than kSortCap candidates, or more than kCommTmp entries -- is appended to `work` (work[0] =
+// how many) for the CTA-wide kernel; a row with more than CAP but at most kSortCap candidates to `work2` for the
+// second tier.  FROM_LIST: the rows are those of `rows_in` (rows_in[0] = how many) instead of 0..n-1.
+template <int CAP, bool FROM_LIST>
 __global__ void __launch_bounds__(kMergeWarps * 32) csr_commutator_merge_kernel(CsrRaw A, CsrRaw B, int64_t n,
                                                                                 int32_t* __restrict__ counts,
                                                                                 int32_t* __restrict__ tmp_ci,
-                                                                                cplx* __restrict__ tmp_v, int* work) {
+                                                                                cplx* __restrict__ tmp_v, int* work,
+                                                                                int* work2, const int* rows_in) {
   constexpr bool WRITE = false;
   extern __shared__ __align__(16) unsigned char cm_smem[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  cplx* sval = reinterpret_cast<cplx*>(cm_smem) + warp * kSortCap;
-  unsigned long long* skey = reinterpret_cast<unsigned long long*>(cm_smem + kMergeWarps * kSortCap * sizeof(cplx)) + warp * kSortCap;
-  int* lq = reinterpret_cast<int*>(cm_smem + kMergeWarps * kSortCap * (sizeof(cplx) + sizeof(unsigned long long))) +
+  cplx* sval = reinterpret_cast<cplx*>(cm_smem) + warp * CAP;
+  unsigned long long* skey = reinterpret_cast<unsigned long long*>(cm_smem + kMergeWarps * CAP * sizeof(cplx)) + warp * CAP;
+  int* lq = reinterpret_cast<int*>(cm_smem + kMergeWarps * CAP * (sizeof(cplx) + sizeof(unsigned long long))) +
             warp * 3 * kCommLists;
   int* llen = lq + kCommLists;
   int* lo = llen + kCommLists;
   const int64_t nwarps = (int64_t)gridDim.x * kMergeWarps;
   const bool narrow = n <= ((int64_t)1 << 22);
-  for (int64_t row = (int64_t)blockIdx.x * kMergeWarps + warp; row < n; row += nwarps) {
+  const int64_t nrows_todo = FROM_LIST ? rows_in[0] : n;
+  for (int64_t it = (int64_t)blockIdx.x * kMergeWarps + warp; it < nrows_todo; it += nwarps) {
+    const int64_t row = FROM_LIST ? rows_in[1 + it] : it;
     const int pa = A.rp[row], lenA = A.rp[row + 1] - pa, pb = B.rp[row], lenB = B.rp[row + 1] - pb;
     const int L = lenA + lenB;
     int total = 0;
@@ -623,6 +632,13 @@ __global__ void __launch_bounds__(kMergeWarps * 32) csr_commutator_merge_kernel(
       }
       continue;
     }
+    if (total > CAP) {                                   // warp-uniform: the second tier takes this row
+      if (lane == 0) {
+        counts[row] = 0;
+        work2[1 + atomicAdd(work2, 1)] = (int)row;
+      }
+      continue;
+    }
     __syncwarp();
     for (int t = lane; t < L; t += 32) {                 // 2. expand
       const bool fromA = t < lenA;
@@ -643,10 +659,10 @@ __global__ void __launch_bounds__(kMergeWarps * 32) csr_commutator_merge_kernel(
     // 3. sort the keys: into registers (lane-contiguous), network, back to shared memory.  When column and
     // position fit 32 bits together (n * 1024 <= 2^32) the network runs on 32-bit keys (min / max per exchange).
     if (narrow) {
-      if (total <= 16 * 32) sort_keys<16, unsigned, WRITE>(skey, total, lane);
+      if (CAP <= 16 * 32 || total <= 16 * 32) sort_keys<16, unsigned, WRITE>(skey, total, lane);
       else sort_keys<32, unsigned, WRITE>(skey, total, lane);
     } else {
-      if (total <= 16 * 32) sort_keys<16, unsigned long long, WRITE>(skey, total, lane);
+      if (CAP <= 16 * 32 || total <= 16 * 32) sort_keys<16, unsigned long long, WRITE>(skey, total, lane);
       else sort_keys<32, unsigned long long, WRITE>(skey, total, lane);
     }
     __syncwarp();
@@ -814,6 +830,7 @@ int csr_commutator_build(const CsrRaw& A, const CsrRaw& B, int64_t n, int32_t** 
   int32_t* rp = nullptr;
   int* overflow = nullptr;
   int* work = nullptr;          // [0] = rows left to the CTA-wide kernel, then the rows
+  int* work2 = nullptr;         // the same for the second tier of the warp kernel
   int32_t* tmp_ci = nullptr;
   cplx* tmp_v = nullptr;
   void* tmp = nullptr;
@@ -826,6 +843,7 @@ int csr_commutator_build(const CsrRaw& A, const CsrRaw& B, int64_t n, int32_t** 
       cudaMalloc(&rp, sizeof(int32_t) * (size_t)(n + 1)) != cudaSuccess ||
       cudaMalloc(&overflow, sizeof(int)) != cudaSuccess ||
       cudaMalloc(&work, sizeof(int) * (size_t)(n + 1)) != cudaSuccess ||
+      cudaMalloc(&work2, sizeof(int) * (size_t)(n + 1)) != cudaSuccess ||
       cudaMalloc(&tmp_ci, sizeof(int32_t) * (size_t)n * kCommTmp) != cudaSuccess ||
       cudaMalloc(&tmp_v, sizeof(cplx) * (size_t)n * kCommTmp) != cudaSuccess) {
     cudaGetLastError();
@@ -840,9 +858,16 @@ int csr_commutator_build(const CsrRaw& A, const CsrRaw& B, int64_t n, int32_t** 
   if (rc == MAGNUS_OK) {
     cudaMemsetAsync(overflow, 0, sizeof(int), st);
     cudaMemsetAsync(work, 0, sizeof(int), st);
+    cudaMemsetAsync(work2, 0, sizeof(int), st);
     cudaMemsetAsync(counts + n, 0, sizeof(int32_t), st);
-    cudaFuncSetAttribute(csr_commutator_merge_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMergeSmem);
-    csr_commutator_merge_kernel<<<mgrid, kMergeWarps * 32, kMergeSmem, st>>>(A, B, n, counts, tmp_ci, tmp_v, work);
+    cudaFuncSetAttribute(csr_commutator_merge_kernel<512, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, merge_smem<512>());
+    cudaFuncSetAttribute(csr_commutator_merge_kernel<kSortCap, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                         merge_smem<kSortCap>());
+    csr_commutator_merge_kernel<512, false><<<mgrid, kMergeWarps * 32, merge_smem<512>(), st>>>(A, B, n, counts, tmp_ci, tmp_v,
+                                                                                              work, work2, nullptr);
+    // second tier: its row count is on the device, so the grid is sized for the machine and strides over the list
+    csr_commutator_merge_kernel<kSortCap, true><<<device_sm_count() * 4, kMergeWarps * 32, merge_smem<kSortCap>(), st>>>(
+        A, B, n, counts, tmp_ci, tmp_v, work, work2, work2);
     cudaMemcpyAsync(&h_work, work, sizeof(int), cudaMemcpyDeviceToHost, st);
     if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) rc = MAGNUS_ECUDA;
     grid = (int)(h_work < gmax ? (h_work > 0 ? h_work : 1) : gmax);
@@ -880,6 +905,7 @@ int csr_commutator_build(const CsrRaw& A, const CsrRaw& B, int64_t n, int32_t** 
   cudaFree(counts);
   cudaFree(overflow);
   cudaFree(work);
+  cudaFree(work2);
   cudaFree(tmp_ci);
   cudaFree(tmp_v);
   cudaFree(tmp);
