@@ -297,6 +297,9 @@ int magnus_host_divided_differences(double theta, int m, double* out_host);
 
 /* Widen [a,b] outward to the grid of spacing 2^(ceil(log2(b-a)) - 12) (c4). */
 int magnus_host_snap_interval(double* a, double* b);
+/* Extreme eigenvalues of the symmetric tridiagonal matrix with diagonal alpha[0..k) and off-diagonal beta[0..k-1)
+ * (HOST arrays; Sturm-count bisection): the host piece of MAGNUS_SHORTCUT_TIGHT_INTERVAL (reading ti). */
+int magnus_host_tridiag_extremes(const double* alpha_host, const double* beta_host, int k, double* lo, double* hi);
 
 /* Per-exponential scalars of one step (c1).  coef_h1[e] multiplies H1 in the e-th
  * exponential's matrix, h_scale[e]*tau is its h; for M4 kappa_out receives

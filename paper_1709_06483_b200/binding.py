@@ -73,7 +73,7 @@ DRIVE = C.CFUNCTYPE(C.c_double, C.c_double, C.c_void_p)
 EXPORTS = [
     "magnus_create", "magnus_create_xxz", "magnus_destroy", "magnus_describe", "leja_expmv", "magnus_step", "magnus_integrate", "magnus_integrate_host",
     "magnus_gershgorin", "magnus_leja_iteration", "magnus_zgemm", "magnus_commutator_dense", "magnus_commutator_csr", "magnus_omega_dense",
-    "magnus_fp64_peaks", "magnus_host_leja_points", "magnus_host_divided_differences", "magnus_host_snap_interval",
+    "magnus_fp64_peaks", "magnus_host_leja_points", "magnus_host_divided_differences", "magnus_host_snap_interval", "magnus_host_tridiag_extremes",
     "magnus_host_step_coefficients", "magnus_strerror", "magnus_last_error", "magnus_version",
 ]
 
@@ -123,6 +123,8 @@ def lib():
         L.magnus_host_leja_points.argtypes = [C.c_int, C.c_void_p]
         L.magnus_host_divided_differences.argtypes = [C.c_double, C.c_int, C.c_void_p]
         L.magnus_host_snap_interval.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.magnus_host_tridiag_extremes.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.POINTER(C.c_double),
+                                                   C.POINTER(C.c_double)]
         L.magnus_host_step_coefficients.argtypes = [C.c_int, DRIVE, C.c_void_p, C.c_double, C.c_double,
                                                     C.POINTER(C.c_double), C.POINTER(C.c_double),
                                                     C.POINTER(C.c_double)]
@@ -382,6 +384,16 @@ def magnus_commutator_csr(A, B, stream=None):
         _check(lib().magnus_commutator_csr(Am.ref(), Bm.ref(), nnz.value, C.byref(nnz), _ptr(rp), _ptr(ci), _ptr(v),
                                            _stream_ptr(stream)))
     return rp, ci[:nnz.value], v[:nnz.value]
+
+
+def magnus_host_tridiag_extremes(alpha, beta) -> Tuple[float, float]:
+    """Extreme eigenvalues of tridiag(alpha; beta) (host; the Sturm bisection of the tight-interval shortcut)."""
+    import numpy as np
+    al = np.ascontiguousarray(alpha, dtype=np.float64)
+    be = np.ascontiguousarray(beta if len(al) > 1 else [0.0], dtype=np.float64)
+    lo, hi = C.c_double(), C.c_double()
+    _check(lib().magnus_host_tridiag_extremes(al.ctypes.data, be.ctypes.data, len(al), C.byref(lo), C.byref(hi)))
+    return lo.value, hi.value
 
 
 def magnus_fp64_peaks(stream=None) -> Tuple[float, float]:

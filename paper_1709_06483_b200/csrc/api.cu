@@ -426,9 +426,8 @@ static void csr_op_from_spec(const magnus_context* h, const ExpSpec& sp, CsrOp* 
 
 // the exponentials of one step (S1) for the operators that are a plain combination of stored terms:
 // commutator-free schemes on either format, and M4 on CSR with its cached commutator
-static int step_specs(magnus_context* h, double t, double tau, ExpSpec* out) {
-  double coef[MAGNUS_MAX_EXP_PER_STEP], hscale[MAGNUS_MAX_EXP_PER_STEP], kappa = 0.0;
-  const int n_exp = step_coefficients(h->scheme, h->f, h->user, t, tau, coef, hscale, &kappa);
+static void specs_from_coefficients(const magnus_context* h, int n_exp, const double* coef, const double* hscale, double kappa,
+                                    double tau, ExpSpec* out) {
   for (int e = 0; e < n_exp; ++e) {
     out[e].g = coef[e];
     out[e].kappa = 0.0;
@@ -440,6 +439,12 @@ static int step_specs(magnus_context* h, double t, double tau, ExpSpec* out) {
     out[0].kappa = kappa;
     out[0].nterms = (h->c_nnz > 0 && kappa != 0.0) ? 3 : 2;
   }
+}
+
+static int step_specs(magnus_context* h, double t, double tau, ExpSpec* out) {
+  double coef[MAGNUS_MAX_EXP_PER_STEP], hscale[MAGNUS_MAX_EXP_PER_STEP], kappa = 0.0;
+  const int n_exp = step_coefficients(h->scheme, h->f, h->user, t, tau, coef, hscale, &kappa);
+  specs_from_coefficients(h, n_exp, coef, hscale, kappa, tau, out);
   return n_exp;
 }
 
@@ -704,6 +709,8 @@ static int magnus_step_unplanned(magnus_context* h, double t, double tau, cplx* 
   cudaStream_t st = h->stream;
   Workspace* ws = &h->ws;
   int rc = MAGNUS_OK;
+  ExpSpec specs[MAGNUS_MAX_EXP_PER_STEP];      // the same scalars in the form the CSR operator takes them
+  specs_from_coefficients(h, n_exp, coef, hscale, kappa, tau, specs);
   for (int e = 0; e < n_exp && rc == MAGNUS_OK; ++e) {
     OpRef op;
     double a = 0.0, b = 0.0;
@@ -717,27 +724,7 @@ static int magnus_step_unplanned(magnus_context* h, double t, double tau, cplx* 
       xxz_gershgorin(op.xx, &a, &b);
     } else if (h->format == MAGNUS_CSR) {
       op.dense = false;
-      op.csr.n = h->n;
-      if (h->scheme == MAGNUS_M4) {
-        // Omega_H = H0 + fbar H1 - i kappa [H0, H1]   (c1; [H(t2),H(t1)] = (f1 - f2)[H0,H1])
-        op.csr.nterms = (h->c_nnz > 0 && kappa != 0.0) ? 3 : 2;
-        op.csr.t[0] = csr_term(&h->H0, 1.0, 0.0);
-        op.csr.t[1] = csr_term(&h->H1, 0.5 * (coef[0] + coef[1]), 0.0);
-        CsrTerm c;
-        c.rp = h->c_rp;
-        c.ci = h->c_ci;
-        c.v = h->c_v;
-        c.coef = make_double2(0.0, -kappa);
-        c.nnz = h->c_nnz;
-        op.csr.t[2] = c;
-      } else {
-        op.csr.nterms = 2;
-        op.csr.t[0] = csr_term(&h->H0, 1.0, 0.0);
-        op.csr.t[1] = csr_term(&h->H1, coef[e], 0.0);
-        op.csr.t[2] = op.csr.t[1];
-      }
-      op.csr.unit_cap = op.csr.nterms == 3 ? h->unit_cap3 : h->unit_cap2;
-      op.csr.slice = h->slice.meta ? &h->slice : nullptr;
+      csr_op_from_spec(h, specs[e], &op.csr);     // S2: the terms with this exponential's coefficients (M4: c1, g12)
       if ((op.csr.nterms == 2 && h->gs_disjoint2) || (op.csr.nterms == 3 && h->gs_disjoint3)) {     // S3
         const int nblk = launch_csr_gershgorin_cached(op.csr, h->gs_r, h->gs_diag, ws, st);
         rc = read_interval(nblk, ws, st, &a, &b);
@@ -864,6 +851,12 @@ int magnus_host_snap_interval(double* a, double* b) {
   return MAGNUS_OK;
 }
 
+int magnus_host_tridiag_extremes(const double* alpha_host, const double* beta_host, int k, double* lo, double* hi) {
+  if (!alpha_host || (k > 1 && !beta_host) || k < 1 || !lo || !hi) { set_error("magnus_host_tridiag_extremes: bad arguments"); return MAGNUS_EINVAL; }
+  tridiag_extreme_eigenvalues(alpha_host, beta_host, k, lo, hi);
+  return MAGNUS_OK;
+}
+
 int magnus_host_step_coefficients(int scheme, magnus_drive_fn f, void* user, double t, double tau, double* coef_h1,
                                   double* h_scale, double* kappa_out) {
   if (!f || !coef_h1 || !h_scale) return MAGNUS_EINVAL;
@@ -912,7 +905,7 @@ int magnus_describe(magnus_handle h, magnus_path_info* out) {
     out->csr_bytes_per_iteration = 20 * (n * (3 * N + 2) / 2) + 4 * (n + 1) * 2 + 64 * n;
   } else if (h->format == MAGNUS_DENSE) {
     out->bytes_per_iteration = 16 * n * n + 64 * n;
-    if (plan_supported(h)) name = "dense_leja_sweep_kernel";
+    if (dense_sweep_supported(n) && h->ws.csr_kernel == 0) name = "dense_leja_sweep_kernel";
   } else {
     int64_t nnz = h->H0.nnz + h->H1.nnz, terms = 2;
     if (h->scheme == MAGNUS_M4 && h->c_nnz > 0) {

@@ -180,3 +180,20 @@ def test_bad_arguments_are_rejected_before_any_cuda_call(M):
         M.magnus_host_leja_points(500)
     with pytest.raises(M.MagnusError):
         M.magnus_host_divided_differences(1.0, 0)
+
+
+def test_tridiag_extremes_against_numpy(M):
+    """The host piece of the tight-interval shortcut (Sturm bisection) against numpy.linalg.eigvalsh: random
+    tridiagonals, k = 1, a zero off-diagonal (decoupled blocks), equal eigenvalues, huge and tiny scales."""
+    r = np.random.default_rng(7)
+    cases = [(r.normal(size=k), np.abs(r.normal(size=k - 1))) for k in (2, 3, 8, 12, 40, 64)]
+    cases += [(np.array([2.5]), np.array([])), (np.array([1.0, -3.0, 2.0]), np.array([0.0, 0.5])),
+              (np.ones(6), np.zeros(5)), (1e150 * r.normal(size=5), 1e150 * np.abs(r.normal(size=4))),
+              (1e-150 * r.normal(size=5), 1e-150 * np.abs(r.normal(size=4)))]
+    for al, be in cases:
+        k = len(al)
+        T = np.diag(al) + (np.diag(be, 1) + np.diag(be, -1) if k > 1 else 0.0)
+        ev = np.linalg.eigvalsh(T)
+        lo, hi = M.magnus_host_tridiag_extremes(al, be)
+        scale = max(np.max(np.abs(al)), np.max(np.abs(be)) if k > 1 else 0.0)
+        assert abs(lo - ev[0]) <= 1e-13 * scale and abs(hi - ev[-1]) <= 1e-13 * scale, (al, be, lo, hi, ev[0], ev[-1])
