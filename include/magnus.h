@@ -79,15 +79,16 @@ typedef struct magnus_options {
   int32_t m_max;       /* maximal interpolation degree per sub-step (c6); default and maximum 128 */
   int32_t check_hermitian; /* 1: sampled check in magnus_create (costs a device pass); default 0 */
   void* stream;        /* cudaStream_t; NULL = legacy default stream */
-  int32_t csr_kernel;  /* 0 auto: n <= 4096 (CSR) / n <= 4096 (dense): whole sweeps per launch and steps planned ahead
-                          (magnus_step, below); CSR n >= 32768: a handle re-stores the operator once in the offset-slot
+  int32_t csr_kernel;  /* 0 auto: CSR n <= 65536 (an 8-CTA cluster up to n = 1024, a cooperative grid above) / dense n <= 4096:
+                          whole sweeps per launch and steps planned ahead (magnus_step, below); CSR n > 65536: a handle re-stores the operator once in the offset-slot
                           layout (kernels_csr_slice.cu: 16 B per entry + 8 B per slot, no column array; kept if a slot
                           holds >= 8 entries on average, about 50% more device memory than the caller's CSR) and runs the
                           slice kernel, else the row-block kernel; in between the generic kernel.
                           Non-zero values force a per-iteration kernel and the stepwise control flow:
                           1 generic, 2 row-block, 3 warp-specialised TMA ring, 4 row-block with TMA staging (3 and 4 need
                           16-byte aligned value and index arrays, else the row-block kernel runs), 5 slices with a
-                          column array, 6 offset-slot slices; values >= 1000 select tuning variants (kernel sources) */
+                          column array, 6 offset-slot slices; 7 forces the cooperative whole-sweep kernel (n <= 65536);
+                          values >= 1000 select tuning variants (kernel sources) */
   int32_t shortcuts;   /* bit mask of beyond-paper shortcuts, default 0 = the mandated path only:
                           MAGNUS_SHORTCUT_CACHED_COMMUTATOR (dense M4), MAGNUS_SHORTCUT_TIGHT_INTERVAL */
   int32_t lanczos_steps; /* MAGNUS_SHORTCUT_TIGHT_INTERVAL: Lanczos steps per exponential; default 8, at most 64 */

@@ -181,9 +181,10 @@ static int expmv_on_interval(const OpRef& op, double a_raw, double b_raw, const 
   const double inv_gamma = 1.0 / gamma, c_over_gamma = c / gamma;
   const cplx phase = make_double2(std::cos(hs * c), -std::sin(hs * c));
   float ms = 0.f;
-  const bool small_csr = !op.xxz && !op.dense && n <= kSmallSweepMaxN && ws->csr_kernel == 0;
+  const bool mid_csr = !op.xxz && !op.dense && csr_mid_sweep_supported(n, ws->csr_kernel);
+  const bool small_csr = !op.xxz && !op.dense && n <= kSmallSweepMaxN && ws->csr_kernel == 0 && !mid_csr;
   const bool mid_dense = !op.xxz && op.dense && dense_sweep_supported(n) && op.dns.ld == n && ws->csr_kernel == 0;
-  if (small_csr || mid_dense) {
+  if (small_csr || mid_dense || mid_csr) {
     // small CSR / medium dense problem: each sub-step sweep is ONE launch (kernels_csr_small.cu,
     // kernels_dense_sweep.cu) on an already assembled operator; the table first covers `have` terms and is
     // extended only if the sweep asks for more
@@ -201,6 +202,8 @@ static int expmv_on_interval(const OpRef& op, double a_raw, double b_raw, const 
         if (ws->time_leja) CU_TRY(cudaEventRecord(ws->ev[0], st));
         const int lrc = small_csr ? launch_csr_leja_sweep_small(op.csr, src, v_out, inv_gamma, c_over_gamma, prm.tol, m_try,
                                                                 phase, tab, ws, st)
+                        : mid_csr ? launch_csr_leja_sweep_mid(op.csr, src, v_out, inv_gamma, c_over_gamma, prm.tol, m_try, phase,
+                                                              tab, ws, st)
                                   : launch_dense_leja_sweep(op.dns, src, v_out, inv_gamma, c_over_gamma, prm.tol, m_try,
                                                             phase, tab, ws, st);
         if (lrc) {
@@ -450,7 +453,8 @@ static int step_specs(magnus_context* h, double t, double tau, ExpSpec* out) {
 
 static bool plan_supported(const magnus_context* h) {
   if (h->is_xxz || (h->shortcuts & MAGNUS_SHORTCUT_TIGHT_INTERVAL)) return false;   // the interval depends on psi
-  if (h->format == MAGNUS_CSR) return h->n <= kSmallSweepMaxN && h->ws.csr_kernel == 0;
+  if (h->format == MAGNUS_CSR)
+    return (h->n <= kSmallSweepMaxN && h->ws.csr_kernel == 0) || csr_mid_sweep_supported(h->n, h->ws.csr_kernel);
   // dense: the commutator-free schemes (M = H0 + g H1 per exponential); M4 / M6 build Omega_H per step
   return h->scheme != MAGNUS_M4 && h->scheme != MAGNUS_M6 && dense_sweep_supported(h->n) && h->ws.csr_kernel == 0;
 }
@@ -608,8 +612,11 @@ static int run_planned(magnus_context* h, double t0, double tau, int64_t s0, int
       const LejaStatus* gate = e_next > seg ? ws->status_arr + e_next - 1 : nullptr;
       const int lrc = dense ? launch_dense_leja_sweep_jobs(h->n, H0v, dense_ld(&h->H0), H1v, dense_ld(&h->H1), h->M, psi, jd,
                                                            nj, h->prm.tol, ws->status_arr + e_next, gate, ws, st)
-                            : launch_csr_leja_sweep_small_jobs(op_all, psi, jd, nj, ws->leja_l, h->prm.tol,
-                                                               ws->status_arr + e_next, gate, ws, st);
+                      : !csr_mid_sweep_supported(h->n, ws->csr_kernel)
+                          ? launch_csr_leja_sweep_small_jobs(op_all, psi, jd, nj, ws->leja_l, h->prm.tol,
+                                                             ws->status_arr + e_next, gate, ws, st)
+                          : launch_csr_leja_sweep_mid_jobs(op_all, psi, jd, nj, h->prm.tol, ws->status_arr + e_next, gate,
+                                                           ws, st);
       if (lrc != MAGNUS_OK) {
         set_error("whole-sweep launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         return MAGNUS_ECUDA;
@@ -915,7 +922,9 @@ int magnus_describe(magnus_handle h, magnus_path_info* out) {
     out->csr_bytes_per_iteration = 20 * nnz + 4 * (n + 1) * terms + 64 * n;
     out->bytes_per_iteration = out->csr_bytes_per_iteration;
     const int k = h->ws.csr_kernel;
-    if (n <= kSmallSweepMaxN && k == 0) {
+    if (csr_mid_sweep_supported(n, k)) {
+      name = "csr_leja_sweep_mid_kernel";
+    } else if (n <= kSmallSweepMaxN && k == 0) {
       name = "csr_leja_sweep_small_kernel";
     } else if (h->slice.meta && (k == 0 || slice_layout_kind(k) != 0)) {
       out->slices = h->slice.nslices;
@@ -1060,7 +1069,7 @@ int magnus_create(magnus_handle* out, const magnus_matrix* H0, const magnus_matr
     // slice-major copy of the operator: asked for explicitly, or by default for large n when its slots are
     // well filled (spin chains: about 20 entries per slot); otherwise the CSR kernels run
     const int kind = slice_layout_kind(csr_kernel);
-    if (kind != 0 || (csr_kernel == 0 && h->n >= kSliceAutoMinN)) {
+    if (kind != 0 || (csr_kernel == 0 && h->n >= kSliceAutoMinN && !csr_mid_sweep_supported(h->n, csr_kernel))) {
       CsrOp op;
       op.n = h->n;
       op.unit_cap = 0;

@@ -155,5 +155,27 @@ __device__ __forceinline__ void block_reduce_minmax(double& lo, double& hi) {
   __syncthreads();
 }
 
+// ---- grid barrier of the persistent (cooperative, all CTAs resident) sweep kernels ----
+__device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
+  unsigned v;
+  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+
+// All CTAs of the (cooperative, co-resident) grid meet here; everything written before is visible after.
+__device__ __forceinline__ void grid_barrier(unsigned* counter, unsigned& generation) {
+  __syncthreads();
+  generation += 1;
+  if (threadIdx.x == 0) {
+    const unsigned target = generation * gridDim.x;
+    __threadfence();
+    atomicAdd(counter, 1u);
+    while (ld_acquire_u32(counter) < target) {
+    }
+    __threadfence();
+  }
+  __syncthreads();
+}
+
 }  // namespace magnus
 #endif

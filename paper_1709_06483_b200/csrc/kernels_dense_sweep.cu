@@ -28,27 +28,6 @@ constexpr int DS_MAX_ROWS = 32;                 // rows per CTA
 constexpr int DS_RG = 7;                        // rows in flight together
 constexpr int DS_SMEM = kDenseSweepMaxN * (int)sizeof(cplx);   // the vector w
 
-__device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
-  unsigned v;
-  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-  return v;
-}
-
-// All CTAs of the (cooperative, co-resident) grid meet here; everything written before is visible after.
-__device__ __forceinline__ void grid_barrier(unsigned* counter, unsigned& generation) {
-  __syncthreads();
-  generation += 1;
-  if (threadIdx.x == 0) {
-    const unsigned target = generation * gridDim.x;
-    __threadfence();
-    atomicAdd(counter, 1u);
-    while (ld_acquire_u32(counter) < target) {
-    }
-    __threadfence();
-  }
-  __syncthreads();
-}
-
 __device__ __forceinline__ cplx ldcg_cplx(const cplx* p) {
   const double2 v = __ldcg(reinterpret_cast<const double2*>(p));
   return v;

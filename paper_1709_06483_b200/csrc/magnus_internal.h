@@ -89,6 +89,8 @@ struct LejaStatus {
 
 // Small CSR problems run a whole Leja sweep in one launch of an 8-CTA cluster (kernels_csr_small.cu).
 const int kSmallSweepMaxN = 4096;
+const int kMidSweepMaxN = 65536;    // CSR problems up to this n run whole sweeps in one cooperative launch (kernels_csr_mid.cu)
+const int kMidSweepMinN = 1024;     // ... above this n (up to it the 8-CTA cluster kernel is faster; csr_kernel 7 forces the cooperative one)
 const int kDenseSweepMaxN = 4096;   // dense problems up to this n run whole sweeps in one cooperative launch
 struct SweepTable {
   cplx d[kMaxDegree + 1];     // divided differences d_k (c3)
@@ -238,6 +240,13 @@ int launch_csr_leja_sweep_small(const CsrOp& op, const cplx* v, cplx* out, doubl
 int launch_csr_leja_sweep_small_jobs(const CsrOp& op, cplx* psi, const SweepJob* jobs, int njobs, const double* leja_l,
                                       double tol, LejaStatus* status, const LejaStatus* gate, Workspace* ws,
                                       cudaStream_t st);
+
+// ---- kernels_csr_mid.cu -----------------------------------------------------
+bool csr_mid_sweep_supported(int64_t n, int csr_kernel);   // csr_kernel 0: by size; 7: forced (any n <= kMidSweepMaxN)
+int launch_csr_leja_sweep_mid_jobs(const CsrOp& op, cplx* psi, const SweepJob* jobs, int njobs, double tol,
+                                   LejaStatus* status, const LejaStatus* gate, Workspace* ws, cudaStream_t st);
+int launch_csr_leja_sweep_mid(const CsrOp& op, const cplx* v, cplx* out, double inv_gamma, double c_over_gamma, double tol,
+                              int m_max, cplx phase, const SweepTable& tab, Workspace* ws, cudaStream_t st);
 
 // ---- kernels_dense.cu -------------------------------------------------------
 int launch_dense_gershgorin(const DenseOp& op, Workspace* ws, cudaStream_t st);

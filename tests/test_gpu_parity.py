@@ -753,3 +753,56 @@ def test_shortcut_tight_interval_vs_oracle(M, oracle, name, size, nsteps, scheme
             st2 = h.integrate(cfg.t0, cfg.t_end, cfg.nsteps, psi2)
         assert st["total_matvecs"] < st2["total_matvecs"]
         assert relerr(host(psi), host(psi2)) <= 1e-9           # two intervals, one exponential
+
+
+# ------------------------------------------------------------------ medium CSR: cooperative whole-sweep kernel
+@pytest.mark.parametrize("scheme", ["cf4", "m4"])
+@pytest.mark.parametrize("N,nsteps", [(11, 4), (13, 3), (15, 2), (16, 1)])
+def test_medium_csr_sweep_kernel(M, oracle, scheme, N, nsteps):
+    """1024 < n <= 65536: planned batches on the persistent cooperative CSR sweep kernel (rows partitioned over the SMs,
+    w through L2 with one grid barrier per iteration).  Against the oracle (counts equal, psi <= 1e-9) and against the
+    per-iteration kernels of the stepwise path (csr_kernel = 1)."""
+    cfg = W.scaled(W.CONFIGS["cfg3"], N, nsteps)
+    H0, H1, psi0, f = W.build(cfg)
+    ref, riters = oracle.magnus_integrate(oracle.CsrHost.of(H0), oracle.CsrHost.of(H1), f, scheme, cfg.t0, cfg.t_end,
+                                          cfg.nsteps, psi0.numpy(), cfg.tol)
+    res = {}
+    for ck in (0, 1):
+        psi = psi0.to(DEV).clone()
+        with M.magnus_create(H0.to(DEV), H1.to(DEV), f, scheme, tol=cfg.tol, csr_kernel=ck) as h:
+            if ck == 0:
+                assert h.describe()["leja_kernel"] == "csr_leja_sweep_mid_kernel"
+            st = h.integrate(cfg.t0, cfg.t_end, cfg.nsteps, psi)
+        assert np.array_equal(st["iters"], riters) and relerr(host(psi), ref) <= 1e-9
+        res[ck] = host(psi)
+    assert relerr(res[0], res[1]) <= 1e-13
+    if N == 11:      # forced on a size the cluster kernel would take, and the cluster kernel forced... by size: N = 10
+        cfg10 = W.scaled(W.CONFIGS["cfg1"], 10, 6)
+        H0, H1, psi0, f = W.build(cfg10)
+        out = {}
+        for ck in (0, 7):
+            psi = psi0.to(DEV).clone()
+            with M.magnus_create(H0.to(DEV), H1.to(DEV), f, scheme, tol=cfg10.tol, csr_kernel=ck) as h:
+                assert h.describe()["leja_kernel"] == ("csr_leja_sweep_mid_kernel" if ck == 7 else "csr_leja_sweep_small_kernel")
+                st = h.integrate(cfg10.t0, cfg10.t_end, cfg10.nsteps, psi)
+            out[ck] = (st["iters"], host(psi))
+        assert np.array_equal(out[0][0], out[7][0]) and relerr(out[0][1], out[7][1]) <= 1e-13
+
+
+def test_medium_csr_sweep_general_matrix_and_expmv(M, oracle):
+    """The same kernel on a general (non-XXZ) Hermitian CSR matrix with empty and long rows, through leja_expmv
+    (one-job launch, out != in), and its non-convergence report (input untouched when in place)."""
+    n = 9001
+    S = random_sparse_hermitian(n, 0.0006, 9, long_row=(17, 1500))
+    Mh = oracle.CsrHost(n, S.indptr.astype(np.int32), S.indices.astype(np.int32), S.data.astype(complex))
+    v = rand_vec(n, 41)
+    ref, rinfo = oracle.leja_expmv(Mh, v, 0.02, 1e-12)
+    vi = torch.from_numpy(v).to(DEV)
+    vo = torch.empty_like(vi)
+    info = M.leja_expmv(csr_from_scipy(S), vi, vo, 0.02, 1e-12)
+    assert info["iters"] == rinfo["iters"] and info["a"] == rinfo["a"] and info["b"] == rinfo["b"]
+    assert relerr(host(vo), ref) <= 1e-12 and torch.equal(vi, torch.from_numpy(v).to(DEV))
+    keep = vi.clone()
+    with pytest.raises(M.MagnusError) as e:
+        M.leja_expmv(csr_from_scipy(S), vi, vi, 3.0, 1e-300)
+    assert e.value.code == -4 and torch.equal(vi, keep)
