@@ -467,7 +467,7 @@ const int kPlanDeclined = 1;   // internal: not a planned-path handle after all
 static int run_planned(magnus_context* h, double t0, double tau, int64_t s0, int ns, cplx* psi, magnus_step_info* infos) {
   Workspace* ws = &h->ws;
   cudaStream_t st = h->stream;
-  if (ensure_sweep_jobs(ws) != MAGNUS_OK) { set_error("planned batch: buffer allocation failed"); return MAGNUS_ENOMEM; }
+  if (ensure_sweep_jobs(ws, st) != MAGNUS_OK) { set_error("planned batch: buffer allocation failed"); return MAGNUS_ENOMEM; }
   std::vector<ExpSpec> specs;
   std::vector<int> first_of_step((size_t)ns + 1, 0);
   for (int s = 0; s < ns; ++s) {
@@ -977,7 +977,7 @@ int magnus_create(magnus_handle* out, const magnus_matrix* H0, const magnus_matr
   default_params(opt, &h->prm, &h->stream, &h->ws.csr_kernel, &h->shortcuts);
   h->lanczos_steps = (opt && opt->lanczos_steps > 0) ? std::min(64, opt->lanczos_steps) : 8;
   const int csr_kernel = h->ws.csr_kernel;
-  rc = workspace_alloc(&h->ws, h->n);
+  rc = workspace_alloc(&h->ws, h->n, h->stream);
   h->ws.csr_kernel = csr_kernel;
   h->ws.time_leja = true;
   if (rc) { set_error("workspace allocation failed (n=%lld)", (long long)h->n); magnus_destroy(h); return rc; }
@@ -1119,7 +1119,7 @@ int magnus_create_xxz(magnus_handle* out, const magnus_xxz_model* model, magnus_
   h->user = user;
   default_params(opt, &h->prm, &h->stream, &h->ws.csr_kernel, &h->shortcuts);
   h->lanczos_steps = (opt && opt->lanczos_steps > 0) ? std::min(64, opt->lanczos_steps) : 8;
-  rc = workspace_alloc(&h->ws, h->n);
+  rc = workspace_alloc(&h->ws, h->n, h->stream);
   h->ws.csr_kernel = 1;       // no whole-sweep kernels on this path
   h->ws.time_leja = true;
   if (rc) { set_error("workspace allocation failed (n=%lld)", (long long)h->n); magnus_destroy(h); return rc; }
@@ -1206,7 +1206,7 @@ int leja_expmv(const magnus_matrix* H, const void* v_in, void* v_out, double h, 
   prm.theta_max = 16.0;
   prm.m_max = kMaxDegree;
   Workspace ws;
-  rc = workspace_alloc(&ws, H->n);
+  rc = workspace_alloc(&ws, H->n, st);
   if (rc) { cudaGetLastError(); workspace_free(&ws); set_error("leja_expmv: workspace allocation failed"); return rc; }
   OpRef op;
   if (H->format == MAGNUS_CSR) {
@@ -1347,7 +1347,7 @@ int magnus_gershgorin(const magnus_matrix* H0, const magnus_matrix* H1, double g
   if (rc) return rc;
   cudaStream_t st = (cudaStream_t)stream;
   Workspace ws;
-  rc = workspace_alloc(&ws, 1);
+  rc = workspace_alloc(&ws, 1, st);
   if (rc) { workspace_free(&ws); return rc; }
   OpRef op;
   cplx* tmp = nullptr;
@@ -1373,7 +1373,7 @@ int magnus_leja_iteration(const magnus_matrix* H0, const magnus_matrix* H1, doub
   if (rc) return rc;
   cudaStream_t st = (cudaStream_t)stream;
   Workspace ws;
-  rc = workspace_alloc(&ws, 1);
+  rc = workspace_alloc(&ws, 1, st);
   if (rc) { workspace_free(&ws); return rc; }
   ws.csr_kernel = csr_kernel;
   OpRef op;
@@ -1468,7 +1468,7 @@ int magnus_omega_dense(int64_t n, const void* H0, int64_t ld0, const void* H1, i
   if (rc) return rc;
   cudaStream_t st = (cudaStream_t)stream;
   Workspace ws;
-  rc = workspace_alloc(&ws, 1);
+  rc = workspace_alloc(&ws, 1, st);
   if (rc) { workspace_free(&ws); return rc; }
   // the same three launches magnus_step makes for M4 on dense H: S2 (A1, A2), D3 (P = A2 A1), D4 + S3
   launch_dense_assemble2(n, (const cplx*)H0, ld0, (const cplx*)H1, ld1, f1, f2, (cplx*)Omega, (cplx*)work_a2, &ws, st);

@@ -71,7 +71,7 @@ void launch_leja_finish(const cplx* p, cplx* out, int64_t n, cplx phase, cudaStr
   launch_scale_copy(p, out, n, phase, st, ws);
 }
 
-int workspace_alloc(Workspace* ws, int64_t n) {
+int workspace_alloc(Workspace* ws, int64_t n, cudaStream_t st) {
   ws->n = n;
   const size_t vb = sizeof(cplx) * (size_t)n;
   if (cudaMalloc(&ws->w[0], vb) != cudaSuccess) return MAGNUS_ENOMEM;
@@ -81,7 +81,8 @@ int workspace_alloc(Workspace* ws, int64_t n) {
   if (cudaMalloc(&ws->gersh, sizeof(double) * (2 * kMaxPartials + 2)) != cudaSuccess) return MAGNUS_ENOMEM;
   if (cudaMalloc(&ws->status, sizeof(LejaStatus)) != cudaSuccess) return MAGNUS_ENOMEM;
   if (cudaMalloc(&ws->tickets, 2 * sizeof(unsigned)) != cudaSuccess) return MAGNUS_ENOMEM;
-  if (cudaMemset(ws->tickets, 0, 2 * sizeof(unsigned)) != cudaSuccess) return MAGNUS_ECUDA;
+  // on the caller's stream: a legacy-stream memset would not be ordered before kernels on a non-blocking stream
+  if (cudaMemsetAsync(ws->tickets, 0, 2 * sizeof(unsigned), st) != cudaSuccess) return MAGNUS_ECUDA;
   if (cudaMallocHost(&ws->status_host, sizeof(LejaStatus)) != cudaSuccess) return MAGNUS_ENOMEM;
   if (cudaMallocHost(&ws->ab_host, 2 * sizeof(double)) != cudaSuccess) return MAGNUS_ENOMEM;
   for (int i = 0; i < 4; ++i)
@@ -110,7 +111,7 @@ struct PlanLayout {
 };
 }  // namespace
 
-int ensure_sweep_jobs(Workspace* ws) {
+int ensure_sweep_jobs(Workspace* ws, cudaStream_t st) {
   if (ws->jobs) return MAGNUS_OK;
   const PlanLayout L;
   char* dev = nullptr;
@@ -118,8 +119,8 @@ int ensure_sweep_jobs(Workspace* ws) {
   bool ok = cudaMalloc(&dev, L.total_dev) == cudaSuccess && cudaMallocHost(&host, L.total_host) == cudaSuccess;
   for (int i = 0; ok && i < 2 * kJobRing; ++i) ok = cudaEventCreate(&ws->ring_ev[i]) == cudaSuccess;
   if (ok)
-    ok = cudaMemset(dev + L.bar, 0, 256) == cudaSuccess &&
-         cudaMemcpy(dev + L.leja, leja_points(), sizeof(double) * (kMaxDegree + 1), cudaMemcpyHostToDevice) == cudaSuccess;
+    ok = cudaMemsetAsync(dev + L.bar, 0, 256, st) == cudaSuccess &&      // leja_points() is a process-lifetime table
+         cudaMemcpyAsync(dev + L.leja, leja_points(), sizeof(double) * (kMaxDegree + 1), cudaMemcpyHostToDevice, st) == cudaSuccess;
   if (!ok) {
     cudaGetLastError();
     cudaFree(dev);

@@ -192,7 +192,7 @@ bool csr_mid_sweep_supported(int64_t n, int csr_kernel) {
 // jobs[0..njobs) applied to psi in order, one cooperative launch; protocol of launch_csr_leja_sweep_small_jobs
 int launch_csr_leja_sweep_mid_jobs(const CsrOp& op, cplx* psi, const SweepJob* jobs, int njobs, double tol,
                                    LejaStatus* status, const LejaStatus* gate, Workspace* ws, cudaStream_t st) {
-  if (ensure_sweep_jobs(ws) != MAGNUS_OK) return MAGNUS_ENOMEM;
+  if (ensure_sweep_jobs(ws, st) != MAGNUS_OK) return MAGNUS_ENOMEM;
   if (cudaMemsetAsync(ws->grid_bar, 0, sizeof(unsigned), st) != cudaSuccess) return MAGNUS_ECUDA;
   CsrOp opv = op;
   const double* leja_l = ws->leja_l;
@@ -212,7 +212,7 @@ int launch_csr_leja_sweep_mid_jobs(const CsrOp& op, cplx* psi, const SweepJob* j
 // one sweep (leja_expmv, sub-steps, the fall-back after a failed batch): a one-job batch through job slot 0
 int launch_csr_leja_sweep_mid(const CsrOp& op, const cplx* v, cplx* out, double inv_gamma, double c_over_gamma, double tol,
                               int m_max, cplx phase, const SweepTable& tab, Workspace* ws, cudaStream_t st) {
-  if (ensure_sweep_jobs(ws) != MAGNUS_OK) return MAGNUS_ENOMEM;
+  if (ensure_sweep_jobs(ws, st) != MAGNUS_OK) return MAGNUS_ENOMEM;
   SweepJob& J = ws->jobs_host[0];
   for (int t = 0; t < 3; ++t) J.coef[t] = op.t[t].coef;
   J.phase = phase;

@@ -264,7 +264,7 @@ int launch_csr_leja_sweep_small_jobs(const CsrOp& op, cplx* psi, const SweepJob*
 int launch_csr_leja_sweep_small(const CsrOp& op, const cplx* v, cplx* out, double inv_gamma, double c_over_gamma,
                                 double tol, int m_max, cplx phase, const SweepTable& tab, Workspace* ws,
                                 cudaStream_t st) {
-  if (ensure_sweep_jobs(ws) != MAGNUS_OK) return MAGNUS_ENOMEM;
+  if (ensure_sweep_jobs(ws, st) != MAGNUS_OK) return MAGNUS_ENOMEM;
   SweepJob& J = ws->jobs_host[0];
   for (int t = 0; t < 3; ++t) J.coef[t] = op.t[t].coef;
   J.phase = phase;

@@ -228,7 +228,7 @@ bool dense_sweep_supported(int64_t n) {
 int launch_dense_leja_sweep_jobs(int64_t n, const cplx* H0, int64_t ld0, const cplx* H1, int64_t ld1, cplx* M, cplx* psi,
                                  const SweepJob* jobs, int njobs, double tol, LejaStatus* status, const LejaStatus* gate,
                                  Workspace* ws, cudaStream_t st) {
-  if (ensure_sweep_jobs(ws) != MAGNUS_OK) return MAGNUS_ENOMEM;
+  if (ensure_sweep_jobs(ws, st) != MAGNUS_OK) return MAGNUS_ENOMEM;
   if (cudaFuncSetAttribute(dense_leja_sweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, DS_SMEM) != cudaSuccess)
     return MAGNUS_ECUDA;
   if (cudaMemsetAsync(ws->grid_bar, 0, sizeof(unsigned), st) != cudaSuccess) return MAGNUS_ECUDA;
@@ -253,7 +253,7 @@ int launch_dense_leja_sweep_jobs(int64_t n, const cplx* H0, int64_t ld0, const c
 // not converge leaves out as that copy.
 int launch_dense_leja_sweep(const DenseOp& op, const cplx* v, cplx* out, double inv_gamma, double c_over_gamma,
                             double tol, int m_max, cplx phase, const SweepTable& tab, Workspace* ws, cudaStream_t st) {
-  if (ensure_sweep_jobs(ws) != MAGNUS_OK) return MAGNUS_ENOMEM;
+  if (ensure_sweep_jobs(ws, st) != MAGNUS_OK) return MAGNUS_ENOMEM;
   SweepJob& J = ws->jobs_host[0];
   J.coef[0] = J.coef[1] = J.coef[2] = make_double2(0.0, 0.0);
   J.phase = phase;

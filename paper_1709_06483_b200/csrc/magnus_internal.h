@@ -151,12 +151,12 @@ struct Workspace {
 };
 // where the Gershgorin kernels put their final (min, max): the slot the planner set, else the workspace's own
 inline double* gersh_final(const Workspace* ws) { return ws->ab_out ? ws->ab_out : ws->gersh + 2 * kMaxPartials; }
-int ensure_sweep_jobs(Workspace* ws);
+int ensure_sweep_jobs(Workspace* ws, cudaStream_t st);   // its initialisation is enqueued on st
 
 // cudaDevAttrMultiProcessorCount of the current device (cached per device; 148 on B200)
 int device_sm_count();
 
-int workspace_alloc(Workspace* ws, int64_t n);
+int workspace_alloc(Workspace* ws, int64_t n, cudaStream_t st);   // its initialisation is enqueued on st
 void workspace_free(Workspace* ws);
 
 struct LejaParams {

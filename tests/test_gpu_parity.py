@@ -806,3 +806,29 @@ def test_medium_csr_sweep_general_matrix_and_expmv(M, oracle):
     with pytest.raises(M.MagnusError) as e:
         M.leja_expmv(csr_from_scipy(S), vi, vi, 3.0, 1e-300)
     assert e.value.code == -4 and torch.equal(vi, keep)
+
+
+def test_runs_on_a_non_blocking_side_stream(M):
+    """Everything a handle enqueues (workspace initialisation, layouts, interval kernels, job uploads, sweeps) is
+    ordered on the caller's stream -- also a torch side stream, which does not synchronise with the legacy default
+    stream.  Same bits as on the default stream (the path is deterministic), for the cluster kernel, the cooperative
+    CSR and dense sweep kernels and the per-iteration kernels."""
+    cases = [("cfg1", 10, 8, "cf4"), ("cfg1", 10, 8, "m4"), ("cfg3", 13, 3, "cf4"), ("cfg2", 300, 4, "cf4"),
+             ("cfg2", 300, 3, "m4"), ("cfg3", 18, 2, "cf4")]
+    side = torch.cuda.Stream()
+    for name, size, nsteps, scheme in cases:
+        cfg = W.scaled(W.CONFIGS[name], size, nsteps)
+        H0, H1, psi0, f = W.build(cfg)
+        d0, d1 = H0.to(DEV), H1.to(DEV)
+        ref = psi0.to(DEV).clone()
+        with M.magnus_create(d0, d1, f, scheme, tol=cfg.tol) as h:
+            st0 = h.integrate(cfg.t0, cfg.t_end, cfg.nsteps, ref)
+        torch.cuda.synchronize()
+        with torch.cuda.stream(side):
+            psi = psi0.to(DEV).clone()
+            side.synchronize()
+            for rep in range(3):                      # fresh handles: their initialisation must not race the first launch
+                psi.copy_(psi0.to(DEV))
+                with M.magnus_create(d0, d1, f, scheme, tol=cfg.tol, stream=side) as h:
+                    st1 = h.integrate(cfg.t0, cfg.t_end, cfg.nsteps, psi)
+                assert np.array_equal(st0["iters"], st1["iters"]) and torch.equal(psi, ref), (name, size, scheme, rep)
