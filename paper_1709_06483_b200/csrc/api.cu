@@ -1120,7 +1120,7 @@ int magnus_create_xxz(magnus_handle* out, const magnus_xxz_model* model, magnus_
   default_params(opt, &h->prm, &h->stream, &h->ws.csr_kernel, &h->shortcuts);
   h->lanczos_steps = (opt && opt->lanczos_steps > 0) ? std::min(64, opt->lanczos_steps) : 8;
   rc = workspace_alloc(&h->ws, h->n, h->stream);
-  h->ws.csr_kernel = (opt && opt->csr_kernel == 8) ? 8 : 1;   // no whole-sweep kernels on this path; 8: the unblocked kernel
+  h->ws.csr_kernel = 1;       // no whole-sweep kernels on this path
   h->ws.time_leja = true;
   if (rc) { set_error("workspace allocation failed (n=%lld)", (long long)h->n); magnus_destroy(h); return rc; }
   *out = h;

@@ -117,118 +117,11 @@ __global__ void __launch_bounds__(256) xxz_leja_iter_kernel(XxzOp op, const cplx
   if (last_block_ticket(ticket)) leja_finalize_warp0(partials, gridDim.x, abs_dk, tol, false, status);   // S7
 }
 
-// The same iteration with a BLOCK of 2^XB_LOG rows per CTA pass: the block's piece of w (32 KB) is loaded into shared
-// memory once, so that the flips of bits 5 .. XB_LOG-1 and the bonds below bit XB_LOG are shared-memory reads instead of
-// L2 gathers (N = 24: 22 instead of 31 L2 gathers per row).  Needs N > XB_LOG.  Same order of the terms as above.
-constexpr int XB_LOG = 11, XB_ROWS = 1 << XB_LOG, XB_THREADS = 256;
-
-__global__ void __launch_bounds__(XB_THREADS) xxz_leja_iter_blocked_kernel(XxzOp op, const cplx* __restrict__ w_in,
-                                                                            cplx* __restrict__ w_out, cplx* __restrict__ p,
-                                                                            double inv_gamma, double shift, cplx dk,
-                                                                            double abs_dk, double tol, LejaStatus* status,
-                                                                            double* partials, unsigned* ticket) {
-  if (status->done) return;
-  __shared__ cplx ws[XB_ROWS];
-  const int N = op.nspins, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int64_t n = (int64_t)1 << N, nblocks = n >> XB_LOG;
-  double sw = 0.0, sp = 0.0;
-  for (int64_t blk = blockIdx.x; blk < nblocks; blk += gridDim.x) {
-    const int64_t base = blk << XB_LOG;
-    __syncthreads();                                  // the previous block's reads of ws are over
-    for (int i = tid; i < XB_ROWS; i += XB_THREADS) ws[i] = w_in[base + i];
-    __syncthreads();
-#pragma unroll 1
-    for (int sl = warp; sl < XB_ROWS / 32; sl += XB_THREADS / 32) {
-      const int loc = (sl << 5) + lane;               // row inside the block
-      const int64_t r = base + loc;
-      const cplx wi = ws[loc];
-      cplx s1 = make_double2(0.0, 0.0);               // H1: single flips, ascending bit
-#pragma unroll
-      for (int b = 0; b < XB_LOG; ++b) {
-        const cplx x = ws[loc ^ (1 << b)];
-        s1.x += x.x;
-        s1.y += x.y;
-      }
-#pragma unroll 8
-      for (int b = XB_LOG; b < N; ++b) {
-        const cplx x = w_in[r ^ ((int64_t)1 << b)];
-        s1.x += x.x;
-        s1.y += x.y;
-      }
-      cplx s2 = make_double2(0.0, 0.0);               // H0: bonds (bit b, bit b-1), descending b
-      int k = 0;
-#pragma unroll 8
-      for (int b = N - 1; b > XB_LOG; --b) {          // both bits above the block bits: the same for the whole block
-        if ((((r >> b) ^ (r >> (b - 1))) & 1) != 0) {
-          const cplx x = w_in[r ^ ((int64_t)3 << (b - 1))];
-          s2.x += x.x;
-          s2.y += x.y;
-          ++k;
-        }
-      }
-      {                                               // bond (XB_LOG, XB_LOG - 1): the partner is in the neighbouring block
-        const bool anti = (((r >> XB_LOG) ^ (r >> (XB_LOG - 1))) & 1) != 0;
-        cplx x = make_double2(0.0, 0.0);
-        if (anti) x = w_in[r ^ ((int64_t)3 << (XB_LOG - 1))];
-        s2.x += x.x;
-        s2.y += x.y;
-        k += anti;
-      }
-#pragma unroll
-      for (int b = XB_LOG - 1; b >= 1; --b) {         // both bits inside the block: shared memory
-        const bool anti = (((loc >> b) ^ (loc >> (b - 1))) & 1) != 0;
-        const cplx x = ws[loc ^ (3 << (b - 1))];
-        if (anti) {
-          s2.x += x.x;
-          s2.y += x.y;
-          ++k;
-        }
-      }
-      {                                               // periodic bond (bit N-1, bit 0)
-        const bool anti = (((r >> (N - 1)) ^ r) & 1) != 0;
-        cplx x = make_double2(0.0, 0.0);
-        if (anti) x = w_in[r ^ (((int64_t)1 << (N - 1)) | 1)];
-        s2.x += x.x;
-        s2.y += x.y;
-        k += anti;
-      }
-      const double dg = op.jz * (double)(N - 2 * k);
-      cplx y;
-      y.x = fma(op.asingle, s1.x, fma(op.apair, s2.x, dg * wi.x));
-      y.y = fma(op.asingle, s1.y, fma(op.apair, s2.y, dg * wi.y));
-      cplx wn;
-      wn.x = inv_gamma * y.x - shift * wi.x;
-      wn.y = inv_gamma * y.y - shift * wi.y;
-      cplx pi = p[r];
-      cfma(pi, dk, wn);
-      w_out[r] = wn;
-      p[r] = pi;
-      sw += wn.x * wn.x + wn.y * wn.y;
-      sp += pi.x * pi.x + pi.y * pi.y;
-    }
-  }
-  block_reduce_sum2<XB_THREADS>(sw, sp);
-  if (threadIdx.x == 0) {
-    partials[2 * blockIdx.x] = sw;
-    partials[2 * blockIdx.x + 1] = sp;
-  }
-  if (last_block_ticket(ticket)) leja_finalize_warp0(partials, gridDim.x, abs_dk, tol, false, status);   // S7
-}
-
 }  // namespace
 
 int launch_xxz_leja_iter(const XxzOp& op, const cplx* w_in, cplx* w_out, cplx* p, double inv_gamma, double shift,
                          cplx dk, double abs_dk, double tol, Workspace* ws, cudaStream_t st) {
   const int64_t n = (int64_t)1 << op.nspins;
-  if (op.nspins > XB_LOG + 1 && ws->csr_kernel != 8) {          // blocked form (csr_kernel 8 forces the plain one: tests)
-    int64_t gb = n >> XB_LOG;
-    const int64_t capb = (int64_t)device_sm_count() * 6;
-    if (gb > capb) gb = capb;
-    xxz_leja_iter_blocked_kernel<<<(int)gb, XB_THREADS, 0, st>>>(op, w_in, w_out, p, inv_gamma, shift, dk, abs_dk, tol,
-                                                                 ws->status, ws->partials, ws->tickets);
-    ws->launches += 1;
-    return (int)gb;
-  }
   int64_t g = (n + 255) / 256;
   const int64_t cap = (int64_t)device_sm_count() * 8;
   if (g > cap) g = cap;
