@@ -832,3 +832,29 @@ def test_runs_on_a_non_blocking_side_stream(M):
                 with M.magnus_create(d0, d1, f, scheme, tol=cfg.tol, stream=side) as h:
                     st1 = h.integrate(cfg.t0, cfg.t_end, cfg.nsteps, psi)
                 assert np.array_equal(st0["iters"], st1["iters"]) and torch.equal(psi, ref), (name, size, scheme, rep)
+
+
+def test_shortcuts_combined_matrix_free_and_tight_interval(M, oracle):
+    """The two shortcuts together: the matrix-free chain with its interval from Lanczos (the fused iteration kernel of
+    the chain serves as the Lanczos mat-vec).  Same intervals and counts as the CSR path in the same mode, and as the
+    oracle in the same mode."""
+    N, m = 12, 10
+    H0, H1 = xxz.xxz_h0(N), xxz.xxz_h1(N)
+    psi0 = torch.from_numpy(rand_vec(1 << N, 77))
+    f = xxz.f_cos2t
+    with oracle.tight_interval(m):
+        ref, riters = oracle.magnus_integrate(oracle.CsrHost.of(H0), oracle.CsrHost.of(H1), f, "cf4", 0.0, 0.15, 3, psi0.numpy(), 1e-12)
+    out = {}
+    for kind in ("xxz", "csr"):
+        psi = psi0.to(DEV).clone()
+        opts = dict(tol=1e-12, shortcuts=M.SHORTCUT_TIGHT_INTERVAL, lanczos_steps=m)
+        h = M.magnus_create_xxz(N, 1.0, 0.5, 1.0, f, "cf4", **opts) if kind == "xxz" else \
+            M.magnus_create(H0.to(DEV), H1.to(DEV), f, "cf4", **opts)
+        with h:
+            info = h.step(0.0, 0.05, psi0.to(DEV).clone())
+            st = h.integrate(0.0, 0.15, 3, psi)
+        out[kind] = (info, st["iters"], host(psi))
+        assert np.array_equal(st["iters"], riters) and relerr(host(psi), ref) <= 1e-9 and st["lanczos_matvecs"] == 6 * m
+    for a, b in zip(out["xxz"][0], out["csr"][0]):
+        assert a["a"] == b["a"] and a["b"] == b["b"] and a["iters"] == b["iters"]
+    assert relerr(out["xxz"][2], out["csr"][2]) <= 1e-12
