@@ -392,6 +392,7 @@ def measure_extra(M, W, torch, dev, peaks, dmma_tf):
             ("cfg3", "cf4", 10, 3, 0, "cfg3_cf4"), ("cfg3", "m4", 10, 3, 0, "cfg3_m4"),
             ("cfg4", "m4", 2, 1, M.SHORTCUT_CACHED_COMMUTATOR, "cfg4_m4_shortcut_cached_commutator"),
             ("cfg4", "cf4", 2, 1, M.SHORTCUT_TIGHT_INTERVAL, "cfg4_cf4_shortcut_tight_interval"),
+            ("cfg5", "cf4", 5, 3, M.SHORTCUT_REAL_VALUES, "cfg5_cf4_shortcut_real_values"),
             ("cfg5", "cf4", 5, 3, XXZ_MATRIX_FREE, "cfg5_cf4_shortcut_matrix_free"),
             ("cfg3", "cf4", 10, 3, XXZ_MATRIX_FREE, "cfg3_cf4_shortcut_matrix_free"))
     for name, scheme, steps, warmup, shortcuts, key in runs:
@@ -403,6 +404,9 @@ def measure_extra(M, W, torch, dev, peaks, dmma_tf):
         out[key] = {"workload": workload_description(cfg, scheme), "steps": steps, "warmup": warmup,
                     "shortcut": ("beyond-paper shortcut, NOT the mandated path: the chain is given by its couplings, "
                                  "no matrix in memory (magnus_create_xxz, SURVEY 8f-4)") if shortcuts == XXZ_MATRIX_FREE else
+                                ("beyond-paper shortcut, NOT the mandated path: the operator has no imaginary parts, the "
+                                 "offset-slot copy keeps the real parts only (8 B per entry); same bits as the mandated "
+                                 "path") if shortcuts == M.SHORTCUT_REAL_VALUES else
                                 ("beyond-paper shortcut, NOT the mandated path: spectral interval from 8 Lanczos steps per "
                                  "exponential instead of Gershgorin (SURVEY 8f-4); its mat-vecs are in lanczos_matvecs, not "
                                  "in matvecs") if shortcuts == M.SHORTCUT_TIGHT_INTERVAL else

@@ -195,6 +195,7 @@ def _drive(f: Callable[[float], float]):
 
 SHORTCUT_CACHED_COMMUTATOR = 1
 SHORTCUT_TIGHT_INTERVAL = 2
+SHORTCUT_REAL_VALUES = 4
 
 
 def _options(tol=None, theta_max=None, m_max=None, check_hermitian=False, stream=None, csr_kernel=0,

@@ -932,7 +932,9 @@ int magnus_describe(magnus_handle h, magnus_path_info* out) {
       out->entries = h->slice.nent;
       if (h->slice.offsets) {
         name = "csr_leja_iter_sliceoff_kernel";
-        out->bytes_per_iteration = 16 * h->slice.nent + 8 * h->slice.nslots + 24 * h->slice.nslices + 64 * n;
+        out->bytes_per_iteration = (h->slice.real_values ? 8 : 16) * h->slice.nent + 8 * h->slice.nslots +
+                                   24 * h->slice.nslices + 64 * n;
+        if (h->slice.real_values) name = "csr_leja_iter_sliceoff_kernel (real values)";
       } else {
         name = "csr_leja_iter_slice_kernel";
         out->bytes_per_iteration = 20 * h->slice.nent + 4 * h->slice.nslots + 24 * h->slice.nslices + 64 * n;
@@ -1083,7 +1085,8 @@ int magnus_create(magnus_handle* out, const magnus_matrix* H0, const magnus_matr
         op.t[2].v = h->c_v;
         op.t[2].nnz = h->c_nnz;
       }
-      if (slice_layout_build(op, &h->slice, h->stream, kind != 1) == MAGNUS_OK && kind == 0 &&
+      const bool allow_real = (h->shortcuts & MAGNUS_SHORTCUT_REAL_VALUES) != 0 || (csr_kernel >= 6500 && csr_kernel < 7000);
+      if (slice_layout_build(op, &h->slice, h->stream, kind != 1, allow_real) == MAGNUS_OK && kind == 0 &&
           (double)h->slice.nent < kSliceAutoMinFill * (double)h->slice.nslots)
         slice_layout_free(&h->slice);                  // poorly filled slots: not worth it
       // on failure the CSR kernels run
@@ -1314,7 +1317,8 @@ static int build_op(const magnus_matrix* H0, const magnus_matrix* H1, double g, 
     op->csr.unit_cap = 0;
     if (csr_unit_cap(op->csr, st, &op->csr.unit_cap) != MAGNUS_OK) op->csr.unit_cap = 0;
     if (tmpS && slice_layout_kind(ws->csr_kernel) != 0 &&
-        slice_layout_build(op->csr, tmpS, st, slice_layout_kind(ws->csr_kernel) == 2) == MAGNUS_OK)
+        slice_layout_build(op->csr, tmpS, st, slice_layout_kind(ws->csr_kernel) == 2,
+                           ws->csr_kernel >= 6500 && ws->csr_kernel < 7000) == MAGNUS_OK)
       op->csr.slice = tmpS;
   } else {
     op->dense = true;

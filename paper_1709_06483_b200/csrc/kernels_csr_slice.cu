@@ -258,10 +258,11 @@ __global__ void __launch_bounds__(SL_WARPS * 32, MINB)
 // FILL = false: count slots and entries per slice; FILL = true: write masks and packed entries.
 // OFFS = true: a slot is stored as the record {row mask, column - row} and no column array is written
 // (the offset-slot layout of csr_kernel 6); OFFS = false: masks and a column per entry (csr_kernel 5).
-template <bool FILL, bool OFFS>
+// REAL (with OFFS): every stored value has a zero imaginary part (checked before), only the real parts are written.
+template <bool FILL, bool OFFS, bool REAL = false>
 __global__ void __launch_bounds__(128)
     slice_merge_kernel(CsrOp op, int64_t nslices, int4* meta, int64_t* ent_ptr, unsigned* slot_mask, uint2* slot_rec,
-                       int32_t* ci_out, cplx* v_out) {
+                       int32_t* ci_out, cplx* v_out, double* vr_out = nullptr) {
   const int lane = threadIdx.x & 31;
   const unsigned lt = (1u << lane) - 1u;
   const int64_t s = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
@@ -299,7 +300,8 @@ __global__ void __launch_bounds__(128)
         if (hit) {
           const int64_t q = eb + ents + __popc(m & lt);
           if (!OFFS) ci_out[q] = col;
-          v_out[q] = vv[cur];
+          if (REAL) vr_out[q] = vv[cur].x;
+          else v_out[q] = vv[cur];
         }
       }
       ents += __popc(m);
@@ -317,6 +319,14 @@ __global__ void __launch_bounds__(128)
     meta[s] = make_int4(0, nslots, op.nterms > 1 ? b[1] : nslots, op.nterms > 2 ? b[2] : nslots);
     ent_ptr[s] = ents;
   }
+}
+
+// flag |= 1 if any stored value of the term has a non-zero imaginary part
+__global__ void __launch_bounds__(256) csr_any_imag_kernel(const cplx* __restrict__ v, int64_t nnz, int* flag) {
+  bool any = false;
+  for (int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; q < nnz; q += (int64_t)gridDim.x * blockDim.x)
+    any |= v[q].y != 0.0;
+  if (__syncthreads_or(any) && threadIdx.x == 0) atomicOr(flag, 1);
 }
 
 // exclusive prefix sums of the slot and entry counts (one CTA; nslices is at most a few million)
@@ -385,9 +395,29 @@ struct SliceViewO {
   const int4* meta;            // per slice: {first slot (global), slots, first slot of term 1, of term 2}
   const int64_t* ent_ptr;      // [nslices + 1]
   const uint2* rec;            // per slot {row mask, column - row}
-  const cplx* v;
+  const cplx* v;               // values, or
+  const double* vr;            // ... their real parts when every imaginary part is zero (real layout: 8 B per entry)
   cplx coef[3];
 };
+
+// value type in flight: complex, or the real part alone
+template <bool REAL> struct SlotVal { typedef cplx type; };
+template <> struct SlotVal<true> { typedef double type; };
+__device__ __forceinline__ double ld_stream_real_if(const double* p, unsigned ok) {
+  double r;
+  asm("{\n .reg .pred q;\n setp.ne.b32 q, %2, 0;\n mov.f64 %0, 0d0000000000000000;\n"
+      " @q ld.global.nc.L1::no_allocate.f64 %0, [%1];\n}"
+      : "=d"(r)
+      : "l"(p), "r"(ok));
+  return r;
+}
+// acc += v x for a real v: the two products the complex form adds with a zero imaginary part are left out, the
+// result is the same to the bit
+__device__ __forceinline__ void slot_fma(cplx& acc, double v, cplx x) {
+  acc.x = fma(v, x.x, acc.x);
+  acc.y = fma(v, x.y, acc.y);
+}
+__device__ __forceinline__ void slot_fma(cplx& acc, cplx v, cplx x) { cfma(acc, v, x); }
 
 __device__ __forceinline__ cplx ld_stream_hint_if(const cplx* p, unsigned ok, uint64_t pol) {
   cplx r;
@@ -415,7 +445,7 @@ __device__ __forceinline__ cplx ld_cached_if(const cplx* p, unsigned ok) {
 }
 
 // POL: 0 no L2 hints; 1 matrix values evict-first; 2 also w gathers evict-last.  SO_U slots in flight per lane.
-template <int SO_U, int MINB, int POL>
+template <int SO_U, int MINB, int POL, bool REAL>
 __global__ void __launch_bounds__(SL_WARPS * 32, MINB)
     csr_leja_iter_sliceoff_kernel(SliceViewO L, const cplx* __restrict__ w_in, cplx* __restrict__ w_out,
                                   cplx* __restrict__ p, double inv_gamma, double shift, cplx dk, double abs_dk,
@@ -463,7 +493,8 @@ __global__ void __launch_bounds__(SL_WARPS * 32, MINB)
     // issue side
     int bufI = 0, jI = 0;
     unsigned runI = 0;                       // entries of the slice before slot jI
-    const cplx* vbI = L.v + DI.eb;
+    typedef typename SlotVal<REAL>::type val_t;
+    const val_t* vbI = (REAL ? (const val_t*)L.vr : (const val_t*)L.v) + DI.eb;
     int64_t rowI = ((int64_t)sI << 5) + lane;
     bool issuing = true;
     // consume side (one batch behind)
@@ -474,12 +505,17 @@ __global__ void __launch_bounds__(SL_WARPS * 32, MINB)
       wi = w_in[rowC];
       pi = p[rowC];
     }
-    cplx v[SO_U], x[SO_U];
+    val_t v[SO_U];
+    cplx x[SO_U];
     auto issue_slot = [&](int u) {
       const uint2 r = s_rec[warp][bufI][jI + u];
       const unsigned ok = r.x & lbit;
-      v[u] = POL >= 1 ? ld_stream_hint_if(vbI + (runI + __popc(r.x & lt)), ok, pol_v)
-                      : ld_stream_if(vbI + (runI + __popc(r.x & lt)), ok);
+      if constexpr (REAL) {
+        v[u] = ld_stream_real_if(vbI + (runI + __popc(r.x & lt)), ok);
+      } else {
+        v[u] = POL >= 1 ? ld_stream_hint_if(vbI + (runI + __popc(r.x & lt)), ok, pol_v)
+                        : ld_stream_if(vbI + (runI + __popc(r.x & lt)), ok);
+      }
       x[u] = POL >= 2 ? ld_cached_hint_if(w_in + (rowI + (int)r.y), ok, pol_w)
                       : ld_cached_if(w_in + (rowI + (int)r.y), ok);
       runI += __popc(r.x);
@@ -504,7 +540,7 @@ __global__ void __launch_bounds__(SL_WARPS * 32, MINB)
           if (have2) load_desc(sI + 2 * stride, D2);
           jI = 0;
           runI = 0;
-          vbI = L.v + DI.eb;
+          vbI = (REAL ? (const val_t*)L.vr : (const val_t*)L.v) + DI.eb;
           rowI = ((int64_t)sI << 5) + lane;
         } else {
           issuing = false;
@@ -520,13 +556,13 @@ __global__ void __launch_bounds__(SL_WARPS * 32, MINB)
       if (issuing) {
 #pragma unroll
         for (int u = 0; u < SO_U; ++u) {
-          cfma(a, v[u], x[u]);
+          slot_fma(a, v[u], x[u]);
           issue_slot(u);
         }
         jI += SO_U;
       } else {
 #pragma unroll
-        for (int u = 0; u < SO_U; ++u) cfma(a, v[u], x[u]);
+        for (int u = 0; u < SO_U; ++u) slot_fma(a, v[u], x[u]);
       }
       jC += SO_U;
       if (jC >= nsC) {
@@ -577,13 +613,17 @@ void slice_layout_free(SliceLayout* L) {
   cudaFree(L->slot_rec);
   cudaFree(L->ci);
   cudaFree(L->v);
+  cudaFree(L->vr);
   *L = SliceLayout();
 }
 
 // Returns MAGNUS_OK and a filled layout, or an error code with *out left empty (callers fall back to
 // the CSR kernels: the layout is an optimisation, never a requirement).  Synchronises the stream once.
 // offsets = true builds the offset-slot layout of csr_kernel 6 (slot records, no column array).
-int slice_layout_build(const CsrOp& op, SliceLayout* out, cudaStream_t st, bool offsets) {
+// allow_real (offset-slot layout only; the shortcut MAGNUS_SHORTCUT_REAL_VALUES): when no stored value of any term has
+// an imaginary part -- a real symmetric operator, e.g. the spin chains -- only the real parts are stored (8 B per
+// entry) and the kernel multiplies by them; the results are the same to the bit.
+int slice_layout_build(const CsrOp& op, SliceLayout* out, cudaStream_t st, bool offsets, bool allow_real) {
   *out = SliceLayout();
   SliceLayout L;
   L.n = op.n;
@@ -591,12 +631,19 @@ int slice_layout_build(const CsrOp& op, SliceLayout* out, cudaStream_t st, bool 
   L.nterms = op.nterms;
   L.offsets = offsets;
   int64_t* totals = nullptr;
-  int64_t host_totals[3] = {0, 0, 0};
+  int64_t host_totals[4] = {0, 0, 0, 0};
   bool ok = cudaMalloc(&L.meta, sizeof(int4) * (size_t)L.nslices) == cudaSuccess &&
             cudaMalloc(&L.ent_ptr, sizeof(int64_t) * (size_t)(L.nslices + 1)) == cudaSuccess &&
-            cudaMalloc(&totals, 3 * sizeof(int64_t)) == cudaSuccess;
+            cudaMalloc(&totals, 4 * sizeof(int64_t)) == cudaSuccess;
   const int64_t blocks = (L.nslices * 32 + 127) / 128;
   if (ok) {
+    cudaMemsetAsync(totals, 0, 4 * sizeof(int64_t), st);
+    if (offsets && allow_real)
+      for (int t = 0; t < op.nterms; ++t) {
+        int64_t g = (op.t[t].nnz + 255) / 256;
+        if (g > (int64_t)device_sm_count() * 16) g = (int64_t)device_sm_count() * 16;
+        if (g > 0) csr_any_imag_kernel<<<(int)g, 256, 0, st>>>(op.t[t].v, op.t[t].nnz, reinterpret_cast<int*>(totals + 3));
+      }
     slice_merge_kernel<false, false><<<(unsigned)blocks, 128, 0, st>>>(op, L.nslices, L.meta, L.ent_ptr, nullptr, nullptr,
                                                                        nullptr, nullptr);
     slice_scan_kernel<<<1, 1024, 0, st>>>(L.nslices, L.meta, L.ent_ptr, totals);
@@ -610,8 +657,9 @@ int slice_layout_build(const CsrOp& op, SliceLayout* out, cudaStream_t st, bool 
   if (ok) {
     L.nslots = host_totals[0];
     L.nent = host_totals[1];
+    L.real_values = offsets && allow_real && host_totals[3] == 0;
     const size_t ns = (size_t)(L.nslots > 0 ? L.nslots : 1), ne = (size_t)(L.nent > 0 ? L.nent : 1);
-    ok = cudaMalloc(&L.v, sizeof(cplx) * ne) == cudaSuccess;
+    ok = L.real_values ? cudaMalloc(&L.vr, sizeof(double) * ne) == cudaSuccess : cudaMalloc(&L.v, sizeof(cplx) * ne) == cudaSuccess;
     if (ok && offsets) {
       ok = cudaMalloc(&L.slot_rec, sizeof(uint2) * ns) == cudaSuccess &&
            cudaMemsetAsync(L.slot_rec, 0, sizeof(uint2) * ns, st) == cudaSuccess;
@@ -622,7 +670,10 @@ int slice_layout_build(const CsrOp& op, SliceLayout* out, cudaStream_t st, bool 
     }
   }
   if (ok) {
-    if (offsets)
+    if (offsets && L.real_values)
+      slice_merge_kernel<true, true, true><<<(unsigned)blocks, 128, 0, st>>>(op, L.nslices, L.meta, L.ent_ptr, nullptr,
+                                                                             L.slot_rec, nullptr, nullptr, L.vr);
+    else if (offsets)
       slice_merge_kernel<true, true><<<(unsigned)blocks, 128, 0, st>>>(op, L.nslices, L.meta, L.ent_ptr, nullptr,
                                                                        L.slot_rec, nullptr, L.v);
     else
@@ -651,17 +702,23 @@ int launch_csr_leja_iter_slice(const CsrOp& op, const cplx* w_in, cplx* w_out, c
     L.ent_ptr = S.ent_ptr;
     L.rec = S.slot_rec;
     L.v = S.v;
+    L.vr = S.vr;
     for (int t = 0; t < 3; ++t) L.coef[t] = t < op.nterms ? op.t[t].coef : make_double2(0.0, 0.0);
     // tuning code 6000 + 100 POL + 10 [4 slots in flight instead of 8] + MINB (default 6004: no hints, 8 slots,
     // 4 CTAs = 16 warps per SM)
-    const int code = ws->csr_kernel >= 6000 && ws->csr_kernel < 7000 ? ws->csr_kernel - 6000 : 4;
+    int code = ws->csr_kernel >= 6000 && ws->csr_kernel < 7000 ? ws->csr_kernel - 6000 : 4;
+    if (code >= 500) code -= 500;       // 6500..6999: the same tuning codes on real-part storage (see slice_layout_build)
     const int minb = code % 10, pol = code / 100, u = (code / 10) % 10 ? 4 : 8;
+    const bool real = S.real_values;
 #define SO_LAUNCH(U, MINB, POL)                                                                                      \
-  if (u == U && minb == MINB && pol == POL) {                                                                        \
+  SO_LAUNCH_(U, MINB, POL, false)                                                                                    \
+  SO_LAUNCH_(U, MINB, POL, true)
+#define SO_LAUNCH_(U, MINB, POL, REAL)                                                                               \
+  if (u == U && minb == MINB && pol == POL && real == REAL) {                                                        \
     int64_t g = (S.nslices + SL_WARPS - 1) / SL_WARPS;                                                               \
     const int64_t cap = (int64_t)device_sm_count() * MINB;                                                           \
     if (g > cap) g = cap;                                                                                            \
-    csr_leja_iter_sliceoff_kernel<U, MINB, POL><<<(int)g, SL_WARPS * 32, 0, st>>>(                                   \
+    csr_leja_iter_sliceoff_kernel<U, MINB, POL, REAL><<<(int)g, SL_WARPS * 32, 0, st>>>(                             \
         L, w_in, w_out, p, inv_gamma, shift, dk, abs_dk, tol, ws->status, ws->partials, ws->tickets);                \
     ws->launches += 1;                                                                                               \
     return (int)g;                                                                                                   \
@@ -676,6 +733,7 @@ int launch_csr_leja_iter_slice(const CsrOp& op, const cplx* w_in, cplx* w_out, c
     SO_LAUNCH(4, 7, 0)
     SO_LAUNCH(4, 8, 0)
 #undef SO_LAUNCH
+#undef SO_LAUNCH_
     return -1;
   }
   SliceView L;

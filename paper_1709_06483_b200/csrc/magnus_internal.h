@@ -51,6 +51,8 @@ struct SliceLayout {
   uint2* slot_rec = nullptr;     // [nslots] {row mask, column - row}: all entries of a slot share column - row
   int32_t* ci = nullptr;         // [nent] columns, slot-major
   cplx* v = nullptr;             // [nent] values, same order
+  bool real_values = false;      // offset-slot layout of an operator without imaginary parts: vr instead of v
+  double* vr = nullptr;          // [nent] real parts of the values
 };
 struct CsrOp {
   int64_t n;
@@ -207,8 +209,10 @@ int launch_csr_leja_iter_stream(const CsrOp& op, const cplx* w_in, cplx* w_out, 
 // ---- kernels_csr_slice.cu ---------------------------------------------------
 // slice-major copy of op's terms (coefficients ignored); an error leaves *out empty and callers keep the CSR kernels
 // offsets: slots stored as {row mask, column - row} records and no column array (csr_kernel 6)
-int slice_layout_build(const CsrOp& op, SliceLayout* out, cudaStream_t st, bool offsets);
-// which slice layout a csr_kernel option asks for: 0 none, 1 with columns (5, 5000..5999), 2 offset slots (6, 6000..6999)
+// allow_real: store only the real parts when no stored value has an imaginary part (offset-slot layout)
+int slice_layout_build(const CsrOp& op, SliceLayout* out, cudaStream_t st, bool offsets, bool allow_real = false);
+// which slice layout a csr_kernel option asks for: 0 none, 1 with columns (5, 5000..5999), 2 offset slots (6, 6000..6999;
+// 6500..6999: real-part storage when the operator has no imaginary parts, tuning code = the option - 500)
 inline int slice_layout_kind(int csr_kernel) {
   if (csr_kernel == 5 || (csr_kernel >= 5000 && csr_kernel < 6000)) return 1;
   if (csr_kernel == 6 || (csr_kernel >= 6000 && csr_kernel < 7000)) return 2;

@@ -126,7 +126,8 @@ def expected_iteration(oracle, Mh, w, p, inv_gamma, shift, d):
     return wn, pn
 
 
-@pytest.mark.parametrize("N,kernel", [(8, 1), (12, 1), (12, 2), (15, 2), (16, 0), (8, 3), (12, 3), (16, 3), (16, 24001), (16, 27081), (16, 22040), (8, 4), (12, 4), (16, 4), (3, 5), (8, 5), (12, 5), (16, 5), (16, 5083), (16, 5045), (3, 6), (8, 6), (12, 6), (16, 6), (16, 6003), (16, 6104), (16, 6204), (16, 6016), (12, 6018)])
+@pytest.mark.parametrize("N,kernel", [(8, 1), (12, 1), (12, 2), (15, 2), (16, 0), (8, 3), (12, 3), (16, 3), (16, 24001), (16, 27081), (16, 22040), (8, 4), (12, 4), (16, 4), (3, 5), (8, 5), (12, 5), (16, 5), (16, 5083), (16, 5045), (3, 6), (8, 6), (12, 6), (16, 6), (16, 6003), (16, 6104), (16, 6204), (16, 6016), (12, 6018),
+                                      (8, 6504), (16, 6504), (16, 6515)])   # 65xx: real-part storage (shortcut) of the real chain
 def test_fused_iteration_csr_xxz(M, oracle, N, kernel):
     n = 1 << N
     H0, H1 = xxz.xxz_h0(N), xxz.xxz_h1(N)
@@ -858,3 +859,36 @@ def test_shortcuts_combined_matrix_free_and_tight_interval(M, oracle):
     for a, b in zip(out["xxz"][0], out["csr"][0]):
         assert a["a"] == b["a"] and a["b"] == b["b"] and a["iters"] == b["iters"]
     assert relerr(out["xxz"][2], out["csr"][2]) <= 1e-12
+
+
+@pytest.mark.parametrize("scheme", ["cf4", "m4"])
+def test_shortcut_real_values(M, oracle, scheme):
+    """MAGNUS_SHORTCUT_REAL_VALUES on a large CSR chain (N = 18: the offset-slot copy keeps the real parts only): the
+    same bits as the mandated path, counts equal to the oracle's; on an operator WITH imaginary parts the flag changes
+    nothing (complex storage stays)."""
+    cfg = W.scaled(W.CONFIGS["cfg3"], 18, 2)
+    H0, H1, psi0, f = W.build(cfg)
+    ref, riters = oracle.magnus_integrate(oracle.CsrHost.of(H0), oracle.CsrHost.of(H1), f, scheme, cfg.t0, cfg.t_end,
+                                          cfg.nsteps, psi0.numpy(), cfg.tol)
+    d0, d1 = H0.to(DEV), H1.to(DEV)
+    out = {}
+    for sc in (0, M.SHORTCUT_REAL_VALUES):
+        psi = psi0.to(DEV).clone()
+        with M.magnus_create(d0, d1, f, scheme, tol=cfg.tol, shortcuts=sc) as h:
+            d = h.describe()
+            st = h.integrate(cfg.t0, cfg.t_end, cfg.nsteps, psi)
+        out[sc] = (d, st["iters"], psi)
+        assert np.array_equal(st["iters"], riters) and relerr(host(psi), ref) <= 1e-9
+    assert torch.equal(out[0][2], out[M.SHORTCUT_REAL_VALUES][2])
+    assert "real values" in out[M.SHORTCUT_REAL_VALUES][0]["leja_kernel"] and "real values" not in out[0][0]["leja_kernel"]
+    assert out[0][0]["bytes_per_iteration"] - out[M.SHORTCUT_REAL_VALUES][0]["bytes_per_iteration"] == 8 * out[0][0]["entries"]
+    # an operator with imaginary parts: i (|r><r'| - |r'><r|)-type entries from a complex phase on H1
+    H1c = xxz.CSR(H1.n, H1.row_ptr, H1.col_idx, H1.values * torch.where(H1.col_idx.long() > torch.repeat_interleave(
+        torch.arange(H1.n), (H1.row_ptr[1:] - H1.row_ptr[:-1]).long()), torch.tensor(1j), torch.tensor(-1j)))
+    with M.magnus_create(d0, H1c.to(DEV), f, "cf4", tol=cfg.tol, shortcuts=M.SHORTCUT_REAL_VALUES) as h:
+        assert "real values" not in h.describe()["leja_kernel"]
+        psi = psi0.to(DEV).clone()
+        st = h.integrate(cfg.t0, cfg.t0 + cfg.tau, 1, psi)
+    refc, ritc = oracle.magnus_integrate(oracle.CsrHost.of(H0), oracle.CsrHost.of(H1c), f, "cf4", cfg.t0, cfg.t0 + cfg.tau, 1,
+                                         psi0.numpy(), cfg.tol)
+    assert np.array_equal(st["iters"], ritc) and relerr(host(psi), refc) <= 1e-9
