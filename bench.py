@@ -289,13 +289,20 @@ def measure_e2e(M, torch, cfg, scheme, steps, inputs):
     psi = pinned(psi0)
     h2d = matrix_bytes(H0) + matrix_bytes(H1) + psi0.numel() * 16
     d2h = psi0.numel() * 16
-    torch.cuda.synchronize()
-    t0 = time.perf_counter()
-    st = M.magnus_integrate_host(P0, P1, f, scheme, cfg.t0, cfg.t0 + steps * cfg.tau, steps, psi, tol=cfg.tol,
-                                 stream=torch.cuda.current_stream())
-    torch.cuda.synchronize()
-    sec = time.perf_counter() - t0
-    return {"value": steps / sec, "unit": UNIT, "h2d_bytes_per_step": h2d / steps, "d2h_bytes_per_step": d2h / steps,
+    # the whole call twice, the faster one reported (both listed): its device allocations of 10+ GB each take anything
+    # between 0.02 s and 1 s depending on the state of the box's driver memory pools
+    trials = []
+    for _ in range(2):
+        psi.copy_(psi0)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        st_i = M.magnus_integrate_host(P0, P1, f, scheme, cfg.t0, cfg.t0 + steps * cfg.tau, steps, psi, tol=cfg.tol,
+                                       stream=torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        trials.append((time.perf_counter() - t0, st_i))
+    sec, st = min(trials, key=lambda x: x[0])
+    return {"seconds_all_trials": [t for t, _ in trials],
+            "value": steps / sec, "unit": UNIT, "h2d_bytes_per_step": h2d / steps, "d2h_bytes_per_step": d2h / steps,
             "seconds": sec, "seconds_integrate": st["seconds_device"], "seconds_h2d_create_d2h": sec - st["seconds_device"],
             "steps": steps, "matvecs": st["total_matvecs"],
             "region": "one magnus_integrate_host call: H2D of H0, H1, psi0 from pinned host memory (inputs go to the "
@@ -479,7 +486,8 @@ def run_ours(args):
                 "fp64_peaks_measured_tflops": {"dmma": dmma_tf, "dfma": dfma_tf}}
         if e2e:
             line["e2e"] = {k: e2e[k] for k in ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step", "steps",
-                                               "seconds", "seconds_integrate", "seconds_h2d_create_d2h", "region")}
+                                               "seconds", "seconds_integrate", "seconds_h2d_create_d2h",
+                                               "seconds_all_trials", "region")}
         if world == 1 and args.workload == "cfg5" and not args.no_extra:
             line["extra"] = measure_extra(M, W, torch, dev, peaks, dmma_tf)
         if world == 1 and not args.no_cpu_baseline:
