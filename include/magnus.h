@@ -245,6 +245,34 @@ int magnus_leja_iteration(const magnus_matrix* H0, const magnus_matrix* H1, doub
                           double d_re, double d_im, void* stream, int csr_kernel, int reps,
                           double* sums_host, float* ms_per_launch);
 
+/* magnus_leja_iteration_dense_noalloc -- the same fused iteration (row S6) on a dense row-major matrix,
+ * for callers that are not allowed to allocate: a process whose GPU memory already belongs to a pool (a PyTorch
+ * caching allocator that has taken the device, a service with a fixed memory budget, a plug-in inside another
+ * program's CUDA context) cannot rely on cudaMalloc succeeding, and a latency-bound loop cannot afford it --
+ * cudaMalloc / cudaFree take driver-wide locks and cudaFree waits for the device.  Every other reducing entry point
+ * here allocates a workspace for its per-block partial sums; this one keeps them in a fixed array inside the library
+ * image and calls no cudaMalloc, cudaMallocHost, cudaFree, event/stream creation or allocating library routine.
+ *   w_out = inv_gamma * M w_in - shift * w_in;   p += (d_re + i d_im) * w_out;
+ *   sums_dev[0] = sum |w_out|^2,  sums_dev[1] = sum |p|^2   (after the update).
+ * All pointers are DEVICE pointers owned by the caller: M (n rows of ld >= n complex128, ld = 0 means n), w_in, w_out,
+ * p (n complex128, pairwise distinct, 16-byte aligned), sums_dev (2 doubles, written by the kernel).  The call only
+ * ENQUEUES on `stream` (a memset of 256 bytes and one kernel) and returns; results are valid in stream order.
+ * For n <= MAGNUS_NOALLOC_MAX_N the results equal magnus_leja_iteration's on the same dense matrix bit for bit.
+ * Limits and rules:
+ *   - n <= MAGNUS_NOALLOC_MAX_N; anything larger returns MAGNUS_EINVAL with a message (nothing is launched).
+ *   - The scratch is 65,792 bytes of device memory that every GPU on which this library is loaded holds until the
+ *     process exits, used or not.
+ *   - One scratch per device, shared by all calls and all threads: calls that may overlap on the GPU (different
+ *     streams without an ordering between them) race on it and return wrong sums.  Order them.
+ *   - It keeps the previous call's contents; the call itself re-zeroes the one word that has to start at zero.
+ *   - The first call on each device (with that device current) resolves the scratch address with
+ *     cudaGetSymbolAddress, which can trigger module loading: make it before any stream capture begins.
+ * Errors: EINVAL (sizes, null / aliased / misaligned pointers), ECUDA (no device, address lookup or enqueue failed). */
+#define MAGNUS_NOALLOC_MAX_N 32768
+int magnus_leja_iteration_dense_noalloc(int64_t n, const void* M, int64_t ld, const void* w_in, void* w_out, void* p,
+                                        double inv_gamma, double shift, double d_re, double d_im, void* stream,
+                                        double* sums_dev);
+
 /* C = A * B, dense row-major complex128 n x n (device), by the FP64 tensor-core
  * (DMMA m8n8k4) kernel used for the M4 commutator (P:262 l.6-7).  C must not
  * alias A or B.  ms (nullable): CUDA-event time of the launch. */

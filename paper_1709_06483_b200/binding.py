@@ -72,7 +72,7 @@ DRIVE = C.CFUNCTYPE(C.c_double, C.c_double, C.c_void_p)
 
 EXPORTS = [
     "magnus_create", "magnus_create_xxz", "magnus_destroy", "magnus_describe", "leja_expmv", "magnus_step", "magnus_integrate", "magnus_integrate_host",
-    "magnus_gershgorin", "magnus_leja_iteration", "magnus_zgemm", "magnus_commutator_dense", "magnus_commutator_csr", "magnus_omega_dense",
+    "magnus_gershgorin", "magnus_leja_iteration", "magnus_leja_iteration_dense_noalloc", "magnus_zgemm", "magnus_commutator_dense", "magnus_commutator_csr", "magnus_omega_dense",
     "magnus_fp64_peaks", "magnus_host_leja_points", "magnus_host_divided_differences", "magnus_host_snap_interval", "magnus_host_tridiag_extremes",
     "magnus_host_step_coefficients", "magnus_strerror", "magnus_last_error", "magnus_version",
 ]
@@ -111,6 +111,9 @@ def lib():
                                             C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_double,
                                             C.c_void_p, C.c_int, C.c_int, C.POINTER(C.c_double),
                                             C.POINTER(C.c_float)]
+        L.magnus_leja_iteration_dense_noalloc.argtypes = [C.c_int64, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p,
+                                                          C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_double,
+                                                          C.c_void_p, C.c_void_p]
         L.magnus_zgemm.argtypes = [C.c_int64, C.c_void_p, C.c_int64, C.c_void_p, C.c_int64, C.c_void_p, C.c_int64,
                                    C.c_void_p, C.POINTER(C.c_float)]
         L.magnus_commutator_dense.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -348,6 +351,21 @@ def magnus_leja_iteration(H0, H1, g: float, w_in, w_out, p, inv_gamma: float, sh
                                        shift, complex(d).real, complex(d).imag, _stream_ptr(stream), csr_kernel, reps,
                                        sums, C.byref(ms)))
     return sums[0], sums[1], ms.value
+
+
+NOALLOC_MAX_N = 32768
+
+
+def magnus_leja_iteration_dense_noalloc(M, w_in, w_out, p, inv_gamma: float, shift: float, d: complex, sums,
+                                        stream=None) -> None:
+    """The fused dense Leja iteration for callers that must not allocate device memory (a process whose GPU
+    memory is owned by a pool, a latency-bound loop): the library's static scratch replaces the workspace, n is
+    limited to NOALLOC_MAX_N, calls must not overlap on one GPU.  `M` is an n x n complex128 device tensor (rows
+    may be strided), `sums` a device tensor of 2 float64 that receives (sum |w_out|^2, sum |p|^2).  Enqueues only:
+    read `sums` after synchronising the stream.  See include/magnus.h."""
+    _check(lib().magnus_leja_iteration_dense_noalloc(int(M.shape[0]), _ptr(M), int(M.stride(0)), _ptr(w_in),
+                                                     _ptr(w_out), _ptr(p), inv_gamma, shift, complex(d).real,
+                                                     complex(d).imag, _stream_ptr(stream), _ptr(sums)))
 
 
 def magnus_zgemm(A, B, Cout, stream=None) -> float:

@@ -16,7 +16,7 @@ BUILD = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libmagnus_b200.so")
 
 CU_SOURCES = ["api.cu", "kernels_common.cu", "kernels_csr.cu", "kernels_csr_rowblock.cu", "kernels_csr_small.cu", "kernels_csr_mid.cu", "kernels_csr_slice.cu", "kernels_csr_stream.cu", "kernels_dense.cu", "kernels_dense_sweep.cu", "kernels_xxz.cu", "kernels_lanczos.cu",
-              "zgemm_dmma.cu"]
+              "zgemm_dmma.cu", "no_alloc.cu"]
 CPP_SOURCES = ["host_leja.cpp"]
 HEADERS = ["magnus_internal.h", "device_utils.cuh", "leja_finalize.cuh", os.path.join("..", "..", "include", "magnus.h")]
 
