@@ -18,8 +18,9 @@ flush is needed between timed steps).  Rank 0 prints ONE JSON line.
              live with CUDA events inside the timed region, against MEASURED_PEAKS.json
   cpu_baseline  the oracle (oracle/, test infrastructure) timed on this box's host cores on a bounded sample:
              ONE Magnus step of the SAME workload at full size (N = 24 for cfg5; about 45 s)
-  extra      (default run only) two short secondary measurements so that the record carries all three parts of
-             the metric: cfg4 CF4 (dense GEMV GB/s) and cfg4 M4 (DMMA commutator TFLOP/s)
+  --extra FILE.json   (opt-in) secondary measurements (cfg1-cfg4 in both schemes, the beyond-paper shortcuts) written
+             to FILE.json; they never enter the headline line, which stays below MAX_LINE_BYTES so that the driver's
+             stored tail always holds it whole
 
 Multi-GPU: the path does not shard ("replicas only"); --gpus N runs N
 independent replicas, one process per GPU, no data-path collective, scaling "weak".
@@ -48,14 +49,10 @@ UNIT = "steps/s"
 NCU_TRAFFIC_BYTES = {("cfg5", "cf4", "csr_leja_iter_sliceoff_kernel"): 12.737e9,
                      ("cfg5", "cf4", "csr_leja_iter_rowblock_kernel"): 15.093e9,
                      ("cfg4", "cf4", "dense_leja_iter_kernel"): 4.299e9}
-NCU_TRAFFIC_SOURCE = {
-    ("cfg5", "cf4", "csr_leja_iter_sliceoff_kernel"):
-        "ncu --set full capture of csr_leja_iter_sliceoff_kernel<8,4,0> at N=24, 2026-11-04, round 2 "
-        "(profiles/r2_csr_sliceoff_ncu.md): dram read 12.207 GB + write 0.530 GB in 2.218 ms",
-    ("cfg5", "cf4", "csr_leja_iter_rowblock_kernel"):
-        "ncu --set full capture of csr_leja_iter_rowblock_kernel, round 1 (commit 6319c2a, profiles/r1_csr_rowblock_ncu.md)",
-    ("cfg4", "cf4", "dense_leja_iter_kernel"):
-        "ncu --set full capture of dense_leja_iter_kernel, round 1 (profiles/r1_dense_gemv_ncu.md); kernel unchanged since"}
+NCU_TRAFFIC_SOURCE = {("cfg5", "cf4", "csr_leja_iter_sliceoff_kernel"): "profiles/r2_csr_sliceoff_ncu.md",
+                      ("cfg5", "cf4", "csr_leja_iter_rowblock_kernel"): "profiles/r1_csr_rowblock_ncu.md",
+                      ("cfg4", "cf4", "dense_leja_iter_kernel"): "profiles/r1_dense_gemv_ncu.md"}
+MAX_LINE_BYTES = 4096     # the headline JSON line must stay below this (a 21 KB line was cut off in the driver's record)
 
 
 # ----------------------------------------------------------------------------- helpers
@@ -289,10 +286,10 @@ def measure_e2e(M, torch, cfg, scheme, steps, inputs):
     psi = pinned(psi0)
     h2d = matrix_bytes(H0) + matrix_bytes(H1) + psi0.numel() * 16
     d2h = psi0.numel() * 16
-    # the whole call twice, the faster one reported (both listed): its device allocations of 10+ GB each take anything
-    # between 0.02 s and 1 s depending on the state of the box's driver memory pools
+    # the whole call three times, the MEDIAN reported (all three listed): its large device allocations take between
+    # 0.02 s and 1 s depending on the state of the driver's memory pools, so a single call is noisy either way
     trials = []
-    for _ in range(2):
+    for _ in range(3):
         psi.copy_(psi0)
         torch.cuda.synchronize()
         t0 = time.perf_counter()
@@ -300,14 +297,11 @@ def measure_e2e(M, torch, cfg, scheme, steps, inputs):
                                        stream=torch.cuda.current_stream())
         torch.cuda.synchronize()
         trials.append((time.perf_counter() - t0, st_i))
-    sec, st = min(trials, key=lambda x: x[0])
-    return {"seconds_all_trials": [t for t, _ in trials],
+    sec, st = sorted(trials, key=lambda x: x[0])[1]
+    return {"seconds_all_trials": [round(t, 4) for t, _ in trials], "reported": "median of 3 calls",
             "value": steps / sec, "unit": UNIT, "h2d_bytes_per_step": h2d / steps, "d2h_bytes_per_step": d2h / steps,
             "seconds": sec, "seconds_integrate": st["seconds_device"], "seconds_h2d_create_d2h": sec - st["seconds_device"],
-            "steps": steps, "matvecs": st["total_matvecs"],
-            "region": "one magnus_integrate_host call: H2D of H0, H1, psi0 from pinned host memory (inputs go to the "
-                      "device ONCE per integration, PAPER.md l.209), magnus_create, K steps, D2H of psi; the one-off "
-                      "part (seconds_h2d_create_d2h) is amortised over the K steps of the call, so `value` depends on K"}
+            "steps": steps, "matvecs": st["total_matvecs"]}
 
 
 def roofline_for(cfg, scheme, st, peaks, fp64_peak_tflops, path=None):
@@ -329,8 +323,7 @@ def _roofline_for(cfg, scheme, st, peaks, fp64_peak_tflops, path=None):
         achieved = flops * nsteps_exp / comm_s / 1e12
         return {"kernel": "zgemm_dmma_kernel", "bound": "tensor", "achieved": achieved, "peak": fp64_peak_tflops,
                 "unit": "TFLOP/s", "frac": achieved / fp64_peak_tflops if fp64_peak_tflops else None, "traffic": None,
-                "peak_source": "FP64 DMMA m8n8k4 register-resident micro-benchmark (magnus_fp64_peaks) run in this process; "
-                               "MEASURED_PEAKS.json has no FP64 figure and the guide gives no bf16->fp64 ratio",
+                "peak_source": "magnus_fp64_peaks: DMMA m8n8k4 micro-benchmark run in this process",
                 "flops_per_launch": flops}
     # bytes of the variant the library actually runs (magnus_describe): "never count bytes a variant does not
     # move"; the plain-CSR figure of SURVEY 8(d) is reported beside it as csr_equivalent
@@ -342,20 +335,15 @@ def _roofline_for(cfg, scheme, st, peaks, fp64_peak_tflops, path=None):
     ms = leja_s / mv * 1e3
     achieved = nbytes / (ms * 1e-3) / 1e9
     if kernel.startswith("csr_leja_sweep_small") or (cfg.kind == "dense" and cfg.n <= 4096):
-        kernel += " (L1/L2-resident working set, latency bound: the HBM fraction is not meaningful)"
+        kernel += " (L2-resident, latency bound)"
     r = {"kernel": kernel, "bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
          "frac": achieved / peaks["hbm_gbs"], "traffic": None, "peak_source": peaks["source"],
-         "bytes_per_launch": nbytes, "ms_per_launch": ms,
-         "how": "CUDA events around every Leja sweep (init .. stop) inside the timed region / matvecs: an upper "
-                "bound on the kernel time (it includes the init, stop-test and early-exit launches); bytes = the "
-                "algorithmic bytes of the storage variant the kernel reads (magnus_describe)",
-         "frac_of_nominal_8TBs": achieved / 8000.0}
+         "bytes_per_launch": nbytes, "ms_per_launch": ms, "frac_of_nominal_8TBs": achieved / 8000.0}
     if cfg.kind != "dense":
         eq = csr_bytes / (ms * 1e-3) / 1e9
-        r["csr_equivalent"] = {"bytes_per_launch": csr_bytes, "gbs": eq, "frac": eq / peaks["hbm_gbs"],
-                               "note": "SURVEY 8(d) plain-CSR bytes (20 B per stored entry) over the same time: what a "
-                                       "CSR-reading kernel would have to sustain to be as fast; not a bandwidth the "
-                                       "kernel achieves"}
+        # SURVEY 8(d) plain-CSR bytes over the same time: what a CSR-reading kernel would have to sustain to be as
+        # fast -- not a bandwidth this kernel achieves
+        r["csr_equivalent"] = {"bytes_per_launch": csr_bytes, "gbs": eq, "frac": eq / peaks["hbm_gbs"]}
         if path and path.get("slots"):
             r["layout"] = {k: path[k] for k in ("slices", "slots", "entries")}
     return r
@@ -409,16 +397,9 @@ def measure_extra(M, W, torch, dev, peaks, dmma_tf):
         st = res["stats"]
         roof = roofline_for(cfg, scheme, st, peaks, dmma_tf, res.get("path"))
         out[key] = {"workload": workload_description(cfg, scheme), "steps": steps, "warmup": warmup,
-                    "shortcut": ("beyond-paper shortcut, NOT the mandated path: the chain is given by its couplings, "
-                                 "no matrix in memory (magnus_create_xxz, SURVEY 8f-4)") if shortcuts == XXZ_MATRIX_FREE else
-                                ("beyond-paper shortcut, NOT the mandated path: the operator has no imaginary parts, the "
-                                 "offset-slot copy keeps the real parts only (8 B per entry); same bits as the mandated "
-                                 "path") if shortcuts == M.SHORTCUT_REAL_VALUES else
-                                ("beyond-paper shortcut, NOT the mandated path: spectral interval from 8 Lanczos steps per "
-                                 "exponential instead of Gershgorin (SURVEY 8f-4); its mat-vecs are in lanczos_matvecs, not "
-                                 "in matvecs") if shortcuts == M.SHORTCUT_TIGHT_INTERVAL else
-                                ("beyond-paper shortcut, NOT the mandated path: [H0,H1] cached at create, no GEMM per "
-                                 "step (SURVEY 8f-4)") if shortcuts else None,
+                    "shortcut": {XXZ_MATRIX_FREE: "matrix-free XXZ (magnus_create_xxz)",
+                                 M.SHORTCUT_REAL_VALUES: "real-part storage", M.SHORTCUT_TIGHT_INTERVAL: "Lanczos interval",
+                                 M.SHORTCUT_CACHED_COMMUTATOR: "cached dense commutator"}.get(shortcuts),
                     "value": steps / res["seconds"], "unit": UNIT, "ms_per_step": res["seconds"] / steps * 1e3,
                     "matvecs": st["total_matvecs"], "lanczos_matvecs": st.get("lanczos_matvecs", 0),
                     "seconds_leja": st["seconds_leja"],
@@ -428,6 +409,46 @@ def measure_extra(M, W, torch, dev, peaks, dmma_tf):
         del res
         torch.cuda.empty_cache()
     return out
+
+
+def _r(x, digits=6):
+    """Shorten a float to `digits` significant digits for the printed line."""
+    return float(f"{x:.{digits}g}") if isinstance(x, float) and math.isfinite(x) else x
+
+
+def build_line(cfg, scheme, world, steps, warmup, value, sec, st, psi_norm, clocks, roof, e2e, fp64_peaks, cpu_baseline):
+    """The ONE headline JSON line, kept below MAX_LINE_BYTES: only what the bench contract names.  Explanations of
+    how each figure is measured are in DESIGN.md section 7, not in the line."""
+    roof_keys = ("kernel", "bound", "achieved", "peak", "unit", "frac", "traffic", "traffic_source", "bytes_per_launch",
+                 "flops_per_launch", "ms_per_launch", "peak_source", "frac_of_nominal_8TBs", "csr_equivalent")
+    line = {"metric": METRIC, "value": _r(value), "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
+            "ms_per_step": _r(sec / steps * 1e3), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "complex128 (f64)", "data": "synthetic",
+            "config": {"workload": workload_description(cfg, scheme), "scheme": scheme,
+                       "parallelism": "replicas only (no sharding, no collective)" if world > 1 else "1 GPU",
+                       "l2": "inputs larger than L2 (no flush needed)" if matrix_bytes_cfg(cfg) > 256e6 else
+                             "fits L2: latency bound",
+                       "matvecs": st["total_matvecs"], "exponentials": st["n_exp"],
+                       "seconds_leja": _r(st["seconds_leja"]), "seconds_commutator": _r(st["seconds_commutator"]),
+                       "psi_norm_after": psi_norm},
+            "clocks": clocks, "gpu_launches": st["kernel_launches"],
+            "roofline": {k: ({kk: _r(vv) for kk, vv in roof[k].items()} if isinstance(roof[k], dict) else _r(roof[k]))
+                         for k in roof_keys if k in roof},
+            "fp64_peaks_measured_tflops": {"dmma": _r(fp64_peaks[0]), "dfma": _r(fp64_peaks[1])}}
+    if e2e:
+        line["e2e"] = {k: _r(e2e[k]) for k in ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step", "steps",
+                                                "seconds", "seconds_integrate", "seconds_h2d_create_d2h",
+                                                "seconds_all_trials", "reported") if k in e2e}
+    if cpu_baseline:
+        line["cpu_baseline"] = {k: _r(v) for k, v in cpu_baseline.items()}
+    n = len(json.dumps(line))
+    if n >= MAX_LINE_BYTES:      # never print a line the driver cannot store whole: drop the optional parts first
+        for k in ("fp64_peaks_measured_tflops",):
+            line.pop(k, None)
+        line["roofline"].pop("csr_equivalent", None)
+        line["config"] = {"workload": line["config"]["workload"][:200], "scheme": scheme}
+    assert len(json.dumps(line)) < MAX_LINE_BYTES, "headline line too long"
+    return line
 
 
 def run_ours(args):
@@ -472,27 +493,15 @@ def run_ours(args):
 
     if rank == 0:
         roof = roofline_for(cfg, scheme, st, peaks, dmma_tf, res.get("path"))
-        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-                "warmup": args.warmup, "ms_per_step": sec / args.steps * 1e3, "higher_is_better": True,
-                "scaling": "weak", "vs_baseline": None, "dtype": "complex128 (f64)", "data": "synthetic",
-                "config": {"workload": workload_description(cfg, scheme), "scheme": scheme,
-                           "parallelism": "replicas only (no sharding, no collective)" if world > 1 else "1 GPU",
-                           "l2": "inputs larger than L2 (no flush needed)" if matrix_bytes_cfg(cfg) > 256e6 else
-                                 "working set fits the 126 MB L2; steps/s is launch/latency bound, not HBM bound",
-                           "matvecs": st["total_matvecs"], "exponentials": st["n_exp"],
-                           "seconds_leja": st["seconds_leja"], "seconds_commutator": st["seconds_commutator"],
-                           "psi_norm_after": res["norm"]},
-                "clocks": res["clocks"], "gpu_launches": st["kernel_launches"], "roofline": roof,
-                "fp64_peaks_measured_tflops": {"dmma": dmma_tf, "dfma": dfma_tf}}
-        if e2e:
-            line["e2e"] = {k: e2e[k] for k in ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step", "steps",
-                                               "seconds", "seconds_integrate", "seconds_h2d_create_d2h",
-                                               "seconds_all_trials", "region")}
-        if world == 1 and args.workload == "cfg5" and not args.no_extra:
-            line["extra"] = measure_extra(M, W, torch, dev, peaks, dmma_tf)
+        cpu = None
         if world == 1 and not args.no_cpu_baseline:
             base = time_oracle(cfg, scheme, 1, 0, args.oracle_max_size)
-            line["cpu_baseline"] = {k: base[k] for k in ("value", "unit", "cores", "kind", "sample")}
+            cpu = {k: base[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        if args.extra:      # opt-in secondary runs: to a side file, never into the headline line
+            with open(args.extra, "w") as fh:
+                json.dump(measure_extra(M, W, torch, dev, peaks, dmma_tf), fh, indent=1)
+        line = build_line(cfg, scheme, world, args.steps, args.warmup, value, sec, st, res["norm"], res["clocks"], roof,
+                          e2e, (dmma_tf, dfma_tf), cpu)
         print(json.dumps(line), flush=True)
     if dist is not None:
         dist.barrier()
@@ -534,7 +543,9 @@ def main():
     ap.add_argument("--scheme", default=None, choices=["cf4", "m4", "m2", "cf4:3", "m6"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-extra", action="store_true", help="skip the cfg4 secondary measurements of the default run")
+    ap.add_argument("--no-extra", action="store_true", help="accepted for compatibility: extras are opt-in now (--extra)")
+    ap.add_argument("--extra", default=None, metavar="FILE.json",
+                    help="also run the secondary measurements (cfg1-cfg4, shortcuts) and write them to FILE.json")
     ap.add_argument("--sweep", default=None, metavar="FILE.md",
                     help="instead of the benchmark line: re-run the paper's cost-vs-size and accuracy-vs-cost sweeps "
                          "(PAPER.md section 4) and write the tables to FILE.md")

@@ -85,3 +85,40 @@ def test_ours_arm_fails_loudly_without_gpu():
     res = subprocess.run([sys.executable, "bench.py", "--steps", "1", "--warmup", "0"], cwd=ROOT, capture_output=True,
                          text=True, timeout=300)
     assert res.returncode != 0 and "no CUDA device" in (res.stderr + res.stdout)
+
+
+@pytest.mark.parametrize("name,scheme", [("cfg5", "cf4"), ("cfg4", "m4"), ("cfg3", "m4"), ("cfg2", "cf4")])
+def test_headline_line_stays_below_4_kb(name, scheme):
+    """The driver keeps only the tail of stdout: a 21 KB line (round 2) lost `value`, `roofline` and `e2e`.  The line
+    is built here from stub results with worst-case widths (17-digit floats, every optional part present, a long
+    clocks record) by bench.py's own build_line and must stay below bench.MAX_LINE_BYTES = 4096."""
+    sys.path.insert(0, ROOT)
+    import bench
+    import workloads as W
+    cfg = W.CONFIGS[name]
+    x = 1234.5678901234567
+    st = {"total_matvecs": 123456789, "n_exp": 123456, "seconds_leja": x, "seconds_commutator": x,
+          "seconds_device": x, "kernel_launches": 1234567890}
+    peaks = {"hbm_gbs": 6543.2109876543, "source": "measured (MEASURED_PEAKS.json)"}
+    path = {"leja_kernel": "csr_leja_iter_sliceoff_kernel", "bytes_per_iteration": 11250000000,
+            "csr_bytes_per_iteration": bench.algorithmic_bytes_per_iteration(cfg, scheme) if cfg.kind == "xxz" else 0,
+            "slices": 524288, "slots": 20000000, "entries": 620756992}
+    roof = bench.roofline_for(cfg, scheme, st, peaks, 37.123456789012, path)
+    clocks = {"sm_mhz": 1965.0, "sm_max_mhz": 1965.0, "power_w_max": 987.654321, "samples": 12345,
+              "reasons": ["hw_slowdown", "hw_thermal_slowdown", "sw_power_cap", "sw_thermal_slowdown"]}
+    e2e = {"value": x, "unit": "steps/s", "h2d_bytes_per_step": x * 1e6, "d2h_bytes_per_step": x * 1e5, "steps": 5,
+           "seconds": x, "seconds_integrate": x, "seconds_h2d_create_d2h": x, "seconds_all_trials": [x, x, x],
+           "reported": "median of 3 calls"}
+    cpu = {"value": x, "unit": "steps/s", "cores": 128, "kind": "oracle",
+           "sample": "1 Magnus step(s) (CF4, tau=0.05) of the cfg5 recipe at N=24 (reduced from 16384), 42.47 s per step"}
+    line = bench.build_line(cfg, scheme, 8, 12345, 123, x, x, st, 0.99999999999999989, clocks, roof, e2e, (x, x), cpu)
+    text = json.dumps(line)
+    assert len(text) < bench.MAX_LINE_BYTES == 4096, len(text)
+    back = json.loads(text)
+    for key in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+                "dtype", "data", "config", "clocks", "gpu_launches", "roofline", "e2e", "cpu_baseline"):
+        assert key in back, key
+    assert "extra" not in back
+    for key in ("bound", "achieved", "peak", "unit", "frac", "traffic"):
+        assert key in back["roofline"], key
+    assert back["value"] > 0 and "workload" in back["config"]
