@@ -44,8 +44,15 @@ __global__ void __launch_bounds__(MS_THREADS, 1)
   unsigned generation = 0;
   for (int k = tid; k <= kMaxDegree; k += MS_THREADS) s_l[k] = leja_l[k];
 
-  // this CTA's (a, b) -> the grid's sum, the same value in every thread of every CTA (fixed order)
-  auto grid_sum2 = [&](double a, double b, int parity, double& ta, double& tb) {
+  // this CTA's (a, b) -> the grid's sum, the same value in every thread of every CTA (fixed order).
+  // The two partials buffers alternate on a counter that runs over ALL calls of the launch (not on the iteration
+  // number): a CTA writes its slot for call c+1 into the buffer call c did not use, and reaches call c+2's write
+  // into call c's buffer only behind barrier c+1, which no CTA passes before it has finished reading for call c.
+  // Keyed on k & 1 instead, a job that stopped at an even k and the next job's init (call "0") shared a buffer with
+  // no barrier in between: a fast CTA could overwrite its slot while a slow one was still summing the stop test.
+  unsigned nsum = 0;
+  auto grid_sum2 = [&](double a, double b, double& ta, double& tb) {
+    const int parity = (int)(nsum++ & 1u);
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
       a += shfl_xor_d(a, o);
@@ -110,7 +117,7 @@ __global__ void __launch_bounds__(MS_THREADS, 1)
       a0 += x.x * x.x + x.y * x.y;
     }
     double s0, dummy;
-    grid_sum2(a0, 0.0, 0, s0, dummy);
+    grid_sum2(a0, 0.0, s0, dummy);
     double e_prev = s_absd[0] * sqrt(s0);
     double err = 0.0, sw = 0.0, sp = 0.0;
     int k = 0, cur = 0;
@@ -157,7 +164,7 @@ __global__ void __launch_bounds__(MS_THREADS, 1)
           __stcg(reinterpret_cast<double2*>(w_out + row), wn);
         }
       }
-      grid_sum2(bw, bp, k & 1, sw, sp);            // S7: one barrier per iteration
+      grid_sum2(bw, bp, sw, sp);                   // S7: one barrier per iteration
       const double e_k = s_absd[k] * sqrt(sw);
       err = e_k + e_prev;
       e_prev = e_k;

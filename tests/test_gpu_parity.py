@@ -790,6 +790,31 @@ def test_medium_csr_sweep_kernel(M, oracle, scheme, N, nsteps):
         assert np.array_equal(out[0][0], out[7][0]) and relerr(out[0][1], out[7][1]) <= 1e-13
 
 
+def test_medium_csr_sweep_many_short_jobs_even_counts(M, oracle):
+    """Stress of the job-to-job hand-over inside ONE cooperative launch: 1200 exponentials of a few iterations each
+    (small tau), most of them stopping at an even degree -- the case in which the stop test of job e and the
+    ||psi||^2 reduction of job e + 1 used to share a partials buffer with no grid barrier in between (a fast CTA could
+    overwrite its slot while a slow one was still summing).  Counts equal to the oracle's, psi <= 1e-9, and three
+    runs give the same bits."""
+    N, nsteps = 11, 600
+    cfg = W.scaled(W.CONFIGS["cfg3"], N, nsteps)
+    H0, H1, psi0, f = W.build(cfg)
+    t_end = cfg.t0 + nsteps * 1e-3          # 6 iterations per exponential at this tau
+    ref, riters = oracle.magnus_integrate(oracle.CsrHost.of(H0), oracle.CsrHost.of(H1), f, "cf4", cfg.t0, t_end, nsteps,
+                                          psi0.numpy(), cfg.tol)
+    assert np.count_nonzero(np.asarray(riters) % 2 == 0) >= len(riters) // 2
+    outs = []
+    with M.magnus_create(H0.to(DEV), H1.to(DEV), f, "cf4", tol=cfg.tol) as h:
+        assert h.describe()["leja_kernel"] == "csr_leja_sweep_mid_kernel"
+        for _ in range(3):
+            psi = psi0.to(DEV).clone()
+            st = h.integrate(cfg.t0, t_end, nsteps, psi)
+            assert np.array_equal(st["iters"], riters)
+            outs.append(host(psi))
+    assert relerr(outs[0], ref) <= 1e-9
+    assert np.array_equal(outs[0], outs[1]) and np.array_equal(outs[0], outs[2])
+
+
 def test_medium_csr_sweep_general_matrix_and_expmv(M, oracle):
     """The same kernel on a general (non-XXZ) Hermitian CSR matrix with empty and long rows, through leja_expmv
     (one-job launch, out != in), and its non-convergence report (input untouched when in place)."""
