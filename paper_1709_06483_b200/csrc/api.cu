@@ -249,8 +249,14 @@ static int expmv_on_interval(const OpRef& op, double a_raw, double b_raw, const 
         ++k;
         need(k);
         const double shift = c_over_gamma + l[k - 1];
-        launch_iter(op, ws->w[(k - 1) & 1], ws->w[k & 1], ws->p, inv_gamma, shift,
-                    make_double2(d[k].real(), d[k].imag()), std::abs(d[k]), prm.tol, ws, st);
+        if (launch_iter(op, ws->w[(k - 1) & 1], ws->w[k & 1], ws->p, inv_gamma, shift,
+                        make_double2(d[k].real(), d[k].imag()), std::abs(d[k]), prm.tol, ws, st) < 0) {
+          // nothing was launched (a csr_kernel tuning code outside the launch tables): without this the host would
+          // poll an unchanged status up to m_max and report a misleading ENOCONV
+          set_error("csr_kernel = %d selects no kernel for this operator (valid: 0 auto, 1 generic, 2 row-block, 3, 4, "
+                    "5, 6 offset-slot, 7 sweep, or a tuning code listed in the kernel sources)", ws->csr_kernel);
+          return MAGNUS_EINVAL;
+        }
       }
       CU_TRY(cudaGetLastError());   // a failed launch must surface as ECUDA, not as ENOCONV at m_max
       if (ws->time_leja) CU_TRY(cudaEventRecord(ws->ev[1], st));
@@ -755,13 +761,21 @@ static int magnus_step_unplanned(magnus_context* h, double t, double tau, cplx* 
         };
         term(0, H0v, 1.0, 0.0); term(1, H1v, f2, 0.0); term(2, nullptr, 0.0, 0.0); term(3, nullptr, 0.0, 0.0);
         if (dense_ld(&h->H0) != n || dense_ld(&h->H1) != n) { set_error("MAGNUS_M6 needs ld == n"); rc = MAGNUS_EINVAL; break; }
+        if (tau == 0.0) {   // Omega_H carries b3 / (12 tau) and 1 / (240 tau); a zero step is the identity anyway
+          set_error("MAGNUS_M6: tau must be non-zero");
+          rc = MAGNUS_EINVAL;
+          break;
+        }
+        auto gemm_failed = [&](const char* which) {
+          set_error("MAGNUS_M6: zgemm launch of %s failed: %s", which, cudaGetErrorString(cudaGetLastError()));
+        };
         launch_dense_lincomb(n, h->M, lc, ws, st);                                   // X1 = H2 = H0 + f2 H1
         if (h->time_comm) cudaEventRecord(h->ev_comm[0], st);
         rc = launch_zgemm(n, h->M, n, H1v, n, h->A2, n, st, &h->zs);                          // X2 = P1 = H2 H1
-        if (rc) break;
+        if (rc) { gemm_failed("P1 = H2 H1"); break; }
         launch_dense_antiherm(n, h->A2, h->P, -1.0, st);                              // X3 = G = P1 - P1^H = [H2, H1]
         rc = launch_zgemm(n, h->M, n, h->P, n, h->A2, n, st, &h->zs);                         // X2 = P2 = H2 G
-        if (rc) break;
+        if (rc) { gemm_failed("P2 = H2 G"); break; }
         launch_dense_antiherm(n, h->A2, h->X4, 1.0, st);                              // X4 = S = P2 + P2^H = [H2, G]
         term(0, h->M, 0.0, 20.0 * tau); term(1, H1v, 0.0, b3); term(2, h->P, -tau * b2, 0.0); term(3, nullptr, 0.0, 0.0);
         launch_dense_lincomb(n, h->A2, lc, ws, st);                                  // X2 = L
@@ -769,9 +783,9 @@ static int magnus_step_unplanned(magnus_context* h, double t, double tau, cplx* 
         term(3, nullptr, 0.0, 0.0);
         launch_dense_lincomb(n, h->X5, lc, ws, st);                                  // X5 = R
         rc = launch_zgemm(n, h->A2, n, h->X5, n, h->X4, n, st, &h->zs);                       // X4 = P3 = L R
-        ws->launches += 5;
+        ws->launches += 5;      // 3 GEMMs + 2 antiherm (the 3 lincomb launches count themselves, the omega launch below too)
         if (h->time_comm) cudaEventRecord(h->ev_comm[1], st);
-        if (rc) break;
+        if (rc) { gemm_failed("P3 = L R"); break; }
         // Omega_H = H2 + (b3/(12 tau)) H1 + (i/(240 tau)) (P3 - P3^H), over X1, with its Gershgorin bounds
         nblk = launch_dense_omega(n, h->M, H1v, h->X4, 1.0, b3 / (12.0 * tau), -1.0 / (240.0 * tau), ws, st);
       } else if (h->scheme == MAGNUS_M4 && h->cached_p0) {
@@ -1047,6 +1061,11 @@ int magnus_create(magnus_handle* out, const magnus_matrix* H0, const magnus_matr
       cudaEventCreate(&h->ev_comm[0]);
       cudaEventCreate(&h->ev_comm[1]);
       h->time_comm = true;
+    }
+    if (scheme == MAGNUS_M6 && (dense_ld(&h->H0) != h->n || dense_ld(&h->H1) != h->n)) {
+      set_error("MAGNUS_M6 needs dense H0, H1 with ld == n (the products read them as n x n blocks)");
+      magnus_destroy(h);
+      return MAGNUS_EINVAL;
     }
     if (scheme == MAGNUS_M4 && (h->shortcuts & MAGNUS_SHORTCUT_CACHED_COMMUTATOR)) {
       if (dense_ld(H0) != h->n || dense_ld(H1) != h->n) {
@@ -1388,8 +1407,10 @@ int magnus_leja_iteration(const magnus_matrix* H0, const magnus_matrix* H1, doub
   if (rc == MAGNUS_OK) {
     cudaMemsetAsync(ws.status, 0, sizeof(LejaStatus), st);
     cudaEventRecord(ws.ev[0], st);
+    bool launched = true;
     for (int r = 0; r < reps; ++r)   // |d_k| = 1, tol = 0: the fused stop test only records the norms
-      launch_iter(op, (const cplx*)w_in, (cplx*)w_out, (cplx*)p, inv_gamma, shift, make_double2(d_re, d_im), 1.0, 0.0, &ws, st);
+      launched = launched && launch_iter(op, (const cplx*)w_in, (cplx*)w_out, (cplx*)p, inv_gamma, shift,
+                                         make_double2(d_re, d_im), 1.0, 0.0, &ws, st) >= 0;
     cudaEventRecord(ws.ev[1], st);
     cudaMemcpyAsync(ws.status_host, ws.status, sizeof(LejaStatus), cudaMemcpyDeviceToHost, st);
     cudaError_t ke = cudaStreamSynchronize(st);
@@ -1398,6 +1419,9 @@ int magnus_leja_iteration(const magnus_matrix* H0, const magnus_matrix* H1, doub
       set_error("magnus_leja_iteration: kernel failed: %s", cudaGetErrorString(ke));
       cudaGetLastError();
       rc = MAGNUS_ECUDA;
+    } else if (!launched) {
+      set_error("magnus_leja_iteration: csr_kernel = %d selects no kernel for this operator", csr_kernel);
+      rc = MAGNUS_EINVAL;
     } else {
       float ms = 0.f;
       cudaEventElapsedTime(&ms, ws.ev[0], ws.ev[1]);

@@ -528,6 +528,42 @@ def test_m6_is_more_accurate_than_m4_and_refuses_large_csr(M):
     assert ei.value.code == -1
 
 
+def test_argument_errors_surface_as_einval_not_as_enoconv(M):
+    """Three misuse cases that used to fail late or misleadingly: (1) MAGNUS_M6 on strided dense input is refused at
+    create (it failed at every step); (2) an M6 step with tau = 0 (Omega_H divides by tau) is EINVAL; (3) a csr_kernel
+    tuning code outside the launch tables launches nothing -- the call reports EINVAL naming the code instead of
+    polling up to m_max and returning ENOCONV."""
+    n = 96
+    cfg = W.scaled(W.CONFIGS["cfg2"], n, 1)
+    H0, H1, psi0, f = W.build(cfg, device=DEV)
+    wide0 = torch.zeros((n, n + 3), dtype=torch.complex128, device=DEV)
+    wide1 = torch.zeros_like(wide0)
+    wide0[:, :n], wide1[:, :n] = H0, H1
+    with pytest.raises(M.MagnusError) as e:
+        M.magnus_create(wide0[:, :n], wide1[:, :n], f, "m6")
+    assert e.value.code == -1 and "ld == n" in str(e.value)
+    with M.magnus_create(H0, H1, f, "m6") as h:
+        psi = psi0.clone()
+        with pytest.raises(M.MagnusError) as e:
+            h.step(0.0, 0.0, psi)
+        assert e.value.code == -1 and "tau" in str(e.value)
+        assert torch.equal(psi, psi0)
+        h.step(0.0, 0.01, psi)                                   # the handle is still usable
+        assert abs(float(torch.linalg.vector_norm(psi)) - 1) < 1e-10
+    big = W.scaled(W.CONFIGS["cfg3"], 12, 1)
+    B0, B1, p0, fb = W.build(big, device=DEV)
+    w, wo, p = p0.clone(), torch.zeros_like(p0), p0.clone()
+    for code in (6013, 5077):
+        with pytest.raises(M.MagnusError) as e:
+            M.magnus_leja_iteration(B0, B1, 0.3, w, wo, p, 0.1, 0.2, 0.5 + 0.1j, csr_kernel=code)
+        assert e.value.code == -1 and str(code) in str(e.value)
+        with M.magnus_create(B0, B1, fb, "cf4", csr_kernel=code) as h:
+            psi = p0.clone()
+            with pytest.raises(M.MagnusError) as e:
+                h.step(0.0, 0.05, psi)
+            assert e.value.code == -1 and str(code) in str(e.value)
+
+
 # ------------------------------------------------------------------ shortcut (SURVEY 8f-4): cached dense commutator
 @pytest.mark.parametrize("n,nsteps", [(200, 5), (515, 3), (2048, 2)])
 def test_shortcut_cached_dense_commutator_vs_oracle(M, oracle, n, nsteps):
