@@ -106,7 +106,9 @@ typedef struct magnus_options {
  * matrix 20x to 57x and so costs 1.6-3x more Leja iterations.  With this bit the interval of every exponential of
  * magnus_step / magnus_integrate comes from lanczos_steps steps of the Lanczos process on the exponentiated matrix,
  * started at the current psi:  [theta_min(T) - beta_m, theta_max(T) + beta_m]  (extreme Ritz values widened by the
- * norm of the last residual), then snapped as usual (reading ti).  Costs lanczos_steps extra mat-vecs per
+ * norm of the last residual), intersected with the Gershgorin interval (the estimate is not an enclosure and may
+ * stick out of it), then snapped as usual (reading ti).  If it undershoots the spectrum badly the interpolation can
+ * fail with MAGNUS_ENOCONV; there is no automatic retry -- repeat the step on a handle without this bit.  Costs lanczos_steps extra mat-vecs per
  * exponential (magnus_stats.lanczos_matvecs); the interval now depends on psi, so steps are not planned ahead. */
 #define MAGNUS_SHORTCUT_TIGHT_INTERVAL 2
 

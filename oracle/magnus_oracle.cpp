@@ -392,8 +392,17 @@ int leja_expmv(const Matrix& M, const cplx* v_in, cplx* v_out, double h, double 
   const int64_t n = M.n;
   const std::vector<double>& l = leja_table();
   double a, b;
-  if (g_lanczos_steps <= 0 || lanczos_interval(M, v_in, g_lanczos_steps, &a, &b, nullptr, nullptr) == 0)
-    M.gershgorin(&a, &b);
+  M.gershgorin(&a, &b);
+  if (g_lanczos_steps > 0) {
+    // reading ti: the Lanczos interval is an ESTIMATE (P:190 asks for no more), not an enclosure, and its widening by
+    // beta_m can stick out of the Gershgorin enclosure; the spectrum lies in both only where they overlap, so the
+    // interval used is their intersection (Gershgorin alone when Lanczos declines or the two do not overlap).
+    double la, lb;
+    if (lanczos_interval(M, v_in, g_lanczos_steps, &la, &lb, nullptr, nullptr) != 0) {
+      const double ia = std::max(a, la), ib = std::min(b, lb);
+      if (ia <= ib) { a = ia; b = ib; }
+    }
+  }
   snap_interval(&a, &b);
   const double c = 0.5 * (a + b);
   const double gamma = 0.25 * (b - a);

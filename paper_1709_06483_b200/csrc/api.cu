@@ -822,8 +822,13 @@ static int magnus_step_unplanned(magnus_context* h, double t, double tau, cplx* 
       double ta = 0.0, tb = 0.0;
       rc = lanczos_interval(h, op, psi, &ta, &tb);
       if (rc == MAGNUS_OK) {
-        a = ta;
-        b = tb;
+        // the Lanczos interval is an estimate, not an enclosure: never let it reach beyond the Gershgorin
+        // enclosure [a, b] on either side (reading ti); disjoint (cannot happen in exact arithmetic): keep [a, b]
+        const double ia = std::max(a, ta), ib = std::min(b, tb);
+        if (ia <= ib) {
+          a = ia;
+          b = ib;
+        }
       } else if (rc == kPlanDeclined) {
         rc = MAGNUS_OK;       // psi = 0: nothing to estimate from, the Gershgorin interval stays
       } else {

@@ -78,3 +78,32 @@ def test_expmv_on_the_tight_interval(kind, size):
         assert info_t["iters"] <= info_g["iters"] and info_t["b"] - info_t["a"] <= info_g["b"] - info_g["a"]
     out_again, info_again = O.leja_expmv(M, v, 0.3, 1e-12)                          # the mode is off again outside the block
     assert info_again["a"] == O.gershgorin(M)[1][0]
+
+
+def test_tight_interval_never_reaches_beyond_gershgorin():
+    """Reading ti: the Lanczos interval [theta_min - beta_m, theta_max + beta_m] is an estimate, not an enclosure; on a
+    DIAGONAL matrix Gershgorin is exact, so every bit of the widening by beta_m lies outside the spectrum.  The interval
+    leja_expmv uses in tight mode is the intersection: equal to Gershgorin's where Lanczos sticks out, tighter where
+    the start vector does not see a part of the spectrum -- and the result is still exp(-ihM)v."""
+    n = 64
+    d = np.linspace(-1.0, 1.0, n)
+    M = np.diag(d).astype(complex)
+    r = np.random.default_rng(11)
+    v = r.normal(size=n) + 1j * r.normal(size=n)
+    v /= np.linalg.norm(v)
+    (la, lb), _, _ = O.lanczos_interval(M, v, 8)
+    assert la < -1.0 and lb > 1.0                              # the raw estimate does stick out on both sides
+    _, info_g = O.leja_expmv(M, v, 0.7, 1e-12)
+    with O.tight_interval(8):
+        out, info_t = O.leja_expmv(M, v, 0.7, 1e-12)
+    assert info_t["a"] == info_g["a"] and info_t["b"] == info_g["b"]
+    assert np.linalg.norm(out - np.exp(-0.7j * d) * v) <= 1e-12
+    v2 = v.copy()
+    v2[n // 2:] = 0.0                                          # sees only the eigenvalues in [-1, -1/63]
+    v2 /= np.linalg.norm(v2)
+    (la2, lb2), _, _ = O.lanczos_interval(M, v2, 8)
+    assert la2 < -1.0 and lb2 < 0.5
+    with O.tight_interval(8):
+        out2, info_2 = O.leja_expmv(M, v2, 0.7, 1e-12)
+    assert info_2["a"] == info_g["a"] and info_2["b"] < info_g["b"]
+    assert np.linalg.norm(out2 - np.exp(-0.7j * d) * v2) <= 1e-12
