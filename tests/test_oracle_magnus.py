@@ -231,6 +231,39 @@ def test_single_step_matches_scheme_formula_with_exact_exponentials(oracle):
     assert np.linalg.norm(got_m4 - ref_m4) < 1e-11
 
 
+def test_single_step_cf43_and_m2_match_printed_products_with_exact_exponentials(oracle):
+    """One Cf4:3 step against the printed product (nodes 1/2, 1/2 -+ sqrt(15)/10, the 3 x 3
+    alpha table, the factor of row 3 acting first) and one M2 step against exp(tau A(t + tau/2)) (lines 87-95), both
+    with eigendecomposition exponentials of A = -iH.  A swapped row order, a transposed alpha or a wrong node fails
+    here at O(tau^3) ~ 1e-3, far above the bar."""
+    n = 10
+    H0, H1 = rand_herm(n, 23, 0.5), rand_herm(n, 24, 0.5)
+    f = lambda t: math.sin(3 * t)
+    psi0 = rand_vec(n, 25)
+    t, tau = 0.4, 0.2
+    s15 = math.sqrt(15.0)
+    c = (0.5 - s15 / 10, 0.5, 0.5 + s15 / 10)
+    A = [-1j * (H0 + f(t + ci * tau) * H1) for ci in c]
+    p, m = 37 / 240 + 10 * s15 / 261, 37 / 240 - 10 * s15 / 261
+    alpha = np.array([[m, -1 / 30, p], [-11 / 360, 23 / 45, -11 / 360], [p, -1 / 30, m]])
+
+    def expm_general(X):            # X = -i * Hermitian
+        return expm_h(1j * X, 1.0)
+
+    y = psi0
+    for row in (2, 1, 0):           # exp(Omega^(1)) exp(Omega^(2)) exp(Omega^(3)) Y_n: the third factor acts first
+        y = expm_general(tau * sum(alpha[row, j] * A[j] for j in range(3))) @ y
+    got, infos = oracle.magnus_step(H0, H1, f, "cf4:3", t, tau, psi0)
+    assert len(infos) == 3 and np.linalg.norm(got - y) < 1e-11
+    wrong = psi0
+    for row in (0, 1, 2):           # negative control: the factors in the other order differ at O(tau^3)
+        wrong = expm_general(tau * sum(alpha[row, j] * A[j] for j in range(3))) @ wrong
+    assert np.linalg.norm(wrong - y) > 1e-6
+    ref_m2 = expm_general(tau * (-1j) * (H0 + f(t + tau / 2) * H1)) @ psi0
+    got_m2, infos = oracle.magnus_step(H0, H1, f, "m2", t, tau, psi0)
+    assert len(infos) == 1 and np.linalg.norm(got_m2 - ref_m2) < 1e-11
+
+
 def test_cfg1_totals_are_stable(oracle):
     """CFG1 end to end on the oracle: norm conserved to 1e-10 (north_star), CF4 and M4
     agree to O(tau^4); the iteration totals are recorded in tests/golden by
