@@ -509,8 +509,8 @@ def run_ours(args):
 
 
 def run_sweep(args):
-    """The paper's sweeps (paper_1709_06483_b200/sweeps.py) with the oracle timed beside the sizes it affords."""
-    from paper_1709_06483_b200 import sweeps
+    """The paper's sweeps (bench_sweeps.py, beside this file: a measurement harness, not part of the package) with the oracle timed beside the sizes it affords."""
+    import bench_sweeps as sweeps
     from oracle import oracle as O
 
     def cpu_timer(example, N, H0, H1, psi0, f, tau, tol):

@@ -1,4 +1,4 @@
-"""The paper's own sweeps re-run on B200: `python -m paper_1709_06483_b200.sweeps --out FILE.md`.
+"""The paper's own sweeps re-run on B200: `python bench_sweeps.py --out FILE.md`.
 
   * cost against problem size at tau = 1e-3 for Example 1 (non-local Heisenberg, stored dense, Figs. 2-3)
     and Example 2 (local Heisenberg, CSR, Figs. 5-6), for M2, M4, M6, Cf4, Cf4:3;
@@ -7,7 +7,7 @@
 
 Timings are CUDA-event seconds of `magnus_integrate` (inputs resident, one warm-up run); the paper's figure data is
 not available, so this is a re-run, not a comparison.  `bench.py --sweep FILE.md` runs the same sweeps with the CPU
-oracle (test infrastructure, which this package never imports) timed beside the sizes it affords, through the
+oracle (test infrastructure, which this file never imports) timed beside the sizes it affords, through the
 `cpu_timer` callback.  Marshalling only: every number comes from the C-ABI library.
 """
 from __future__ import annotations
@@ -18,7 +18,7 @@ import os
 import sys
 import time
 
-ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
@@ -114,7 +114,7 @@ def main():
     ap.add_argument("--out", required=True)
     ap.add_argument("--quick", action="store_true", help="small sizes only (a few seconds)")
     args = ap.parse_args()
-    cmd = f"python -m paper_1709_06483_b200.sweeps --out {args.out}{' --quick' if args.quick else ''}"
+    cmd = f"python bench_sweeps.py --out {args.out}{' --quick' if args.quick else ''}"
     print("\n".join(run_all(args.out, None, args.quick, cmd)))
 
 
