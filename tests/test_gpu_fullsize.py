@@ -302,3 +302,61 @@ def test_cfg3_m4_late_step_vs_oracle(M, oracle):
     assert info[0]["a"] == rinfo[0]["a"] and info[0]["b"] == rinfo[0]["b"] and info[0]["theta"] == rinfo[0]["theta"]
     got = host(psi)
     assert np.linalg.norm(got - ref) / np.linalg.norm(ref) <= 1e-9
+
+
+# ------------------------------------------------------------------ whole integrations against the stored oracle runs
+def _golden_full_files():
+    import glob
+    import os
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    return sorted(os.path.basename(p) for p in glob.glob(os.path.join(here, "*_full.json")))
+
+
+@pytest.mark.parametrize("fname", _golden_full_files())
+def test_whole_integration_vs_stored_oracle_run(M, fname):
+    """ALL K steps of a BASELINE config through the C-ABI against the oracle's whole run, stored by
+    tests/golden/make_golden_full.py (oracle + workloads only; wall time in the file): every per-exponential iteration
+    count exactly, every snapped interval and theta bit for bit, psi_K at 1024 seeded indices element by element to
+    1e-9 ||psi_K|| (north_star's bar), and ||psi_K||.  Run twice: step by step (magnus_step, which reports the
+    intervals) and in one magnus_integrate call (the call bench.py times); the two must also agree with each other.
+    Inputs: the matrices are generated on the device (exact values), psi0 on the host exactly as the generator did."""
+    import json
+    import os
+    with open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", fname)) as fh:
+        G = json.load(fh)
+    cfg = W.CONFIGS[G["config"]]
+    scheme = G["scheme"]
+    assert cfg.n == G["n"] and cfg.nsteps == G["nsteps"] and cfg.tol == G["tol"]
+    if cfg.kind == "xxz":
+        H0, H1, _, f = W.build(cfg, device=DEV)
+        psi0 = W.xxz.neel_state(cfg.size) if cfg.psi0 == "neel" else rng.random_unit_vector(cfg.n)
+    else:
+        H0, H1, psi0, f = W.build(cfg)
+        H0, H1 = H0.to(DEV), H1.to(DEV)
+    psi0 = psi0.to(DEV)
+    tau = (cfg.t_end - cfg.t0) / cfg.nsteps
+    idx = torch.tensor(G["sample_index"], dtype=torch.int64, device=DEV)
+    want = np.array(G["sample_re"]) + 1j * np.array(G["sample_im"])
+    with M.magnus_create(H0, H1, f, scheme, tol=cfg.tol) as h:
+        psi = psi0.clone()
+        iters, a_hex, b_hex, th_hex = [], [], [], []
+        for s in range(cfg.nsteps):
+            for i in h.step(cfg.t0 + s * tau, tau, psi):
+                iters.append(i["iters"])
+                a_hex.append(float(i["a"]).hex())
+                b_hex.append(float(i["b"]).hex())
+                th_hex.append(float(i["theta"]).hex())
+        assert iters == G["iters"]
+        assert a_hex == G["a_hex"] and b_hex == G["b_hex"] and th_hex == G["theta_hex"]
+        norm = float(torch.linalg.vector_norm(psi))
+        assert abs(norm - G["norm"]) <= 1e-10
+        got = host(psi[idx])
+        assert np.max(np.abs(got - want)) <= 1e-9 * G["norm"]                       # element by element
+        assert np.linalg.norm(got - want) <= 1e-9 * np.linalg.norm(want)            # the sample as a vector
+        psi2 = psi0.clone()
+        st = h.integrate(cfg.t0, cfg.t_end, cfg.nsteps, psi2)
+        assert list(st["iters"]) == G["iters"]
+        got2 = host(psi2[idx])
+        assert np.linalg.norm(got2 - want) <= 1e-9 * np.linalg.norm(want)
+        assert np.max(np.abs(got2 - want)) <= 1e-9 * G["norm"]
+        assert float(torch.linalg.vector_norm(psi2 - psi)) <= 1e-12 * norm
